@@ -1,0 +1,243 @@
+"""fp64 CPU oracle for the demagnetizing-field convolution -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Python face of ``oracle/demag_oracle.c`` (ctypes) plus the few oracle pieces that are one-liners in
+NumPy.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this module; the CUDA path never does, and this module never
+imports ``paper_2308_08447_b200``.
+
+Citations are ``PAPER.md:<line>`` (arXiv 2308.08447) or a DESIGN.md reading (R<n>).
+
+    tensor_table        N over non-negative offsets (R1, R4)          [C]
+    direct_sum          O-A, Eq. (1) written out                   [C]
+    direct_sum_sampled  O-S, Eq. (1) at chosen cells                                [C]
+    naive_dft_conv      O-B, padded convolution via O(N^2) DFTs    [C]
+    fft_conv            O-C, the same through numpy.fft (library cross-check)       [NumPy]
+    energy              E = -(mu0/2) V_cell sum M.H (R12)                            [NumPy]
+    macrocell_average   Eq. (9) (R13)                              [NumPy]
+    macrocell_scatter   "applied equally to all spins" (R14)           [NumPy]
+
+All of them are pinned in tests/test_oracle_pins.py; none is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "demag_oracle.c")
+_LIB = os.path.join(_HERE, "libdemag_oracle.so")
+
+MU0 = 4.0e-7 * np.pi           # vacuum permeability, T m / A
+MU_B = 9.2740100783e-24        # Bohr magneton, J / T  (= A m^2)
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the C oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        d, i = ctypes.c_double, ctypes.c_int
+        lib.oracle_newell_N.argtypes = [d, d, d, d, d, d, _dp]
+        lib.oracle_quad_N.argtypes = [d, d, d, d, d, d, i, _dp]
+        lib.oracle_N_at.argtypes = [d, d, d, d, d, d, _dp]
+        lib.oracle_tensor_table.argtypes = [i, i, i, d, d, d, _dp]
+        lib.oracle_direct_sum.argtypes = [i, i, i, _dp, _dp, _dp]
+        lib.oracle_direct_sum_sampled.argtypes = [i, i, i, _dp, _dp, i,
+                                                  ctypes.POINTER(ctypes.c_longlong), _dp]
+        lib.oracle_naive_dft_conv.argtypes = [i, i, i, i, i, i, _dp, _dp, _dp]
+        lib.oracle_naive_dft_conv.restype = i
+        lib.oracle_kernel_spectrum_imag_ratio.argtypes = [i, i, i, i, i, i, _dp]
+        lib.oracle_kernel_spectrum_imag_ratio.restype = d
+        lib.oracle_num_threads.restype = i
+        _lib = lib
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(_dp)
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def _n6(fn, *args) -> np.ndarray:
+    out = np.empty(6, dtype=np.float64)
+    fn(*args, _p(out))
+    return out
+
+
+def newell_N(r, h) -> np.ndarray:
+    """Closed-form N (xx,yy,zz,xy,xz,yz) at offset r [m] for cell h [m] (R1)."""
+    return _n6(_load().oracle_newell_N, *map(float, r), *map(float, h))
+
+
+def quad_N(r, h, m: int = 3) -> np.ndarray:
+    """Integral definition of N by m-point Gauss-Legendre per half axis (R4)."""
+    lib = _load()
+    out = np.empty(6, dtype=np.float64)
+    lib.oracle_quad_N(*map(float, r), *map(float, h), int(m), _p(out))
+    return out
+
+
+def N_at(r, h) -> np.ndarray:
+    """N as the oracle uses it: Newell near, quadrature far (R4)."""
+    return _n6(_load().oracle_N_at, *map(float, r), *map(float, h))
+
+
+def tensor_table(n, h) -> np.ndarray:
+    """T[6][nz][ny][nx] = N_c(d*h) over non-negative cell offsets d (scope row a0)."""
+    nx, ny, nz = map(int, n)
+    T = np.empty((6, nz, ny, nx), dtype=np.float64)
+    _load().oracle_tensor_table(nx, ny, nz, *map(float, h), _p(T))
+    return T
+
+
+def _check(T, M):
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    M = np.ascontiguousarray(M, dtype=np.float64)
+    assert T.ndim == 4 and T.shape[0] == 6 and M.ndim == 4 and M.shape[0] == 3
+    assert T.shape[1:] == M.shape[1:], (T.shape, M.shape)
+    nz, ny, nx = M.shape[1:]
+    return T, M, nx, ny, nz
+
+
+def direct_sum(T, M) -> np.ndarray:
+    """O-A: H_i = -sum_j N(i-j) M_j for every cell (Eq. (1))."""
+    T, M, nx, ny, nz = _check(T, M)
+    H = np.empty_like(M)
+    _load().oracle_direct_sum(nx, ny, nz, _p(T), _p(M), _p(H))
+    return H
+
+
+def direct_sum_sampled(T, M, cells) -> np.ndarray:
+    """O-S: Eq. (1) at flat cell indices ``cells`` ((iz*ny+iy)*nx+ix); returns [len(cells)][3]."""
+    T, M, nx, ny, nz = _check(T, M)
+    cells = np.ascontiguousarray(cells, dtype=np.int64)
+    Hs = np.empty((len(cells), 3), dtype=np.float64)
+    _load().oracle_direct_sum_sampled(nx, ny, nz, _p(T), _p(M), len(cells),
+                                      cells.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)), _p(Hs))
+    return Hs
+
+
+def padded_shape(n, pbc=(False, False, False)):
+    """P_a = 2 n_a for an open axis with n_a > 1, else n_a (R6)."""
+    return tuple(int(na) if (na == 1 or p) else 2 * int(na) for na, p in zip(n, pbc))
+
+
+def naive_dft_conv(T, M, P=None) -> np.ndarray:
+    """O-B: zero-padded convolution through O(N^2) DFTs."""
+    T, M, nx, ny, nz = _check(T, M)
+    Px, Py, Pz = P if P is not None else padded_shape((nx, ny, nz))
+    H = np.empty_like(M)
+    rc = _load().oracle_naive_dft_conv(nx, ny, nz, Px, Py, Pz, _p(T), _p(M), _p(H))
+    if rc != 0:
+        raise ValueError(f"oracle_naive_dft_conv failed: {rc}")
+    return H
+
+
+def kernel_spectrum_imag_ratio(T, P=None) -> float:
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    nz, ny, nx = T.shape[1:]
+    Px, Py, Pz = P if P is not None else padded_shape((nx, ny, nz))
+    return float(_load().oracle_kernel_spectrum_imag_ratio(nx, ny, nz, Px, Py, Pz, _p(T)))
+
+
+# parity of component c along (x, y, z): diagonal even; xy odd in x,y; xz odd in x,z; yz odd in y,z
+PARITY = np.array([[1, 1, 1], [1, 1, 1], [1, 1, 1], [-1, -1, 1], [-1, 1, -1], [1, -1, -1]])
+# (row, col) -> component index of the symmetric 3x3 tensor
+COMP = np.array([[0, 3, 4], [3, 1, 5], [4, 5, 2]])
+
+
+def padded_kernel(T, P=None) -> np.ndarray:
+    """K[6][Pz][Py][Px]: N(s(d)) with s_a = d_a (d_a<n_a), d_a-P_a (d_a>n_a), 0 at d_a=n_a (R6)."""
+    T = np.asarray(T, dtype=np.float64)
+    nz, ny, nx = T.shape[1:]
+    Px, Py, Pz = P if P is not None else padded_shape((nx, ny, nz))
+    K = np.zeros((6, Pz, Py, Px))
+    for c in range(6):
+        A = T[c]
+        for axis, (na, Pa, par) in enumerate(zip((nz, ny, nx), (Pz, Py, Px), PARITY[c][::-1])):
+            if Pa == na:
+                continue
+            shp = list(A.shape)
+            shp[axis] = Pa
+            B = np.zeros(shp)
+            sl = [slice(None)] * 3
+            sl[axis] = slice(0, na)
+            B[tuple(sl)] = A
+            src = [slice(None)] * 3
+            src[axis] = slice(na - 1, 0, -1)         # offsets -(na-1) .. -1 -> slots Pa-na+1 .. Pa-1
+            dst = [slice(None)] * 3
+            dst[axis] = slice(Pa - na + 1, Pa)
+            B[tuple(dst)] = par * A[tuple(src)]
+            A = B
+        K[c] = A
+    return K
+
+
+def fft_conv(T, M, P=None) -> np.ndarray:
+    """O-C: the same padded convolution through numpy.fft (a library routine the path reduces to);
+    a cross-check validated against O-A/O-B on small grids, not the authority."""
+    T = np.asarray(T, dtype=np.float64)
+    M = np.asarray(M, dtype=np.float64)
+    nz, ny, nx = M.shape[1:]
+    Px, Py, Pz = P if P is not None else padded_shape((nx, ny, nz))
+    s = (Pz, Py, Px)
+    Mh = [np.fft.rfftn(M[b], s=s, axes=(0, 1, 2)) for b in range(3)]
+    H = np.empty_like(M)
+    Kh = {}
+    for a in range(3):
+        acc = 0
+        for b in range(3):
+            c = int(COMP[a, b])
+            if c not in Kh:
+                Kh[c] = np.fft.rfftn(_padded_one(T[c], c, (Px, Py, Pz)), s=s, axes=(0, 1, 2))
+            acc = acc + Kh[c] * Mh[b]
+        H[a] = -np.fft.irfftn(acc, s=s, axes=(0, 1, 2))[:nz, :ny, :nx]
+    return H
+
+
+def _padded_one(Tc, c, P):
+    """padded_kernel for a single component (avoids building all six at once)."""
+    T6 = np.zeros((6,) + Tc.shape)
+    T6[c] = Tc
+    return padded_kernel(T6, P)[c]
+
+
+def energy(M, H, h) -> float:
+    """E = -(mu0/2) V_cell sum_i M_i . H_i  (R12; formula not printed in the paper)."""
+    M = np.asarray(M, dtype=np.float64)
+    H = np.asarray(H, dtype=np.float64)
+    return float(-0.5 * MU0 * float(np.prod(h)) * np.sum(M * H))
+
+
+def macrocell_average(S, c, mu_s, a) -> np.ndarray:
+    """Eq. (9): M_cell = mu_B mu_s sum(S_hat) / (cx cy cz a^3)  [A/m]  (R13).
+    S: unit spins [3][Lz][Ly][Lx]; c = (cx, cy, cz) spins per macrocell edge."""
+    S = np.asarray(S, dtype=np.float64)
+    cx, cy, cz = map(int, c)
+    _, Lz, Ly, Lx = S.shape
+    assert Lx % cx == 0 and Ly % cy == 0 and Lz % cz == 0
+    R = S.reshape(3, Lz // cz, cz, Ly // cy, cy, Lx // cx, cx).sum(axis=(2, 4, 6))
+    return R * (MU_B * mu_s / (cx * cy * cz * a ** 3))
+
+
+def macrocell_scatter(H, c) -> np.ndarray:
+    """the cell field is applied equally to all spins of the cell (R14)."""
+    cx, cy, cz = map(int, c)
+    return np.repeat(np.repeat(np.repeat(np.asarray(H), cz, axis=1), cy, axis=2), cx, axis=3)
