@@ -1,0 +1,112 @@
+/*
+ * demag.h -- C ABI of the B200-native demagnetizing-field convolution.
+ *
+ * Computes, on ONE GPU, the long-range demagnetizing field of arXiv 2308.08447, Eq. (1)
+ * (Section II):
+ *
+ *        H_d,i = - sum_j N(i-j) M_j        (sum over all cells j of the mesh, j = i included)
+ *
+ * evaluated as a zero-padded 3D FFT convolution (Appendix A :228-343):
+ * x R2C FFT -> y FFT -> z FFT -> multiply with the transformed tensor -> inverse z, y -> x C2R.
+ *
+ * Conventions (readings R3, R6, R8):
+ *   - mesh of nx*ny*nz cuboid cells of size hx*hy*hz metres; every n_a is a power of two, n_a <= 4096;
+ *   - an axis is zero-padded to N_a = 2 n_a unless n_a == 1 or its PBC flag is set (then N_a = n_a);
+ *   - M, H: planar device arrays [3][nz][ny][nx], x fastest, components x,y,z, in A/m,
+ *     float (DEMAG_FP32) or double (DEMAG_FP64), 16-byte aligned, not aliased;
+ *   - tensor component order: xx, yy, zz, xy, xz, yz; N is dimensionless;
+ *   - pointers named *_dev are device pointers, *_host are host pointers;
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream);
+ *   - every function returns a demag_status; no exceptions, no abort, no printing.
+ *
+ * Ownership: the plan owns its workspace, twiddle tables and kernel spectrum (allocated in
+ * demag_plan_create / demag_set_kernel).  The caller owns M, H, S, Hs, E.
+ * demag_apply / demag_energy / demag_apply_atomistic never allocate, never synchronise, never touch
+ * the host: they only enqueue kernels on `cuda_stream`.  A plan is not re-entrant (one apply in
+ * flight per plan).
+ */
+#ifndef DEMAG_H_
+#define DEMAG_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct demag_plan_s* demag_plan_t;            /* opaque; owned by the library */
+
+typedef enum {
+    DEMAG_OK = 0,
+    DEMAG_ERR_INVALID_ARG = 1,   /* NULL / misaligned / aliased pointer, non-positive size          */
+    DEMAG_ERR_UNSUPPORTED = 2,   /* size not a power of two or > 4096, built-in tensor with PBC ...  */
+    DEMAG_ERR_ALLOC = 3,         /* cudaMalloc / malloc failed                                       */
+    DEMAG_ERR_CUDA = 4,          /* a CUDA runtime call or launch failed (see demag_last_error)      */
+    DEMAG_ERR_NO_KERNEL = 5      /* demag_apply before demag_set_kernel                              */
+} demag_status;
+
+enum { DEMAG_FP32 = 0, DEMAG_FP64 = 1 };                 /* precision of M, H, workspace, spectrum */
+enum { DEMAG_PBC_X = 1, DEMAG_PBC_Y = 2, DEMAG_PBC_Z = 4 };  /* pbc_flags bitmask     */
+
+/* Create a plan for an nx*ny*nz mesh of hx*hy*hz [m] cells (the statement of the
+ * problem; :31-35 padding; :47 PBC axes are not padded).  Allocates workspace and FFT tables on the
+ * current CUDA device.  *out is set to NULL on failure. */
+demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz,
+                               double hx, double hy, double hz,
+                               unsigned pbc_flags, int precision);
+
+/* Compute and store the transformed tensor ("convolution kernel ... computed in the initialization
+ * stage"; stored packed by its y/z symmetries as real arrays).
+ *   N6_host == NULL: built-in fp64 Newell builder on the GPU ("formulas in Ref. [23]";
+ *                    DESIGN.md R1, R4).  DEMAG_ERR_UNSUPPORTED if any PBC flag is set.
+ *   N6_host != NULL: host array double[6][nz][ny][nx]: N_c at the non-negative cell offsets
+ *                    (dx,dy,dz); negative offsets follow by parity (diagonal even; xy odd in x,y;
+ *                    xz odd in x,z; yz odd in y,z).  On a PBC axis the n_a entries are the periodic
+ *                    kernel at offsets 0..n_a-1 (no parity folding on that axis).
+ * The spectrum is computed in fp64, the factor -1/(Nx Ny Nz) is folded in (R3), and it is
+ * rounded once to fp32 (kept fp64 for a DEMAG_FP64 plan).  Synchronous (plan-time call). */
+demag_status demag_set_kernel(demag_plan_t plan, const double* N6_host);
+
+/* H = -N * M  (Eq. (1); execution order of Appendix A).
+ * M_dev, H_dev: device arrays [3][nz][ny][nx] of the plan's precision.  Asynchronous on the stream.
+ * M is not modified; H is overwritten.  DEMAG_ERR_NO_KERNEL before demag_set_kernel. */
+demag_status demag_apply(demag_plan_t plan, const void* M_dev, void* H_dev, void* cuda_stream);
+
+/* Demagnetizing energy  E = -(mu0/2) hx hy hz sum_i M_i . H_i  [J] (R12), accumulated in
+ * fp64 and written to the device scalar *E_dev (double).  Asynchronous on the stream. */
+demag_status demag_energy(demag_plan_t plan, const void* M_dev, const void* H_dev,
+                          double* E_dev, void* cuda_stream);
+
+/* Atomistic front end (Eq. (9)): unit spins S_dev [3][Lz][Ly][Lx] on a simple cubic
+ * lattice (constant a [m], moment mu_s_in_muB Bohr magnetons) are averaged into macrocells of
+ * cx*cy*cz spins, M = mu_B mu_s sum(S^) / (cx cy cz a^3); the plan's convolution is applied; the
+ * cell field is written to every spin of the cell, Hs_dev [3][Lz][Ly][Lx] (overwritten if
+ * accumulate == 0, added to if accumulate != 0).  The spin lattice is (nx*cx, ny*cy, nz*cz); the plan
+ * must have been created with h_a = c_a * a (checked to 1e-9 relative). */
+demag_status demag_apply_atomistic(demag_plan_t plan, const void* S_dev, void* Hs_dev,
+                                   int cx, int cy, int cz, double mu_s_in_muB, double a,
+                                   int accumulate, void* cuda_stream);
+
+/* Copy back the REAL-SPACE tensor the plan was given or built: double[6][nz][ny][nx] (host).
+ * For builder-vs-oracle parity tests.  Synchronous. */
+demag_status demag_get_kernel_real(demag_plan_t plan, double* N6_host);
+
+/* Bytes of device memory the plan holds (workspace + tables + kernel spectrum). */
+size_t demag_workspace_bytes(demag_plan_t plan);
+
+/* Tuning knob: how many kx planes one L2-resident slab of the y/z stages covers (0 = automatic).
+ * Does not change results. */
+demag_status demag_set_slab(demag_plan_t plan, int kx_per_slab);
+
+/* Number of kernel launches one demag_apply enqueues with the current settings. */
+int demag_launches_per_apply(demag_plan_t plan);
+
+/* Last error message of the calling thread ("" if none). */
+const char* demag_last_error(void);
+
+demag_status demag_plan_destroy(demag_plan_t plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEMAG_H_ */

@@ -1,0 +1,493 @@
+// plan.cu -- the C ABI of include/demag.h: argument checking, workspace, launch configuration.
+// Every step of the hot path runs in the kernels of kernels.cuh; this file only enqueues them.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "../../include/demag.h"
+#include "builder.cuh"
+#include "kernels.cuh"
+
+using namespace demag;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+demag_status fail(demag_status st, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+#define CUDA_TRY(call)                                                                          \
+    do {                                                                                        \
+        cudaError_t e_ = (call);                                                                \
+        if (e_ != cudaSuccess)                                                                  \
+            return fail(e_ == cudaErrorMemoryAllocation ? DEMAG_ERR_ALLOC : DEMAG_ERR_CUDA,     \
+                        "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);   \
+    } while (0)
+
+constexpr int kMaxSmem = 232448;          // 227 KB opt-in dynamic shared memory per CTA (sm_100)
+constexpr size_t kSlabBytes = 40u << 20;  // target size of the L2-resident W2 slab (L2 is ~126 MB)
+
+inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+inline int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+inline int pow2_floor(long long v) { int p = 1; while (2LL * p <= v) p *= 2; return p; }
+
+}  // namespace
+
+struct demag_plan_s {
+    Geo g;
+    double h[3];
+    unsigned pbc;
+    int prec;
+    size_t esz;       // sizeof real
+    int device;
+    int sm_count;
+    void* W1 = nullptr; size_t w1_bytes = 0;
+    void* W2 = nullptr; size_t w2_bytes = 0;
+    void* K = nullptr;  size_t k_bytes = 0, kcomp_stride = 0;
+    void* tw[3] = {nullptr, nullptr, nullptr}; size_t tw_bytes = 0;
+    void* Mc = nullptr; void* Hc = nullptr; size_t macro_bytes = 0;   // atomistic macrocell buffers
+    bool has_kernel = false;
+    // launch configuration
+    int R1, thr1, smem1;          // K1 / K5
+    int B2, thr2, smem2;          // K2 / K4
+    int TY, thr3, smem3;          // K3
+    int nkx_slab, nkx_auto;
+};
+
+namespace {
+
+int pick_threads(long long elems)
+{
+    long long t = elems / 16;
+    t = (t + 31) / 32 * 32;
+    if (t < 64) t = 64;
+    if (t > 512) t = 512;
+    return (int)t;
+}
+
+template <typename T>
+demag_status set_func_attrs()
+{
+    CUDA_TRY(cudaFuncSetAttribute(k_x_r2c<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_x_c2r<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_z_mul<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    return DEMAG_OK;
+}
+
+// exp(-2 pi i k / N), k = 0..N-1, evaluated in long double, octant-reduced
+template <typename C>
+demag_status make_twiddles(int N, void** out, size_t* bytes)
+{
+    std::vector<C> t((size_t)N);
+    const long double tp = 6.283185307179586476925286766559005768L;
+    for (int k = 0; k < N; ++k) {
+        const long double a = tp * (long double)k / (long double)N;
+        t[k].x = (decltype(C::x))cosl(a);
+        t[k].y = (decltype(C::x))(-sinl(a));
+    }
+    if (N >= 4) { t[N / 4].x = 0; t[N / 4].y = -1; t[N / 2].x = -1; t[N / 2].y = 0; t[3 * N / 4].x = 0; t[3 * N / 4].y = 1; }
+    else if (N == 2) { t[1].x = -1; t[1].y = 0; }
+    CUDA_TRY(cudaMalloc(out, sizeof(C) * (size_t)N));
+    CUDA_TRY(cudaMemcpy(*out, t.data(), sizeof(C) * (size_t)N, cudaMemcpyHostToDevice));
+    *bytes += sizeof(C) * (size_t)N;
+    return DEMAG_OK;
+}
+
+void configure(demag_plan_s* p)
+{
+    const Geo& g = p->g;
+    const size_t csz = 2 * p->esz;
+    // K1 / K5: R rows of Lc complex.  R >= 4 keeps the transposed stores at >= 32 B (fp32) runs.
+    {
+        const long long Lc = 1LL << g.lLc;
+        int R = pow2_floor(std::max<long long>(1, (48 << 10) / (long long)(Lc * csz)));
+        if (R < 4) R = 4;
+        if (R > 16) R = 16;
+        while (R > 1 && (long long)R * Lc * csz > 200 << 10) R /= 2;
+        if (R > g.ny) R = g.ny;
+        p->R1 = R;
+        const long long elems = (long long)R * Lc;
+        p->smem1 = (int)(((elems + 15) / 16 * 16) * csz);
+        p->thr1 = pick_threads(elems);
+    }
+    // K2 / K4: B lines of Ny complex, about 32 KB per tile
+    {
+        int B = (int)std::max<long long>(1, (32 << 10) / (long long)(g.Ny * csz));
+        if (B > 16) B = 16;
+        const long long nlines_min = 3LL * g.nz;
+        if (B > nlines_min) B = (int)nlines_min;
+        p->B2 = B;
+        const long long elems = (long long)B * g.Ny;
+        p->smem2 = (int)(((elems + 15) / 16 * 16) * csz);
+        p->thr2 = pick_threads(elems);
+    }
+    // K3: TY ky columns x Nz x 3 components
+    {
+        int TY = 16;
+        while (TY > 1 && (long long)TY * 3 * g.Nz * csz > 100 << 10) TY /= 2;
+        if (TY > g.Ny) TY = g.Ny;
+        p->TY = TY;
+        const long long elems = 3LL * TY * g.Nz;
+        p->smem3 = (int)(((elems + 15) / 16 * 16) * csz);
+        p->thr3 = pick_threads(elems);
+    }
+    // slab of kx planes whose W2 part stays L2-resident between K2, K3 and K4
+    {
+        const size_t per_kx = (size_t)3 * g.nz * g.Ny * csz;
+        long long n = (long long)(kSlabBytes / per_kx);
+        if (n < 1) n = 1;
+        if (n > g.hx) n = g.hx;
+        p->nkx_auto = (int)n;
+        p->nkx_slab = (int)n;
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* demag_last_error(void) { return g_err; }
+
+demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double hx, double hy, double hz,
+                               unsigned pbc_flags, int precision)
+{
+    g_err[0] = 0;
+    if (!out) return fail(DEMAG_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return fail(DEMAG_ERR_INVALID_ARG, "mesh sizes must be >= 1");
+    if (!(hx > 0 && hy > 0 && hz > 0) || !isfinite(hx) || !isfinite(hy) || !isfinite(hz))
+        return fail(DEMAG_ERR_INVALID_ARG, "cell sizes must be positive and finite");
+    if (precision != DEMAG_FP32 && precision != DEMAG_FP64) return fail(DEMAG_ERR_INVALID_ARG, "bad precision");
+    if (pbc_flags & ~7u) return fail(DEMAG_ERR_INVALID_ARG, "bad pbc_flags");
+    if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz))
+        return fail(DEMAG_ERR_UNSUPPORTED, "mesh sizes must be powers of two (got %d x %d x %d)", nx, ny, nz);
+    if (nx > 4096 || ny > 4096 || nz > 4096) return fail(DEMAG_ERR_UNSUPPORTED, "mesh sizes must be <= 4096");
+
+    demag_plan_s* p = new (std::nothrow) demag_plan_s();
+    if (!p) return fail(DEMAG_ERR_ALLOC, "out of host memory");
+    Geo& g = p->g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.Nx = (nx == 1 || (pbc_flags & DEMAG_PBC_X)) ? nx : 2 * nx;
+    g.Ny = (ny == 1 || (pbc_flags & DEMAG_PBC_Y)) ? ny : 2 * ny;
+    g.Nz = (nz == 1 || (pbc_flags & DEMAG_PBC_Z)) ? nz : 2 * nz;
+    g.hx = g.Nx / 2 + 1;
+    g.lLc = g.Nx >= 2 ? ilog2(g.Nx / 2) : 0;
+    g.lNy = ilog2(g.Ny); g.lNz = ilog2(g.Nz);
+    g.kpy = g.Ny / 2 + 1; g.kpz = g.Nz / 2 + 1;
+    g.kpitch = (g.kpy + 7) / 8 * 8;
+    p->h[0] = hx; p->h[1] = hy; p->h[2] = hz;
+    p->pbc = pbc_flags; p->prec = precision;
+    p->esz = precision == DEMAG_FP32 ? 4 : 8;
+    demag_status st = DEMAG_OK;
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
+    if (e != cudaSuccess) { delete p; return fail(DEMAG_ERR_CUDA, "no CUDA device: %s", cudaGetErrorString(e)); }
+    configure(p);
+    const size_t csz = 2 * p->esz;
+    p->w1_bytes = (size_t)3 * g.hx * g.nz * g.ny * csz;
+    p->w2_bytes = (size_t)3 * p->nkx_auto * g.nz * g.Ny * csz;
+    p->kcomp_stride = (size_t)g.hx * g.kpz * g.kpitch;
+    p->k_bytes = 6 * p->kcomp_stride * p->esz;
+    auto alloc_all = [&]() -> demag_status {
+        if (precision == DEMAG_FP32) { demag_status s = set_func_attrs<float>(); if (s) return s; }
+        else { demag_status s = set_func_attrs<double>(); if (s) return s; }
+        CUDA_TRY(cudaFuncSetAttribute(k_sym_axis, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+        CUDA_TRY(cudaMalloc(&p->W1, p->w1_bytes));
+        CUDA_TRY(cudaMalloc(&p->W2, p->w2_bytes));
+        CUDA_TRY(cudaMalloc(&p->K, p->k_bytes));
+        CUDA_TRY(cudaMemset(p->K, 0, p->k_bytes));
+        const int N[3] = {g.Nx, g.Ny, g.Nz};
+        for (int a = 0; a < 3; ++a) {
+            demag_status s = precision == DEMAG_FP32 ? make_twiddles<float2>(N[a], &p->tw[a], &p->tw_bytes)
+                                                     : make_twiddles<double2>(N[a], &p->tw[a], &p->tw_bytes);
+            if (s) return s;
+        }
+        return DEMAG_OK;
+    };
+    st = alloc_all();
+    if (st != DEMAG_OK) { demag_plan_destroy(p); return st; }
+    *out = p;
+    return DEMAG_OK;
+}
+
+demag_status demag_plan_destroy(demag_plan_t p)
+{
+    if (!p) return DEMAG_OK;
+    cudaFree(p->W1); cudaFree(p->W2); cudaFree(p->K);
+    for (int a = 0; a < 3; ++a) cudaFree(p->tw[a]);
+    cudaFree(p->Mc); cudaFree(p->Hc);
+    delete p;
+    return DEMAG_OK;
+}
+
+size_t demag_workspace_bytes(demag_plan_t p)
+{
+    if (!p) return 0;
+    return p->w1_bytes + p->w2_bytes + p->k_bytes + p->tw_bytes + p->macro_bytes;
+}
+
+demag_status demag_set_slab(demag_plan_t p, int kx_per_slab)
+{
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (kx_per_slab < 0) return fail(DEMAG_ERR_INVALID_ARG, "kx_per_slab < 0");
+    int n = kx_per_slab == 0 ? p->nkx_auto : kx_per_slab;
+    if (n > p->nkx_auto) n = p->nkx_auto;      // the W2 slab was sized for nkx_auto planes
+    p->nkx_slab = n;
+    return DEMAG_OK;
+}
+
+int demag_launches_per_apply(demag_plan_t p)
+{
+    if (!p) return 0;
+    const int nslab = (p->g.hx + p->nkx_slab - 1) / p->nkx_slab;
+    return 2 + 3 * nslab;
+}
+
+}  // extern "C"
+
+// ================================================================================ plan-time: kernel
+namespace {
+
+// Real-space tensor table on the device, fp64 [6][nz][ny][nx] (built-in builder).
+demag_status build_table_dev(demag_plan_s* p, double** T_out)
+{
+    const Geo& g = p->g;
+    const size_t nc = (size_t)g.nx * g.ny * g.nz;
+    double* T = nullptr;
+    CUDA_TRY(cudaMalloc(&T, 6 * nc * sizeof(double)));
+    k_tensor_table<<<(unsigned)((nc + 127) / 128), 128>>>(g.nx, g.ny, g.nz, p->h[0], p->h[1], p->h[2], T);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { cudaFree(T); return fail(DEMAG_ERR_CUDA, "k_tensor_table: %s", cudaGetErrorString(e)); }
+    *T_out = T;
+    return DEMAG_OK;
+}
+
+demag_status launch_sym_axis(const double* in, double* out, int n, int N, int par, int ni, size_t no,
+                             size_t so_in, size_t se_in, size_t so_out, size_t se_out, const double2* tw)
+{
+    const int lN = ilog2(N);
+    int B = std::max(1, std::min(8, 8192 / N));
+    if (B > ni) B = ni;
+    const long long elems = (long long)B * N;
+    const int smem = (int)(((elems + 15) / 16 * 16) * sizeof(double2));
+    const int thr = pick_threads(elems);
+    const size_t tilesI = (size_t)(ni + B - 1) / B;
+    const size_t grid = tilesI * no;
+    if (grid > 0x7fffffffULL) return fail(DEMAG_ERR_UNSUPPORTED, "kernel transform grid too large");
+    k_sym_axis<<<(unsigned)grid, thr, smem>>>(in, out, n, lN, N / 2 + 1, par, ni, B, so_in, se_in, so_out, se_out, tw);
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}
+
+template <typename T>
+void launch_pack(const double* A, void* K, const Geo& g, double scale)
+{
+    const size_t n = (size_t)g.hx * g.kpz * g.kpy;
+    const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
+    k_pack_kernel<T><<<grid, 256>>>(A, (T*)K, g.hx, g.kpy, g.kpz, g.kpitch, scale);
+}
+
+}  // namespace
+
+extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (!N6_host && p->pbc) return fail(DEMAG_ERR_UNSUPPORTED, "built-in tensor builder does not support PBC");
+    const Geo& g = p->g;
+    const size_t nc = (size_t)g.nx * g.ny * g.nz;
+    static const int par[6][3] = {{1, 1, 1}, {1, 1, 1}, {1, 1, 1}, {-1, -1, 1}, {-1, 1, -1}, {1, -1, -1}};
+    double *Tdev = nullptr, *A = nullptr, *B1 = nullptr, *B2 = nullptr, *B3 = nullptr;
+    double2* tw64[3] = {nullptr, nullptr, nullptr};
+    size_t dummy = 0;
+    demag_status st = DEMAG_OK;
+    auto body = [&]() -> demag_status {
+        if (!N6_host) { demag_status s = build_table_dev(p, &Tdev); if (s) return s; }
+        else CUDA_TRY(cudaMalloc(&A, nc * sizeof(double)));
+        CUDA_TRY(cudaMalloc(&B1, (size_t)g.nz * g.ny * g.hx * sizeof(double)));
+        CUDA_TRY(cudaMalloc(&B2, (size_t)g.nz * g.kpy * g.hx * sizeof(double)));
+        CUDA_TRY(cudaMalloc(&B3, (size_t)g.kpz * g.kpy * g.hx * sizeof(double)));
+        const int N[3] = {g.Nx, g.Ny, g.Nz};
+        for (int a = 0; a < 3; ++a) { demag_status s = make_twiddles<double2>(N[a], (void**)&tw64[a], &dummy); if (s) return s; }
+        for (int c = 0; c < 6; ++c) {
+            const double* src;
+            if (N6_host) { CUDA_TRY(cudaMemcpy(A, N6_host + c * nc, nc * sizeof(double), cudaMemcpyHostToDevice)); src = A; }
+            else src = Tdev + c * nc;
+            demag_status s;
+            // x: rows (z,y); y: lines (z; kx); z: lines (ky,kx)
+            s = launch_sym_axis(src, B1, g.nx, g.Nx, par[c][0], 1, (size_t)g.nz * g.ny, g.nx, 1, g.hx, 1, tw64[0]);
+            if (s) return s;
+            s = launch_sym_axis(B1, B2, g.ny, g.Ny, par[c][1], g.hx, g.nz, (size_t)g.ny * g.hx, g.hx,
+                                (size_t)g.kpy * g.hx, g.hx, tw64[1]);
+            if (s) return s;
+            s = launch_sym_axis(B2, B3, g.nz, g.Nz, par[c][2], g.kpy * g.hx, 1, 0, (size_t)g.kpy * g.hx, 0,
+                                (size_t)g.kpy * g.hx, tw64[2]);
+            if (s) return s;
+            int nodd = 0;
+            for (int a = 0; a < 3; ++a) nodd += par[c][a] < 0;
+            // each odd axis contributes a factor i (X = i Im X): two odd axes -> -1.  Eq. (1)'s minus sign and
+            // the inverse-transform normalisation 1/(Nx Ny Nz) are folded in here (R3).
+            const double scale = (nodd == 2 ? -1.0 : 1.0) * (-1.0) / ((double)g.Nx * g.Ny * g.Nz);
+            if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, scale);
+            else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, scale);
+            CUDA_TRY(cudaGetLastError());
+        }
+        CUDA_TRY(cudaDeviceSynchronize());
+        return DEMAG_OK;
+    };
+    st = body();
+    cudaFree(Tdev); cudaFree(A); cudaFree(B1); cudaFree(B2); cudaFree(B3);
+    for (int a = 0; a < 3; ++a) cudaFree(tw64[a]);
+    if (st == DEMAG_OK) p->has_kernel = true;
+    return st;
+}
+
+extern "C" demag_status demag_get_kernel_real(demag_plan_t p, double* N6_host)
+{
+    g_err[0] = 0;
+    if (!p || !N6_host) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
+    if (p->pbc) return fail(DEMAG_ERR_UNSUPPORTED, "built-in tensor builder does not support PBC");
+    double* T = nullptr;
+    demag_status st = build_table_dev(p, &T);
+    if (st) return st;
+    const size_t nc = (size_t)p->g.nx * p->g.ny * p->g.nz;
+    cudaError_t e = cudaMemcpy(N6_host, T, 6 * nc * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaFree(T);
+    if (e != cudaSuccess) return fail(DEMAG_ERR_CUDA, "copy back: %s", cudaGetErrorString(e));
+    return DEMAG_OK;
+}
+
+// ================================================================================ hot path
+namespace {
+
+template <typename T>
+demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st)
+{
+    using C = typename cx_of<T>::type;
+    const Geo& g = p->g;
+    C* W1 = (C*)p->W1; C* W2 = (C*)p->W2;
+    const C* twx = (const C*)p->tw[0]; const C* twy = (const C*)p->tw[1]; const C* twz = (const C*)p->tw[2];
+    const size_t nc = (size_t)g.nx * g.ny * g.nz;
+    if (g.Nx == 1) {
+        const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
+        k_x_copy_fwd<T><<<grid, 256, 0, st>>>(3 * nc, M, W1);
+    } else {
+        k_x_r2c<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, M, W1, twx);
+    }
+    for (int kx0 = 0; kx0 < g.hx; kx0 += p->nkx_slab) {
+        const int nkx = std::min(p->nkx_slab, g.hx - kx0);
+        const unsigned g2 = (unsigned)((3LL * nkx * g.nz + p->B2 - 1) / p->B2);
+        k_y_fwd<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W1, W2, twy);
+        k_z_mul<T><<<(unsigned)(nkx * (g.Ny / p->TY)), p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, (const T*)p->K,
+                                                                               p->kcomp_stride, twz);
+        k_y_inv<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W2, W1, twy);
+    }
+    if (g.Nx == 1) {
+        const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
+        k_x_copy_inv<T><<<grid, 256, 0, st>>>(3 * nc, W1, H);
+    } else {
+        k_x_c2r<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, W1, H, twx);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}
+
+demag_status check_apply_args(demag_plan_s* p, const void* a, const void* b, size_t bytes)
+{
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (!a || !b) return fail(DEMAG_ERR_INVALID_ARG, "NULL device pointer");
+    if (((uintptr_t)a & 15) || ((uintptr_t)b & 15)) return fail(DEMAG_ERR_INVALID_ARG, "device pointers must be 16-byte aligned");
+    const char *pa = (const char*)a, *pb = (const char*)b;
+    if (pa < pb + bytes && pb < pa + bytes) return fail(DEMAG_ERR_INVALID_ARG, "input and output overlap");
+    return DEMAG_OK;
+}
+
+}  // namespace
+
+extern "C" demag_status demag_apply(demag_plan_t p, const void* M_dev, void* H_dev, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    const size_t bytes = (size_t)3 * p->g.nx * p->g.ny * p->g.nz * p->esz;
+    demag_status s = check_apply_args(p, M_dev, H_dev, bytes);
+    if (s) return s;
+    if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return p->prec == DEMAG_FP32 ? apply_impl<float>(p, (const float*)M_dev, (float*)H_dev, st)
+                                 : apply_impl<double>(p, (const double*)M_dev, (double*)H_dev, st);
+}
+
+extern "C" demag_status demag_energy(demag_plan_t p, const void* M_dev, const void* H_dev, double* E_dev, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!p || !M_dev || !H_dev || !E_dev) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
+    if ((uintptr_t)E_dev & 7) return fail(DEMAG_ERR_INVALID_ARG, "E_dev must be 8-byte aligned");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n3 = (size_t)3 * p->g.nx * p->g.ny * p->g.nz;
+    const double mu0 = 4.0e-7 * 3.14159265358979323846;
+    const double scale = -0.5 * mu0 * p->h[0] * p->h[1] * p->h[2];
+    CUDA_TRY(cudaMemsetAsync(E_dev, 0, sizeof(double), st));
+    const unsigned grid = (unsigned)std::min<size_t>((n3 + 255) / 256, (size_t)p->sm_count * 8);
+    if (p->prec == DEMAG_FP32) k_energy<float><<<grid, 256, 0, st>>>(n3, (const float*)M_dev, (const float*)H_dev, scale, E_dev);
+    else k_energy<double><<<grid, 256, 0, st>>>(n3, (const double*)M_dev, (const double*)H_dev, scale, E_dev);
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}
+
+extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev, void* Hs_dev, int cx, int cy, int cz,
+                                              double mu_s_in_muB, double a, int accumulate, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (cx < 1 || cy < 1 || cz < 1 || !(a > 0) || !isfinite(mu_s_in_muB))
+        return fail(DEMAG_ERR_INVALID_ARG, "bad macrocell / lattice arguments");
+    const Geo& g = p->g;
+    const double want[3] = {cx * a, cy * a, cz * a};
+    for (int i = 0; i < 3; ++i)
+        if (fabs(want[i] - p->h[i]) > 1e-9 * p->h[i])
+            return fail(DEMAG_ERR_INVALID_ARG, "plan cell size must equal macrocell size c*a (axis %d)", i);
+    const size_t nspin3 = (size_t)3 * g.nx * cx * g.ny * cy * g.nz * cz;
+    demag_status s = check_apply_args(p, S_dev, Hs_dev, nspin3 * p->esz);
+    if (s) return s;
+    if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
+    const size_t nc = (size_t)g.nx * g.ny * g.nz;
+    if (!p->Mc) {   // first atomistic call on this plan: allocate the two macrocell buffers (documented)
+        CUDA_TRY(cudaMalloc(&p->Mc, 3 * nc * p->esz));
+        CUDA_TRY(cudaMalloc(&p->Hc, 3 * nc * p->esz));
+        p->macro_bytes = 6 * nc * p->esz;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const double muB = 9.2740100783e-24;
+    const double f = muB * mu_s_in_muB / ((double)cx * cy * cz * a * a * a);
+    const unsigned ga = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)1 << 22);
+    const unsigned gs = (unsigned)std::min<size_t>((nspin3 / 4 + 255) / 256 + 1, (size_t)p->sm_count * 32);
+    if (p->prec == DEMAG_FP32) {
+        k_macro_avg<float><<<ga, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const float*)S_dev, (float*)p->Mc, f);
+        s = apply_impl<float>(p, (const float*)p->Mc, (float*)p->Hc, st);
+        if (s) return s;
+        k_macro_scatter<float><<<gs, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const float*)p->Hc, (float*)Hs_dev, accumulate);
+    } else {
+        k_macro_avg<double><<<ga, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const double*)S_dev, (double*)p->Mc, f);
+        s = apply_impl<double>(p, (const double*)p->Mc, (double*)p->Hc, st);
+        if (s) return s;
+        k_macro_scatter<double><<<gs, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const double*)p->Hc, (double*)Hs_dev, accumulate);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}

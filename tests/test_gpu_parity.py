@@ -1,0 +1,250 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle -- needs a B200.
+
+Tolerances (BASELINE.json north_star): max |H_gpu - H_ref| / Ms <= 2e-5 for fp32, <= 1e-11 for fp64,
+with the oracle's N pushed through demag_set_kernel (R5 "convolution parity").
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL32 = 2e-5
+TOL64 = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2308_08447_b200 import binding
+    binding.lib()          # fail loudly if the CUDA library is missing
+    return binding
+
+
+def run_gpu(torch, B, n, h, T, M, prec, slab=0, builtin=False):
+    dt = torch.float32 if prec == B.DEMAG_FP32 else torch.float64
+    with B.Plan(n, h, 0, prec) as p:
+        p.set_kernel(None if builtin else T)
+        if slab:
+            p.set_slab(slab)
+        Md = torch.from_numpy(np.ascontiguousarray(M)).to("cuda", dt)
+        Hd = torch.full_like(Md, float("nan"))
+        p.apply(Md, Hd)
+        torch.cuda.synchronize()
+        assert torch.equal(Md.cpu(), torch.from_numpy(np.ascontiguousarray(M)).to(dt)), "M was modified"
+        return Hd.cpu().numpy().astype(np.float64)
+
+
+def rand_M(n, Ms, seed):
+    from paper_2308_08447_b200 import workloads as W
+    return W.random_unit_vectors(n, Ms, seed)
+
+
+# --------------------------------------------------------------------------------- config 1
+def test_config1_full_direct_sum_and_naive_dft(torch, B, oracle):
+    from paper_2308_08447_b200 import workloads as W
+    cfg = W.CONFIGS["C1"]
+    M = W.make_magnetisation(cfg)
+    T = oracle.tensor_table(cfg.n, cfg.h)
+    HA = oracle.direct_sum(T, M.astype(np.float64))
+    HB = oracle.naive_dft_conv(T, M.astype(np.float64))
+    assert np.abs(HA - HB).max() / cfg.Ms < 1e-13
+    H32 = run_gpu(torch, B, cfg.n, cfg.h, T, M, B.DEMAG_FP32)
+    assert np.abs(H32 - HA).max() / cfg.Ms <= TOL32
+    H64 = run_gpu(torch, B, cfg.n, cfg.h, T, M, B.DEMAG_FP64)
+    assert np.abs(H64 - HA).max() / cfg.Ms <= TOL64
+    assert np.abs(H64 - HB).max() / cfg.Ms <= TOL64
+
+
+# --------------------------------------------------------------------------------- shape sweep
+SHAPES = [(1, 1, 1), (2, 1, 1), (1, 2, 1), (1, 1, 2), (2, 2, 2), (4, 2, 8), (8, 8, 8), (16, 4, 2), (64, 1, 1),
+          (1, 64, 1), (1, 1, 64), (1, 16, 4), (32, 16, 1), (4, 128, 8), (128, 4, 2), (2, 2, 128), (16, 32, 16),
+          (512, 2, 1), (2, 512, 2), (64, 64, 4)]
+
+
+@pytest.mark.parametrize("n", SHAPES)
+@pytest.mark.parametrize("prec", [0, 1])
+def test_shapes_against_oracle(torch, B, oracle, n, prec):
+    """Every power-of-two length per axis incl. degenerate 1-cell axes, several tiles and ragged tile
+    tails (line counts not divisible by the batch)."""
+    h = (2e-9, 3e-9, 1e-9)
+    Ms = 8e5
+    M = rand_M(n, Ms, 100 + sum(n))
+    T = oracle.tensor_table(n, h)
+    ref = oracle.fft_conv(T, M.astype(np.float64))
+    if np.prod(n) <= 4096:
+        ref_ds = oracle.direct_sum(T, M.astype(np.float64))
+        assert np.abs(ref - ref_ds).max() / Ms < 1e-12
+        ref = ref_ds
+    H = run_gpu(torch, B, n, h, T, M, prec)
+    err = np.abs(H - ref).max() / Ms
+    assert err <= (TOL32 if prec == 0 else TOL64), err
+
+
+@pytest.mark.parametrize("slab", [1, 3, 7])
+def test_slab_size_does_not_change_result(torch, B, oracle, slab):
+    n, h = (32, 16, 8), (2e-9, 2e-9, 2e-9)
+    M = rand_M(n, 8e5, 5)
+    T = oracle.tensor_table(n, h)
+    H0 = run_gpu(torch, B, n, h, T, M, 0)
+    H1 = run_gpu(torch, B, n, h, T, M, 0, slab=slab)
+    assert np.array_equal(H0, H1)
+
+
+def test_impulse_returns_tensor_column(torch, B, oracle):
+    """A single magnetised cell reads the kernel back through the whole pipeline: catches every
+    padding / crop / packing / parity-sign bug."""
+    n, h = (16, 8, 4), (1e-9, 1.5e-9, 0.5e-9)
+    T = oracle.tensor_table(n, h)
+    j = (5, 3, 1)
+    for b in range(3):
+        M = np.zeros((3, n[2], n[1], n[0]), dtype=np.float32)
+        M[b, j[2], j[1], j[0]] = 1.0
+        H = run_gpu(torch, B, n, h, T, M, B.DEMAG_FP64)
+        for iz, iy, ix in [(0, 0, 0), (3, 7, 15), (1, 3, 5), (2, 0, 9), (0, 7, 0), (3, 2, 14)]:
+            N6 = oracle.N_at(((ix - j[0]) * h[0], (iy - j[1]) * h[1], (iz - j[2]) * h[2]), h)
+            want = -N6[oracle.COMP][:, b]
+            assert np.abs(H[:, iz, iy, ix] - want).max() < 1e-12
+
+
+def test_linearity(torch, B, oracle):
+    n, h = (16, 16, 4), (2e-9, 2e-9, 2e-9)
+    T = oracle.tensor_table(n, h)
+    M1 = rand_M(n, 1.0, 1).astype(np.float64); M2 = rand_M(n, 1.0, 2).astype(np.float64)
+    H1 = run_gpu(torch, B, n, h, T, M1, 1); H2 = run_gpu(torch, B, n, h, T, M2, 1)
+    H3 = run_gpu(torch, B, n, h, T, 2.0 * M1 - 3.0 * M2, 1)
+    assert np.abs(H3 - (2.0 * H1 - 3.0 * H2)).max() < 1e-12
+
+
+# --------------------------------------------------------------------------------- tensor builder
+@pytest.mark.parametrize("n,h", [((64, 32, 4), (2e-9, 2e-9, 1e-9)), ((128, 128, 1), (2e-9, 2e-9, 1e-9)),
+                                 ((32, 32, 32), (3e-9, 3e-9, 3e-9)), ((256, 8, 2), (1e-9, 1.5e-9, 0.5e-9))])
+def test_builtin_tensor_builder_vs_oracle(torch, B, oracle, n, h):
+    """DESIGN.md R5 (ii): |dN| <= 1e-10 everywhere and <= 1e-6 |N| in the far field.  The builder uses
+    a multipole series in the far field, the oracle Gauss-Legendre quadrature: independent routes."""
+    with B.Plan(n, h, 0, B.DEMAG_FP64) as p:
+        Tg = p.get_kernel_real()
+    To = oracle.tensor_table(n, h)
+    assert np.abs(Tg - To).max() <= 1e-10
+    d = np.stack(np.meshgrid(np.arange(n[2]) * h[2], np.arange(n[1]) * h[1], np.arange(n[0]) * h[0], indexing="ij"))
+    far = np.sqrt((d ** 2).sum(0)) > 30 * max(h)
+    if far.any():
+        rel = np.abs(Tg - To)[:, far] / np.maximum(np.abs(To[:, far]), 1e-300)
+        big = np.abs(To[:, far]) > 1e-3 * np.abs(To[:, far]).max()
+        assert rel[big].max() <= 1e-6
+
+
+def test_builtin_kernel_end_to_end(torch, B, oracle):
+    n, h, Ms = (32, 32, 2), (4e-9, 4e-9, 4e-9), 8e5
+    M = rand_M(n, Ms, 1001)
+    ref = oracle.direct_sum(oracle.tensor_table(n, h), M.astype(np.float64))
+    H32 = run_gpu(torch, B, n, h, None, M, 0, builtin=True)
+    assert np.abs(H32 - ref).max() / Ms <= TOL32
+    H64 = run_gpu(torch, B, n, h, None, M, 1, builtin=True)
+    assert np.abs(H64 - ref).max() / Ms <= 1e-9          # R5 (iii): reported, bounded by builder parity
+
+
+# --------------------------------------------------------------------------------- energy
+def test_energy(torch, B, oracle):
+    n, h, Ms = (16, 8, 4), (2e-9, 3e-9, 1e-9), 8e5
+    M = rand_M(n, Ms, 3)
+    T = oracle.tensor_table(n, h)
+    Href = oracle.direct_sum(T, M.astype(np.float64))
+    for prec, dt, tol in ((0, torch.float32, 1e-5), (1, torch.float64, 1e-12)):
+        with B.Plan(n, h, 0, prec) as p:
+            p.set_kernel(T)
+            Md = torch.from_numpy(M).to("cuda", dt); Hd = torch.empty_like(Md)
+            E = torch.zeros(1, dtype=torch.float64, device="cuda")
+            p.apply(Md, Hd); p.energy(Md, Hd, E)
+            torch.cuda.synchronize()
+            Eref = oracle.energy(M.astype(np.float64), Href, h)
+            assert E.item() > 0
+            assert abs(E.item() - Eref) <= tol * Eref
+
+
+# --------------------------------------------------------------------------------- atomistic
+def test_atomistic_small_lattice(torch, B, oracle):
+    """64^3 spins -> 16^3 macrocells of 4x4x4 (Eq. (9)); scatter is bitwise the cell value."""
+    from paper_2308_08447_b200 import workloads as W
+    L, c, a, mu_s = (64, 64, 64), (4, 4, 4), 0.3e-9, 2.0
+    n = (16, 16, 16); h = (1.2e-9,) * 3
+    S = W.random_spins_numpy(L, 1005)
+    Mref = oracle.macrocell_average(S.astype(np.float64), c, mu_s, a)
+    Ms = oracle.MU_B * mu_s / a ** 3
+    T = oracle.tensor_table(n, h)
+    Href = oracle.fft_conv(T, Mref)
+    with B.Plan(n, h, 0, B.DEMAG_FP32) as p:
+        p.set_kernel(T)
+        Sd = torch.from_numpy(S).cuda(); Hs = torch.full_like(Sd, float("nan"))
+        p.apply_atomistic(Sd, Hs, c, mu_s, a)
+        torch.cuda.synchronize()
+        Hs_h = Hs.cpu().numpy()
+        want = oracle.macrocell_scatter(Href, c)
+        assert np.abs(Hs_h - want).max() / Ms <= TOL32
+        cells = Hs_h[:, ::4, ::4, ::4]
+        assert np.array_equal(Hs_h, oracle.macrocell_scatter(cells, c))      # piecewise constant, bitwise
+        Hs2 = Hs.clone()
+        p.apply_atomistic(Sd, Hs2, c, mu_s, a, accumulate=True)
+        torch.cuda.synchronize()
+        assert np.allclose(Hs2.cpu().numpy(), 2 * Hs_h, rtol=1e-6, atol=0)
+    # non-cubic macrocell, fp64
+    L2, c2 = (32, 16, 8), (2, 4, 1)
+    n2 = (16, 4, 8); h2 = (2 * a, 4 * a, 1 * a)
+    S2 = W.random_spins_numpy(L2, 7).astype(np.float64)
+    M2 = oracle.macrocell_average(S2, c2, mu_s, a)
+    T2 = oracle.tensor_table(n2, h2)
+    want = oracle.macrocell_scatter(oracle.direct_sum(T2, M2), c2)
+    with B.Plan(n2, h2, 0, B.DEMAG_FP64) as p:
+        p.set_kernel(T2)
+        Sd = torch.from_numpy(S2).cuda(); Hs = torch.empty_like(Sd)
+        p.apply_atomistic(Sd, Hs, c2, mu_s, a)
+        torch.cuda.synchronize()
+        assert np.abs(Hs.cpu().numpy() - want).max() / Ms <= TOL64
+
+
+# --------------------------------------------------------------------------------- ABI error paths
+def test_error_paths(torch, B):
+    with pytest.raises(B.DemagError) as e:
+        B.demag_plan_create(0, 4, 4, 1e-9, 1e-9, 1e-9)
+    assert e.value.status == 1
+    with pytest.raises(B.DemagError) as e:
+        B.demag_plan_create(12, 4, 4, 1e-9, 1e-9, 1e-9)
+    assert e.value.status == 2
+    with pytest.raises(B.DemagError) as e:
+        B.demag_plan_create(8192, 4, 4, 1e-9, 1e-9, 1e-9)
+    assert e.value.status == 2
+    with pytest.raises(B.DemagError) as e:
+        B.demag_plan_create(4, 4, 4, -1e-9, 1e-9, 1e-9)
+    assert e.value.status == 1
+    with pytest.raises(B.DemagError) as e:
+        B.demag_plan_create(4, 4, 4, 1e-9, 1e-9, 1e-9, 0, 7)
+    assert e.value.status == 1
+    with B.Plan((4, 4, 4), (1e-9,) * 3) as p:
+        M = torch.zeros((3, 4, 4, 4), device="cuda"); H = torch.zeros_like(M)
+        with pytest.raises(B.DemagError) as e:
+            p.apply(M, H)
+        assert e.value.status == 5                      # NO_KERNEL
+        p.set_kernel(None)
+        with pytest.raises(B.DemagError) as e:
+            p.apply(M, M)
+        assert e.value.status == 1                      # aliasing
+        with pytest.raises(B.DemagError) as e:
+            B._check(B.lib().demag_apply(p.handle, None, H.data_ptr(), None))
+        assert e.value.status == 1
+        with pytest.raises(B.DemagError) as e:
+            B._check(B.lib().demag_apply(p.handle, M.data_ptr() + 4, H.data_ptr(), None))
+        assert e.value.status == 1                      # misaligned
+        assert p.workspace_bytes() > 0 and p.launches_per_apply() >= 5
+        with pytest.raises(B.DemagError) as e:
+            p.apply_atomistic(M, H, (2, 2, 2), 2.0, 0.3e-9)
+        assert e.value.status == 1                      # h != c*a
+    with B.Plan((4, 4, 4), (1e-9,) * 3, B.DEMAG_PBC_X) as p:
+        with pytest.raises(B.DemagError) as e:
+            p.set_kernel(None)
+        assert e.value.status == 2                      # built-in builder has no PBC kernel
