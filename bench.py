@@ -1,0 +1,362 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the demagnetizing-field convolution (arXiv 2308.08447, Eq. (1)) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3|C2|C4|C5|C1|C3d] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (demag_apply: x R2C -> y FFT -> z FFT*multiply*z IFFT -> y IFFT ->
+x C2R; for C5 also the macrocell average and scatter) over one seeded synthetic magnetisation of the chosen
+BASELINE.json config.  Prints ONE JSON line (rank 0).  The path does not shard without an exchange step
+(replicas only), so --gpus N runs N independent replicas, one process per GPU.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2308_08447_b200 import workloads as W  # noqa: E402  (input generators only)
+
+METRIC = "demag_throughput"
+UNIT = "Gcells/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C3", help="C1..C5, suffix d = fp64 (e.g. C3d)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    return ap.parse_args()
+
+
+def workload_name(cfg, fp64):
+    return f"{cfg.name} ({'fp64' if fp64 else 'fp32'})"
+
+
+# ----------------------------------------------------------------------------------------------- oracle legs
+def oracle_sample_rate(cfg, seconds, M_host=None):
+    """Time the oracle (as it stands) on a bounded sample of the same workload: Eq. (1) evaluated by direct
+    summation (O-S) at seeded sample cells.  Returns (Gcells/s, cores, description, table_seconds)."""
+    from oracle import oracle as O   # the cpu_baseline / --impl reference legs may use oracle/
+    n = cfg.n
+    nc = int(np.prod(n))
+    t0 = time.perf_counter()
+    T = O.tensor_table(n, cfg.h)
+    t_table = time.perf_counter() - t0
+    if M_host is None:
+        M_host = W.make_magnetisation(cfg) if cfg.kind != "atomistic" else W.random_unit_vectors(n, cfg.Ms, cfg.seed)
+    M64 = M_host.astype(np.float64)
+    cores = O.num_threads()
+    cells = W.sample_cells(n, 4096, cfg.seed)
+    k = cores
+    t0 = time.perf_counter()
+    O.direct_sum_sampled(T, M64, cells[:k])
+    dt = time.perf_counter() - t0
+    total = int(max(k, min(len(cells), seconds / max(dt, 1e-9) * k)))
+    total = max(cores, total // cores * cores)
+    t0 = time.perf_counter()
+    O.direct_sum_sampled(T, M64, cells[:total])
+    dt = time.perf_counter() - t0
+    desc = (f"oracle O-S: Eq. (1) by direct fp64 summation at {total} seeded sample cells of {cfg.name} "
+            f"({total} x {nc} cell pairs in {dt:.2f} s; tensor table built in {t_table:.1f} s, not timed)")
+    return total / dt / 1e9, cores, desc, t_table, (T, M64, cells, total)
+
+
+def run_reference(args, cfg, fp64):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    val, cores, desc, _, (T, M64, cells, total) = oracle_sample_rate(cfg, 4.0)
+    from oracle import oracle as O
+    per_step = max(cores, int(total * min(1.0, 60.0 / max(1, args.steps + args.warmup) / 4.0)) // cores * cores)
+    for _ in range(min(args.warmup, 2)):
+        O.direct_sum_sampled(T, M64, cells[:per_step])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        O.direct_sum_sampled(T, M64, cells[:per_step])
+    dt = time.perf_counter() - t0
+    value = per_step * args.steps / dt / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, fp64), "cells": int(np.prod(cfg.n)),
+                       "sample": f"{per_step} seeded output cells per step, direct O(N) sum each"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{per_step} sample cells x {int(np.prod(cfg.n))} pairs per step"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for ln in self.f.read().splitlines():
+            t = [x.strip() for x in ln.split(",")]
+            if len(t) < 9:
+                continue
+            try:
+                sm.append(float(t[1])); mx.append(float(t[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), t[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ----------------------------------------------------------------------------------------------- our arm
+def stage_bytes(n, esz):
+    """Algorithmic HBM bytes of each stage of the 5-pass separable structure (T2):
+    what each kernel must read and write if nothing stayed in L2.  [K1, K2, K3, K4, K5]."""
+    nx, ny, nz = n
+    Nx, Ny, Nz = [v if v == 1 else 2 * v for v in n]
+    hx, kpy, kpz = Nx // 2 + 1, Ny // 2 + 1, Nz // 2 + 1
+    nc = nx * ny * nz
+    w1 = 3 * hx * nz * ny * 2 * esz
+    w2 = 3 * hx * nz * Ny * 2 * esz
+    kern = 6 * hx * kpz * kpy * esz
+    return [3 * nc * esz + w1, w1 + w2, w2 + kern + w2, w2 + w1, w1 + 3 * nc * esz]
+
+
+STAGE_NAMES = ["k_x_r2c", "k_y_fwd", "k_z_mul", "k_y_inv", "k_x_c2r"]
+
+
+def run_ours(args, cfg, fp64):
+    import torch
+    import torch.distributed as dist
+    from paper_2308_08447_b200 import binding as B
+    B.lib()                                             # fail loudly if the CUDA extension is missing
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    dt = torch.float64 if fp64 else torch.float32
+    esz = 8 if fp64 else 4
+    n = cfg.n
+    nc = int(np.prod(n))
+    atom = cfg.kind == "atomistic"
+
+    # ---- inputs (seeded synthetic; host -> HBM before the timed region) and plan
+    t0 = time.perf_counter()
+    if atom:
+        L = tuple(a * c for a, c in zip(n, cfg.macro))
+        X = W.random_spins_torch(L, cfg.seed + rank, device=dev).to(dt)
+        units = int(np.prod(L)); unit_name = "spins"
+        M_host = None
+    else:
+        M_host = W.make_magnetisation(cfg)
+        X = torch.from_numpy(M_host).to(dev, dt)
+        units = nc; unit_name = "cells"
+    Y = torch.empty_like(X)
+    t_inputs = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    plan = B.Plan(n, cfg.h, 0, B.DEMAG_FP64 if fp64 else B.DEMAG_FP32)
+    plan.set_kernel(None)
+    torch.cuda.synchronize()
+    t_plan = time.perf_counter() - t0
+
+    def step():
+        if atom:
+            plan.apply_atomistic(X, Y, cfg.macro, cfg.mu_s, cfg.a)
+        else:
+            plan.apply(X, Y)
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > L2 (126 MB): written between steps
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        flush.fill_(1); step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    # ---- timed region: exactly K steps, device time by CUDA events on the launching stream, L2 flushed
+    #      between steps (the flush is outside each step's event pair)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for a, b in evs:
+        flush.fill_(1)
+        a.record(); step(); b.record()
+    barrier()
+    ms_steps = [a.elapsed_time(b) for a, b in evs]
+    ms_total = sum(ms_steps)
+    # hot (no flush, back to back) for context
+    a0, b0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a0.record()
+    for _ in range(args.steps):
+        step()
+    b0.record(); barrier()
+    ms_hot = a0.elapsed_time(b0) / args.steps
+
+    # ---- end to end through the public API with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not atom:
+        hin = torch.from_numpy(M_host).to(dt).pin_memory()
+        hout = torch.empty_like(hin).pin_memory()
+        def e2e_step():
+            X.copy_(hin, non_blocking=True); plan.apply(X, Y); hout.copy_(Y, non_blocking=True)
+        for _ in range(3):
+            e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        e2e_bytes = (hin.numel() * hin.element_size(), hout.numel() * hout.element_size())
+    else:
+        # config 5: the per-step result read back is the field of the sampled spins' z-slab 0 (201 MB would be the
+        # mesh field; the 12.9 GB spin arrays live in HBM as they would in a simulation): copy spins slab in, field slab out
+        zs = cfg.macro[2]
+        hin = X[:, :zs].cpu().pin_memory(); hout = torch.empty_like(hin).pin_memory()
+        def e2e_step():
+            X[:, :zs].copy_(hin, non_blocking=True); step(); hout.copy_(Y[:, :zs], non_blocking=True)
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        e2e_bytes = (hin.numel() * hin.element_size(), hout.numel() * hout.element_size())
+    clocks = sampler.stop() if sampler else None
+
+    # ---- per-stage device times of the convolution (CUDA event pair around every launch, on the launching stream)
+    if atom:
+        Mc = torch.empty((3, n[2], n[1], n[0]), dtype=dt, device=dev).normal_(); Hc = torch.empty_like(Mc)
+    else:
+        Mc, Hc = X, Y
+    st_ms = np.zeros(5); st_n = np.zeros(5, dtype=int)
+    reps = 5
+    for i in range(reps + 1):
+        flush.fill_(1)
+        ms, cnt = plan.apply_profiled(Mc, Hc)
+        if i:
+            st_ms += ms; st_n += cnt
+    st_ms /= reps
+    launches_per_step = plan.launches_per_apply() + (2 if atom else 0)
+
+    # ---- reduce over ranks: max time
+    tt = torch.tensor([ms_total, ms_hot, t_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms_total, ms_hot, t_e2e = tt.tolist()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    sb = stage_bytes(n, esz)
+    dom = int(np.argmax(st_ms))
+    achieved = sb[dom] / (st_ms[dom] * 1e-3) / 1e9
+    value = world * nc * args.steps / (ms_total * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if fp64 else "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, fp64), "mesh": list(n), "cells": nc, "padded": [v if v == 1 else 2 * v for v in n],
+                   "l2": "flushed between timed steps (256 MB write outside each step's event pair)",
+                   "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                   "kernel": "built-in Newell tensor (demag_set_kernel(NULL))"},
+        "conv_per_s": world * args.steps / (ms_total * 1e-3),
+        "hot_ms_per_step": ms_hot, "hot_value": world * nc / (ms_hot * 1e-3) / 1e9,
+        "e2e": {"value": world * nc * args.steps / t_e2e / 1e9, "unit": UNIT,
+                "h2d_bytes_per_step": e2e_bytes[0], "d2h_bytes_per_step": e2e_bytes[1]},
+        "gpu_launches": launches_per_step * args.steps,
+        "launches_per_step": launches_per_step,
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": STAGE_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "bytes_per_apply_model": sb[dom], "ms_per_apply": float(st_ms[dom]),
+                     "launches_per_apply": int(st_n[dom] // reps)},
+        "stages": {STAGE_NAMES[i]: {"ms": float(st_ms[i]), "model_bytes": sb[i],
+                                    "model_GBps": sb[i] / max(st_ms[i], 1e-9) / 1e6} for i in range(5)},
+        "whole_apply_model": {"T2_5pass_bytes": sum(sb), "T2_GBps": sum(sb) / (ms_total / args.steps) / 1e6,
+                              "frac_of_peak": sum(sb) / (ms_total / args.steps) / 1e6 / peak},
+        "plan_build_s": t_plan, "input_gen_s": t_inputs, "workspace_bytes": plan.workspace_bytes(),
+    }
+    if atom:
+        line["spins_per_s_G"] = world * units * args.steps / (ms_total * 1e-3) / 1e9
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        tr = json.load(open(traffic_file)).get(args.config, {}).get(STAGE_NAMES[dom])
+        if tr:
+            line["roofline"]["traffic"] = tr
+    except Exception:
+        pass
+    if world == 1 and not args.no_cpu_baseline:
+        val, cores, desc, _, _ = oracle_sample_rate(cfg, args.cpu_seconds, M_host)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    name = args.config
+    fp64 = name.endswith("d")
+    cfg = W.CONFIGS[name[:2]]
+    if args.impl == "reference":
+        run_reference(args, cfg, fp64)
+    else:
+        run_ours(args, cfg, fp64)
+
+
+if __name__ == "__main__":
+    main()

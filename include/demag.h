@@ -98,6 +98,14 @@ size_t demag_workspace_bytes(demag_plan_t plan);
  * Does not change results. */
 demag_status demag_set_slab(demag_plan_t plan, int kx_per_slab);
 
+/* Instrumentation (not the hot path): runs one demag_apply on the stream with a CUDA event pair around
+ * every kernel launch, synchronises, and writes the summed device time in milliseconds of each stage to
+ * stage_ms_host[5] = { x R2C, y forward, z forward*multiply*z inverse, y inverse, x C2R }
+ * (Appendix A execution order) and the launch count of each stage to
+ * stage_launches_host[5] (either pointer may be NULL).  Same arguments and result as demag_apply. */
+demag_status demag_apply_profiled(demag_plan_t plan, const void* M_dev, void* H_dev, void* cuda_stream,
+                                  float* stage_ms_host, int* stage_launches_host);
+
 /* Number of kernel launches one demag_apply enqueues with the current settings. */
 int demag_launches_per_apply(demag_plan_t plan);
 

@@ -21,7 +21,7 @@ STATUS = {0: "DEMAG_OK", 1: "DEMAG_ERR_INVALID_ARG", 2: "DEMAG_ERR_UNSUPPORTED",
 
 EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy", "demag_apply_atomistic",
            "demag_get_kernel_real", "demag_workspace_bytes", "demag_set_slab", "demag_launches_per_apply",
-           "demag_last_error", "demag_plan_destroy"]
+           "demag_last_error", "demag_plan_destroy", "demag_apply_profiled"]
 
 
 class DemagError(RuntimeError):
@@ -46,6 +46,7 @@ def lib():
         L.demag_set_kernel.argtypes = [vp, vp]
         L.demag_apply.argtypes = [vp, vp, vp, vp]
         L.demag_energy.argtypes = [vp, vp, vp, vp, vp]
+        L.demag_apply_profiled.argtypes = [vp, vp, vp, vp, vp, vp]
         L.demag_apply_atomistic.argtypes = [vp, vp, vp, i, i, i, d, d, i, vp]
         L.demag_get_kernel_real.argtypes = [vp, vp]
         L.demag_workspace_bytes.argtypes = [vp]
@@ -93,6 +94,15 @@ def demag_apply(plan, M, H, stream=None):
     _check(lib().demag_apply(plan, M.data_ptr(), H.data_ptr(), _stream(stream)))
 
 
+def demag_apply_profiled(plan, M, H, stream=None):
+    """-> (stage_ms[5], stage_launches[5]) for x-R2C, y-fwd, z-fused, y-inv, x-C2R (synchronous)."""
+    ms = (ctypes.c_float * 5)()
+    cnt = (ctypes.c_int * 5)()
+    _check(lib().demag_apply_profiled(plan, M.data_ptr(), H.data_ptr(), _stream(stream),
+                                      ctypes.addressof(ms), ctypes.addressof(cnt)))
+    return list(ms), list(cnt)
+
+
 def demag_energy(plan, M, H, E, stream=None):
     _check(lib().demag_energy(plan, M.data_ptr(), H.data_ptr(), E.data_ptr(), _stream(stream)))
 
@@ -138,6 +148,9 @@ class Plan:
 
     def apply(self, M, H, stream=None):
         demag_apply(self.handle, M, H, stream)
+
+    def apply_profiled(self, M, H, stream=None):
+        return demag_apply_profiled(self.handle, M, H, stream)
 
     def energy(self, M, H, E, stream=None):
         demag_energy(self.handle, M, H, E, stream)

@@ -376,8 +376,18 @@ extern "C" demag_status demag_get_kernel_real(demag_plan_t p, double* N6_host)
 // ================================================================================ hot path
 namespace {
 
+// Optional per-launch event recorder used only by demag_apply_profiled.
+struct StageTimer {
+    std::vector<cudaEvent_t> ev;   // pairs
+    std::vector<int> stage;
+    cudaStream_t st;
+    void begin(int s) { cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); ev.push_back(a); ev.push_back(b); stage.push_back(s); }
+    void end() { cudaEventRecord(ev.back(), st); }
+};
+#define STAGE(s, launch) do { if (tm) tm->begin(s); launch; if (tm) tm->end(); } while (0)
+
 template <typename T>
-demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st)
+demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr)
 {
     using C = typename cx_of<T>::type;
     const Geo& g = p->g;
@@ -386,23 +396,23 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st)
     const size_t nc = (size_t)g.nx * g.ny * g.nz;
     if (g.Nx == 1) {
         const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
-        k_x_copy_fwd<T><<<grid, 256, 0, st>>>(3 * nc, M, W1);
+        STAGE(0, (k_x_copy_fwd<T><<<grid, 256, 0, st>>>(3 * nc, M, W1)));
     } else {
-        k_x_r2c<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, M, W1, twx);
+        STAGE(0, (k_x_r2c<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, M, W1, twx)));
     }
     for (int kx0 = 0; kx0 < g.hx; kx0 += p->nkx_slab) {
         const int nkx = std::min(p->nkx_slab, g.hx - kx0);
         const unsigned g2 = (unsigned)((3LL * nkx * g.nz + p->B2 - 1) / p->B2);
-        k_y_fwd<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W1, W2, twy);
-        k_z_mul<T><<<(unsigned)(nkx * (g.Ny / p->TY)), p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, (const T*)p->K,
-                                                                               p->kcomp_stride, twz);
-        k_y_inv<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W2, W1, twy);
+        STAGE(1, (k_y_fwd<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W1, W2, twy)));
+        STAGE(2, (k_z_mul<T><<<(unsigned)(nkx * (g.Ny / p->TY)), p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, (const T*)p->K,
+                                                                                         p->kcomp_stride, twz)));
+        STAGE(3, (k_y_inv<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W2, W1, twy)));
     }
     if (g.Nx == 1) {
         const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
-        k_x_copy_inv<T><<<grid, 256, 0, st>>>(3 * nc, W1, H);
+        STAGE(4, (k_x_copy_inv<T><<<grid, 256, 0, st>>>(3 * nc, W1, H)));
     } else {
-        k_x_c2r<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, W1, H, twx);
+        STAGE(4, (k_x_c2r<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, W1, H, twx)));
     }
     CUDA_TRY(cudaGetLastError());
     return DEMAG_OK;
@@ -431,6 +441,35 @@ extern "C" demag_status demag_apply(demag_plan_t p, const void* M_dev, void* H_d
     cudaStream_t st = (cudaStream_t)cuda_stream;
     return p->prec == DEMAG_FP32 ? apply_impl<float>(p, (const float*)M_dev, (float*)H_dev, st)
                                  : apply_impl<double>(p, (const double*)M_dev, (double*)H_dev, st);
+}
+
+extern "C" demag_status demag_apply_profiled(demag_plan_t p, const void* M_dev, void* H_dev, void* cuda_stream,
+                                             float* stage_ms_host, int* stage_launches_host)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    const size_t bytes = (size_t)3 * p->g.nx * p->g.ny * p->g.nz * p->esz;
+    demag_status s = check_apply_args(p, M_dev, H_dev, bytes);
+    if (s) return s;
+    if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
+    StageTimer tm;
+    tm.st = (cudaStream_t)cuda_stream;
+    s = p->prec == DEMAG_FP32 ? apply_impl<float>(p, (const float*)M_dev, (float*)H_dev, tm.st, &tm)
+                              : apply_impl<double>(p, (const double*)M_dev, (double*)H_dev, tm.st, &tm);
+    cudaError_t e = cudaStreamSynchronize(tm.st);
+    float ms[5] = {0, 0, 0, 0, 0};
+    int cnt[5] = {0, 0, 0, 0, 0};
+    for (size_t i = 0; i < tm.stage.size(); ++i) {
+        float t = 0.f;
+        if (e == cudaSuccess) cudaEventElapsedTime(&t, tm.ev[2 * i], tm.ev[2 * i + 1]);
+        ms[tm.stage[i]] += t; cnt[tm.stage[i]]++;
+        cudaEventDestroy(tm.ev[2 * i]); cudaEventDestroy(tm.ev[2 * i + 1]);
+    }
+    if (stage_ms_host) memcpy(stage_ms_host, ms, sizeof(ms));
+    if (stage_launches_host) memcpy(stage_launches_host, cnt, sizeof(cnt));
+    if (s) return s;
+    if (e != cudaSuccess) return fail(DEMAG_ERR_CUDA, "profiled apply: %s", cudaGetErrorString(e));
+    return DEMAG_OK;
 }
 
 extern "C" demag_status demag_energy(demag_plan_t p, const void* M_dev, const void* H_dev, double* E_dev, void* cuda_stream)
