@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(512) k_sym_axis(const double* __restrict__ in,
         s[swz<3>(e * B + b)] = make_double2(v, 0.0);
     }
     __syncthreads();
-    fft_tile<double, false>(s, lN, B, tw, 0, tid, nthr);
+    fft_tile<double, false, true>(s, lN, B, B, tw, 0, tid, nthr);
     double* dst = out + o * so_out + i0;
     for (int idx = tid; idx < nout * B; idx += nthr) {
         const int b = idx % B, k = idx / B;
@@ -179,15 +179,21 @@ __global__ void __launch_bounds__(512) k_sym_axis(const double* __restrict__ in,
     }
 }
 
-// K[kx][kz][ky (pitch)] = scale * A[kz][ky][kx]
+// K[kx][kz'][py] = sign_y * scale * A[kz'][ky'][kx],  ky = freq_of_pos(py), ky' = min(ky, Ny-ky),
+// sign_y = -1 on mirrored ky of a component that is odd in y (the y axis is stored unpacked, in the
+// digit-reversed "position" order in which the y FFT leaves W2, so the hot path never permutes).
 template <typename T>
 __global__ void k_pack_kernel(const double* __restrict__ A, T* __restrict__ K, int hx, int kpy, int kpz,
-                              int kpitch, double scale)
+                              int Ny, int lNy, int par_y, double scale)
 {
-    const size_t n = (size_t)hx * kpz * kpy;
+    const size_t n = (size_t)hx * kpz * Ny;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const int ky = (int)(i % kpy), kz = (int)((i / kpy) % kpz), kx = (int)(i / ((size_t)kpy * kpz));
-        K[((size_t)kx * kpz + kz) * kpitch + ky] = (T)(scale * A[((size_t)kz * kpy + ky) * hx + kx]);
+        const int py = (int)(i % Ny), kz = (int)((i / Ny) % kpz), kx = (int)(i / ((size_t)Ny * kpz));
+        const int ky = freq_of_pos(py, lNy);
+        const bool my = 2 * ky > Ny;
+        const int kyp = my ? Ny - ky : ky;
+        const double sg = (my && par_y < 0) ? -1.0 : 1.0;
+        K[i] = (T)(sg * scale * A[((size_t)kz * kpy + kyp) * hx + kx]);
     }
 }
 

@@ -3,14 +3,19 @@
 // Appendix A :296-321 xFFT / yFFT / zFFT).  sm_100a only; no cuFFT.
 //
 // A tile is a logical array  s[p][b]  of complex numbers, p = 0..L-1 the transform axis, b = 0..B-1
-// the batch (independent lines), flattened q = p*B + b and XOR-swizzled so that both unit-stride and
-// power-of-two-strided accesses of a half warp fall in distinct banks (no padding bytes).
+// the batch (independent lines), stored at  p*pitch + b.  Two addressing modes:
+//   SWZ = false  batch-fastest tiles with >= 16 lines (or an odd pitch): a half warp touches 16
+//                consecutive batch slots, so every access is conflict free with plain addressing;
+//   SWZ = true   few long lines (B < 16): the flattened index is XOR-swizzled so that unit-stride and
+//                power-of-two-strided accesses both spread over the banks (no padding bytes).
 //
 // Forward  = decimation in frequency, in place, natural order in  -> digit-reversed order out.
 // Inverse  = decimation in time,      in place, digit-reversed in -> natural order out.
-// The convolution never needs the permutation undone in shared memory: the loaders / storers address
-// the tile through pos_of_freq().  Neither direction scales; the 1/(Nx Ny Nz) lives in the kernel
-// spectrum (R3).
+// The convolution never undoes the permutation in shared memory: loaders / storers address the tile
+// through pos_of_freq().  Neither direction scales; 1/(Nx Ny Nz) lives in the kernel spectrum (R3).
+//
+// fp32 complex arithmetic uses Blackwell's packed f32x2 instructions (FADD2 / FMUL2 / FFMA2): one
+// issue slot per complex add, two per complex multiply.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -24,13 +29,69 @@ template <> struct cx_of<float>  { using type = float2;  static constexpr int RO
 template <> struct cx_of<double> { using type = double2; static constexpr int ROWBITS = 3; };
 
 template <typename C> __device__ __forceinline__ C cmake(decltype(C::x) a, decltype(C::x) b) { C r; r.x = a; r.y = b; return r; }
-template <typename C> __device__ __forceinline__ C cadd(C a, C b) { return cmake<C>(a.x + b.x, a.y + b.y); }
-template <typename C> __device__ __forceinline__ C csub(C a, C b) { return cmake<C>(a.x - b.x, a.y - b.y); }
-template <typename C> __device__ __forceinline__ C cmul(C a, C b) { return cmake<C>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-template <typename C> __device__ __forceinline__ C cmulc(C a, C b) { /* a * conj(b) */ return cmake<C>(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }
-template <typename C> __device__ __forceinline__ C cconj(C a) { return cmake<C>(a.x, -a.y); }
-// multiply by -i (forward) or +i (inverse)
-template <bool INV, typename C> __device__ __forceinline__ C cmul_mi(C a) { return INV ? cmake<C>(-a.y, a.x) : cmake<C>(a.y, -a.x); }
+
+// ---- packed fp32 pair primitives ---------------------------------------------------------------
+__device__ __forceinline__ float2 p_add(float2 a, float2 b)
+{
+    float2 r;
+    asm("{.reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; add.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc;}"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 p_sub(float2 a, float2 b)
+{
+    float2 r;
+    asm("{.reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; sub.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc;}"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 p_mul(float2 a, float2 b)
+{
+    float2 r;
+    asm("{.reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mul.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc;}"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 p_fma(float2 a, float2 b, float2 c)
+{
+    float2 r;
+    asm("{.reg .b64 ra, rb, rc, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mov.b64 rc, {%6,%7}; fma.rn.f32x2 rd, ra, rb, rc; mov.b64 {%0,%1}, rd;}"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return r;
+}
+__device__ __forceinline__ double2 p_add(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 p_sub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 p_mul(double2 a, double2 b) { return make_double2(a.x * b.x, a.y * b.y); }
+__device__ __forceinline__ double2 p_fma(double2 a, double2 b, double2 c) { return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
+
+// ---- complex helpers -----------------------------------------------------------------------------
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { return p_add(a, b); }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { return p_sub(a, b); }
+template <typename C> __device__ __forceinline__ C cswap(C a) { return cmake<C>(a.y, a.x); }
+// a * w
+template <typename C> __device__ __forceinline__ C cmul(C a, C w)
+{
+    return p_fma(cmake<C>(a.x, a.x), w, p_mul(cmake<C>(a.y, a.y), cmake<C>(-w.y, w.x)));
+}
+// a * conj(w)
+template <typename C> __device__ __forceinline__ C cmulc(C a, C w)
+{
+    return p_fma(cmake<C>(a.x, a.x), cmake<C>(w.x, -w.y), p_mul(cmake<C>(a.y, a.y), cmake<C>(w.y, w.x)));
+}
+// a + (-i) b  (forward rotation)  /  a + (+i) b
+template <typename C> __device__ __forceinline__ C cadd_mi(C a, C b)
+{
+    using T = decltype(C::x);
+    return p_fma(cswap(b), cmake<C>((T)1, (T)-1), a);
+}
+template <typename C> __device__ __forceinline__ C cadd_pi(C a, C b)
+{
+    using T = decltype(C::x);
+    return p_fma(cswap(b), cmake<C>((T)-1, (T)1), a);
+}
+// a + rot(b), a - rot(b) with rot = multiplication by -i (forward) or +i (inverse)
+template <bool INV, typename C> __device__ __forceinline__ C cadd_rot(C a, C b) { return INV ? cadd_pi(a, b) : cadd_mi(a, b); }
+template <bool INV, typename C> __device__ __forceinline__ C csub_rot(C a, C b) { return INV ? cadd_mi(a, b) : cadd_pi(a, b); }
 
 // XOR swizzle of the flattened element index: rows of 2^ROWBITS elements (= 128 bytes), the in-row
 // index is XORed with the folded row number.
@@ -40,13 +101,7 @@ template <int ROWBITS> __device__ __forceinline__ int swz(int q)
     const int f = (r ^ (r >> ROWBITS) ^ (r >> (2 * ROWBITS)) ^ (r >> (3 * ROWBITS))) & ((1 << ROWBITS) - 1);
     return q ^ f;
 }
-
-// Pass schedule for length 2^log2L: radix-8 passes, then one radix-4 or radix-2 pass.
-struct Sched {
-    int log2L;
-    __device__ __host__ __forceinline__ int npass() const { return (log2L + 2) / 3; }
-    __device__ __host__ __forceinline__ int lr(int i) const { return (i < log2L / 3) ? 3 : (log2L % 3); }
-};
+template <bool SWZ, int ROWBITS> __device__ __forceinline__ int taddr(int q) { return SWZ ? swz<ROWBITS>(q) : q; }
 
 // position (in the digit-reversed tile) that holds frequency k after the forward passes
 __device__ __forceinline__ int pos_of_freq(int k, int log2L)
@@ -67,46 +122,79 @@ __device__ __forceinline__ int freq_of_pos(int p, int log2L)
 }
 
 // ---- radix butterflies in registers: natural order in, natural order out, unnormalised ------------
-template <bool INV, typename C> __device__ __forceinline__ void dft2(C* a)
+// HALF_IN: the upper half of the inputs is known to be zero (zero padding).
+template <bool INV, bool HALF_IN, typename C> __device__ __forceinline__ void dft2(C* a)
 {
+    if (HALF_IN) { a[1] = a[0]; return; }
     const C t = a[0]; a[0] = cadd(t, a[1]); a[1] = csub(t, a[1]);
 }
-template <bool INV, typename C> __device__ __forceinline__ void dft4(C* a)
+template <bool INV, bool HALF_IN, typename C> __device__ __forceinline__ void dft4(C* a)
 {
-    const C d0 = cadd(a[0], a[2]), d2 = csub(a[0], a[2]);
-    const C d1 = cadd(a[1], a[3]), d3 = cmul_mi<INV>(csub(a[1], a[3]));
+    C d0, d2;
+    if (HALF_IN) { d0 = a[0]; d2 = a[0]; } else { d0 = cadd(a[0], a[2]); d2 = csub(a[0], a[2]); }
+    C d1, t;
+    if (HALF_IN) { d1 = a[1]; t = a[1]; } else { d1 = cadd(a[1], a[3]); t = csub(a[1], a[3]); }
     a[0] = cadd(d0, d1); a[2] = csub(d0, d1);
-    a[1] = cadd(d2, d3); a[3] = csub(d2, d3);
+    a[1] = cadd_rot<INV>(d2, t); a[3] = csub_rot<INV>(d2, t);
 }
-template <bool INV, typename C> __device__ __forceinline__ void dft8(C* a)
+template <bool INV, bool HALF_IN, typename C> __device__ __forceinline__ void dft8(C* a)
 {
     using T = decltype(C::x);
     const T h = (T)0.70710678118654752440;
     C e[4], o[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) { e[j] = cadd(a[j], a[j + 4]); o[j] = csub(a[j], a[j + 4]); }
-    // o[j] *= w8^j   (forward w8 = exp(-i pi/4); inverse conj)
-    {
-        const C t1 = o[1], t3 = o[3];
-        if (!INV) { o[1] = cmake<C>((t1.x + t1.y) * h, (t1.y - t1.x) * h); o[3] = cmake<C>((t3.y - t3.x) * h, -(t3.x + t3.y) * h); }
-        else      { o[1] = cmake<C>((t1.x - t1.y) * h, (t1.x + t1.y) * h); o[3] = cmake<C>(-(t3.x + t3.y) * h, (t3.x - t3.y) * h); }
-        o[2] = cmul_mi<INV>(o[2]);
+    for (int j = 0; j < 4; ++j) {
+        if (HALF_IN) { e[j] = a[j]; o[j] = a[j]; } else { e[j] = cadd(a[j], a[j + 4]); o[j] = csub(a[j], a[j + 4]); }
     }
-    dft4<INV>(e); dft4<INV>(o);
+    // o[1] *= w8, o[3] *= w8^3 (forward w8 = exp(-i pi/4)); o[2]'s rotation is folded into the dft4 below
+    const C hh = cmake<C>(h, h);
+    if (!INV) {
+        o[1] = p_fma(cswap(o[1]), cmake<C>(h, -h), p_mul(o[1], hh));            // (x+y, y-x) h
+        o[3] = p_fma(cswap(o[3]), cmake<C>(h, -h), p_mul(o[3], cmake<C>(-h, -h)));  // (y-x, -x-y) h
+    } else {
+        o[1] = p_fma(cswap(o[1]), cmake<C>(-h, h), p_mul(o[1], hh));            // (x-y, x+y) h
+        o[3] = p_fma(cswap(o[3]), cmake<C>(-h, h), p_mul(o[3], cmake<C>(-h, -h)));  // (-x-y, x-y) h
+    }
+    dft4<INV, false>(e);
+    {   // dft4 of (o0, o1, rot(o2), o3) with the rotation of o2 folded in
+        const C d0 = cadd_rot<INV>(o[0], o[2]), d2 = csub_rot<INV>(o[0], o[2]);
+        const C d1 = cadd(o[1], o[3]), t = csub(o[1], o[3]);
+        o[0] = cadd(d0, d1); o[2] = csub(d0, d1);
+        o[1] = cadd_rot<INV>(d2, t); o[3] = csub_rot<INV>(d2, t);
+    }
 #pragma unroll
     for (int j = 0; j < 4; ++j) { a[2 * j] = e[j]; a[2 * j + 1] = o[j]; }
 }
-template <int LR, bool INV, typename C> __device__ __forceinline__ void dftR(C* a)
+template <int LR, bool INV, bool HALF_IN, typename C> __device__ __forceinline__ void dftR(C* a)
 {
-    if (LR == 3) dft8<INV>(a); else if (LR == 2) dft4<INV>(a); else dft2<INV>(a);
+    if (LR == 3) dft8<INV, HALF_IN>(a); else if (LR == 2) dft4<INV, HALF_IN>(a); else if (LR == 1) dft2<INV, HALF_IN>(a);
 }
 
-template <typename C> __device__ __forceinline__ C ldg_c(const C* p) { return __ldg(p); }
+// a[m] *= w^m (forward) or conj(w)^m (inverse), m = 1..R-1, w^m read / derived from the table at j*m
+template <int LR, bool INV, typename C>
+__device__ __forceinline__ void twiddle(C* a, const C* __restrict__ tw, int j)
+{
+    if (LR == 3) {
+        const C w1 = __ldg(tw + j), w2 = __ldg(tw + 2 * j), w4 = __ldg(tw + 4 * j);
+        const C w3 = cmul(w1, w2), w5 = cmul(w1, w4), w6 = cmul(w2, w4), w7 = cmul(w3, w4);
+        if (!INV) { a[1] = cmul(a[1], w1); a[2] = cmul(a[2], w2); a[3] = cmul(a[3], w3); a[4] = cmul(a[4], w4);
+                    a[5] = cmul(a[5], w5); a[6] = cmul(a[6], w6); a[7] = cmul(a[7], w7); }
+        else      { a[1] = cmulc(a[1], w1); a[2] = cmulc(a[2], w2); a[3] = cmulc(a[3], w3); a[4] = cmulc(a[4], w4);
+                    a[5] = cmulc(a[5], w5); a[6] = cmulc(a[6], w6); a[7] = cmulc(a[7], w7); }
+    } else if (LR == 2) {
+        const C w1 = __ldg(tw + j), w2 = __ldg(tw + 2 * j); const C w3 = cmul(w1, w2);
+        if (!INV) { a[1] = cmul(a[1], w1); a[2] = cmul(a[2], w2); a[3] = cmul(a[3], w3); }
+        else      { a[1] = cmulc(a[1], w1); a[2] = cmulc(a[2], w2); a[3] = cmulc(a[3], w3); }
+    } else if (LR == 1) {
+        const C w1 = __ldg(tw + j);
+        a[1] = INV ? cmulc(a[1], w1) : cmul(a[1], w1);
+    }
+}
 
-// One pass over the tile.  LR = log2 radix, ls = log2 S (stride between butterfly legs, in points).
-// tw: table exp(-2 pi i k / Ntab); lt = log2(Ntab / L)  (so w_L^j = tw[j << lt]).
-template <typename T, int LR, bool INV>
-__device__ __forceinline__ void fft_pass(typename cx_of<T>::type* s, int log2L, int ls, int B,
+// One in-place pass over the tile.  LR = log2 radix, ls = log2 S (stride between butterfly legs, in
+// points).  tw: table exp(-2 pi i k / Ntab); lt = log2(Ntab / L)  (so w_L^j = tw[j << lt]).
+template <typename T, int LR, bool INV, bool SWZ>
+__device__ __forceinline__ void fft_pass(typename cx_of<T>::type* s, int log2L, int ls, int B, int pitch,
                                          const typename cx_of<T>::type* __restrict__ tw, int lt,
                                          int tid, int nthr)
 {
@@ -116,69 +204,48 @@ __device__ __forceinline__ void fft_pass(typename cx_of<T>::type* s, int log2L, 
     const int nb = (B << log2L) >> LR;           // butterflies in the tile
     const int S = 1 << ls;
     const int ltw = log2L - LR - ls + lt;        // w_n^j = tw[j << ltw],  n = R*S
-    const bool pow2B = (B & (B - 1)) == 0;
-    const int lB = 31 - __clz(B);
-    for (int t = tid; t < nb; t += nthr) {
-        int i, b;
-        if (pow2B) { i = t >> lB; b = t & (B - 1); } else { i = t / B; b = t - i * B; }
+    const int stride = pitch << ls;
+    // lines fastest: butterfly t = i*B + b; (i, b) advance incrementally by nthr per iteration (no division in the loop)
+    int b = tid % B, i = tid / B;
+    const int db = nthr % B, di = nthr / B;
+    for (int t = tid; t < nb; t += nthr, b += db, i += di) {
+        if (b >= B) { b -= B; ++i; }
         const int lo = i & (S - 1);
         const int p0 = ((i >> ls) << (ls + LR)) + lo;
+        const int q0 = p0 * pitch + b;
         C a[R];
-        int addr[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) { addr[r] = swz<RB>((p0 + (r << ls)) * B + b); a[r] = s[addr[r]]; }
+        for (int r = 0; r < R; ++r) a[r] = s[taddr<SWZ, RB>(q0 + r * stride)];
         if (!INV) {
-            dftR<LR, false>(a);
-            if (ls > 0) {
-                const int j = lo << ltw;
-                if (LR == 3) {
-                    const C w1 = ldg_c(tw + j), w2 = ldg_c(tw + 2 * j), w4 = ldg_c(tw + 4 * j);
-                    const C w3 = cmul(w1, w2), w5 = cmul(w1, w4), w6 = cmul(w2, w4), w7 = cmul(w3, w4);
-                    a[1] = cmul(a[1], w1); a[2] = cmul(a[2], w2); a[3] = cmul(a[3], w3); a[4] = cmul(a[4], w4);
-                    a[5] = cmul(a[5], w5); a[6] = cmul(a[6], w6); a[7] = cmul(a[7], w7);
-                } else if (LR == 2) {
-                    const C w1 = ldg_c(tw + j), w2 = ldg_c(tw + 2 * j); const C w3 = cmul(w1, w2);
-                    a[1] = cmul(a[1], w1); a[2] = cmul(a[2], w2); a[3] = cmul(a[3], w3);
-                } else { a[1] = cmul(a[1], ldg_c(tw + j)); }
-            }
+            dftR<LR, false, false>(a);
+            if (ls > 0) twiddle<LR, false>(a, tw, lo << ltw);
         } else {
-            if (ls > 0) {
-                const int j = lo << ltw;
-                if (LR == 3) {
-                    const C w1 = ldg_c(tw + j), w2 = ldg_c(tw + 2 * j), w4 = ldg_c(tw + 4 * j);
-                    const C w3 = cmul(w1, w2), w5 = cmul(w1, w4), w6 = cmul(w2, w4), w7 = cmul(w3, w4);
-                    a[1] = cmulc(a[1], w1); a[2] = cmulc(a[2], w2); a[3] = cmulc(a[3], w3); a[4] = cmulc(a[4], w4);
-                    a[5] = cmulc(a[5], w5); a[6] = cmulc(a[6], w6); a[7] = cmulc(a[7], w7);
-                } else if (LR == 2) {
-                    const C w1 = ldg_c(tw + j), w2 = ldg_c(tw + 2 * j); const C w3 = cmul(w1, w2);
-                    a[1] = cmulc(a[1], w1); a[2] = cmulc(a[2], w2); a[3] = cmulc(a[3], w3);
-                } else { a[1] = cmulc(a[1], ldg_c(tw + j)); }
-            }
-            dftR<LR, true>(a);
+            if (ls > 0) twiddle<LR, true>(a, tw, lo << ltw);
+            dftR<LR, true, false>(a);
         }
 #pragma unroll
-        for (int r = 0; r < R; ++r) s[addr[r]] = a[r];
+        for (int r = 0; r < R; ++r) s[taddr<SWZ, RB>(q0 + r * stride)] = a[r];
     }
 }
 
 // All passes of a length-2^log2L transform on the tile s[L][B].  Caller has synchronised before
 // (tile fully written); on return the tile is synchronised (all threads see the result).
-template <typename T, bool INV>
-__device__ __forceinline__ void fft_tile(typename cx_of<T>::type* s, int log2L, int B,
+template <typename T, bool INV, bool SWZ>
+__device__ __forceinline__ void fft_tile(typename cx_of<T>::type* s, int log2L, int B, int pitch,
                                          const typename cx_of<T>::type* __restrict__ tw, int lt,
                                          int tid, int nthr)
 {
     const int n8 = log2L / 3, rem = log2L % 3;
     if (!INV) {
         int ls = log2L;
-        for (int i = 0; i < n8; ++i) { ls -= 3; fft_pass<T, 3, false>(s, log2L, ls, B, tw, lt, tid, nthr); __syncthreads(); }
-        if (rem == 2) { fft_pass<T, 2, false>(s, log2L, 0, B, tw, lt, tid, nthr); __syncthreads(); }
-        else if (rem == 1) { fft_pass<T, 1, false>(s, log2L, 0, B, tw, lt, tid, nthr); __syncthreads(); }
+        for (int i = 0; i < n8; ++i) { ls -= 3; fft_pass<T, 3, false, SWZ>(s, log2L, ls, B, pitch, tw, lt, tid, nthr); __syncthreads(); }
+        if (rem == 2) { fft_pass<T, 2, false, SWZ>(s, log2L, 0, B, pitch, tw, lt, tid, nthr); __syncthreads(); }
+        else if (rem == 1) { fft_pass<T, 1, false, SWZ>(s, log2L, 0, B, pitch, tw, lt, tid, nthr); __syncthreads(); }
     } else {
-        if (rem == 2) { fft_pass<T, 2, true>(s, log2L, 0, B, tw, lt, tid, nthr); __syncthreads(); }
-        else if (rem == 1) { fft_pass<T, 1, true>(s, log2L, 0, B, tw, lt, tid, nthr); __syncthreads(); }
+        if (rem == 2) { fft_pass<T, 2, true, SWZ>(s, log2L, 0, B, pitch, tw, lt, tid, nthr); __syncthreads(); }
+        else if (rem == 1) { fft_pass<T, 1, true, SWZ>(s, log2L, 0, B, pitch, tw, lt, tid, nthr); __syncthreads(); }
         int ls = rem;
-        for (int i = 0; i < n8; ++i) { fft_pass<T, 3, true>(s, log2L, ls, B, tw, lt, tid, nthr); __syncthreads(); ls += 3; }
+        for (int i = 0; i < n8; ++i) { fft_pass<T, 3, true, SWZ>(s, log2L, ls, B, pitch, tw, lt, tid, nthr); __syncthreads(); ls += 3; }
     }
 }
 

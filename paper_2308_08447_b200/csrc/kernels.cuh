@@ -9,7 +9,7 @@
 // Data layout:
 //   M, H  [3][nz][ny][nx] real          W1 [3][hx][nz][ny] complex (y fastest)
 //   W2    [3][nkx][nz][Ny] complex, one L2-resident slab of nkx kx-planes
-//   K     [6][hx][kpz][kpitch] real, ky' fastest, packed over ky' = min(ky, Ny-ky), kz' likewise
+//   K     [6][hx][kpz][Ny] real: z packed over kz' = min(kz, Nz-kz); y unpacked, in W2's position order
 #pragma once
 #include "fft_core.cuh"
 
@@ -26,8 +26,8 @@ struct Geo {
 
 // ------------------------------------------------------------------------------------------ K1
 // tile = R consecutive y rows of one (component, z); smem s[Lc][R], Lc = Nx/2.
-template <typename T>
-__global__ void __launch_bounds__(512) k_x_r2c(Geo g, int R, const T* __restrict__ M,
+template <typename T, bool SWZ>
+__global__ void __launch_bounds__(512) k_x_r2c(Geo g, int R, int pitch, const T* __restrict__ M,
                                                typename cx_of<T>::type* __restrict__ W1,
                                                const typename cx_of<T>::type* __restrict__ twx)
 {
@@ -47,11 +47,11 @@ __global__ void __launch_bounds__(512) k_x_r2c(Geo g, int R, const T* __restrict
         const int b = idx >> g.lLc, m = idx & (Lc - 1);
         C v = cmake<C>((T)0, (T)0);
         if (m < nin) v = *reinterpret_cast<const C*>(M + rowbase + (size_t)b * g.nx + 2 * m);
-        s[swz<RB>(m * R + b)] = v;
+        s[taddr<SWZ, RB>(m * pitch + b)] = v;
     }
     (void)lnin;
     __syncthreads();
-    fft_tile<T, false>(s, g.lLc, R, twx, 1, tid, nthr);
+    fft_tile<T, false, SWZ>(s, g.lLc, R, pitch, twx, 1, tid, nthr);
     const int c = cz / g.nz, z = cz - c * g.nz;
     const size_t plane = (size_t)g.nz * g.ny;
     C* out = W1 + ((size_t)c * g.hx * g.nz + z) * g.ny + y0;
@@ -59,8 +59,8 @@ __global__ void __launch_bounds__(512) k_x_r2c(Geo g, int R, const T* __restrict
     for (int idx = tid; idx < R * g.hx; idx += nthr) {
         int k, b;
         if (pow2R) { k = idx >> lR; b = idx & (R - 1); } else { k = idx / R; b = idx - k * R; }
-        const C Zk = s[swz<RB>(pos_of_freq(k & (Lc - 1), g.lLc) * R + b)];
-        const C Zm = s[swz<RB>(pos_of_freq((Lc - k) & (Lc - 1), g.lLc) * R + b)];
+        const C Zk = s[taddr<SWZ, RB>(pos_of_freq(k & (Lc - 1), g.lLc) * pitch + b)];
+        const C Zm = s[taddr<SWZ, RB>(pos_of_freq((Lc - k) & (Lc - 1), g.lLc) * pitch + b)];
         const C E = cmake<C>((T)0.5 * (Zk.x + Zm.x), (T)0.5 * (Zk.y - Zm.y));
         const C D = cmake<C>(Zk.x - Zm.x, Zk.y + Zm.y);
         const C t = cmul(D, __ldg(twx + k));
@@ -84,8 +84,8 @@ __global__ void k_x_copy_inv(size_t n, const typename cx_of<T>::type* __restrict
 }
 
 // ------------------------------------------------------------------------------------------ K5
-template <typename T>
-__global__ void __launch_bounds__(512) k_x_c2r(Geo g, int R, const typename cx_of<T>::type* __restrict__ W1,
+template <typename T, bool SWZ>
+__global__ void __launch_bounds__(512) k_x_c2r(Geo g, int R, int pitch, const typename cx_of<T>::type* __restrict__ W1,
                                                T* __restrict__ H,
                                                const typename cx_of<T>::type* __restrict__ twx)
 {
@@ -110,23 +110,23 @@ __global__ void __launch_bounds__(512) k_x_c2r(Geo g, int R, const typename cx_o
         const C A = cmake<C>(Xk.x + Xm.x, Xk.y - Xm.y);          // Xk + conj(Xm)
         const C D = cmake<C>(Xk.x - Xm.x, Xk.y + Xm.y);          // Xk - conj(Xm)
         const C u = cmulc(D, __ldg(twx + k));                    // conj(w^k) D
-        s[swz<RB>(pos_of_freq(k, g.lLc) * R + b)] = cmake<C>(A.x - u.y, A.y + u.x);   // A + i u
+        s[taddr<SWZ, RB>(pos_of_freq(k, g.lLc) * pitch + b)] = cmake<C>(A.x - u.y, A.y + u.x);   // A + i u
     }
     __syncthreads();
-    fft_tile<T, true>(s, g.lLc, R, twx, 1, tid, nthr);
+    fft_tile<T, true, SWZ>(s, g.lLc, R, pitch, twx, 1, tid, nthr);
     const int nout = g.nx >> 1;
     const int lno = 31 - __clz(nout);
     const size_t rowbase = ((size_t)cz * g.ny + y0) * g.nx;
     for (int idx = tid; idx < R * nout; idx += nthr) {
         const int b = idx >> lno, m = idx & (nout - 1);
-        *reinterpret_cast<C*>(H + rowbase + (size_t)b * g.nx + 2 * m) = s[swz<RB>(m * R + b)];
+        *reinterpret_cast<C*>(H + rowbase + (size_t)b * g.nx + 2 * m) = s[taddr<SWZ, RB>(m * pitch + b)];
     }
 }
 
 // ------------------------------------------------------------------------------------------ K2 / K4
 // lines l = (c*nkx + kxl)*nz + z of the slab [kx0, kx0+nkx); tile = B consecutive lines; smem s[Ny][B].
-template <typename T>
-__global__ void __launch_bounds__(512) k_y_fwd(Geo g, int B, int kx0, int nkx,
+template <typename T, bool SWZ>
+__global__ void __launch_bounds__(512) k_y_fwd(Geo g, int B, int pitch, int kx0, int nkx,
                                                const typename cx_of<T>::type* __restrict__ W1,
                                                typename cx_of<T>::type* __restrict__ W2,
                                                const typename cx_of<T>::type* __restrict__ twy)
@@ -146,20 +146,20 @@ __global__ void __launch_bounds__(512) k_y_fwd(Geo g, int B, int kx0, int nkx,
             const int z = l % g.nz, ck = l / g.nz, kxl = ck % nkx, c = ck / nkx;
             v = W1[(((size_t)c * g.hx + kx0 + kxl) * g.nz + z) * g.ny + p];
         }
-        s[swz<RB>(p * B + b)] = v;
+        s[taddr<SWZ, RB>(p * pitch + b)] = v;
     }
     (void)lny;
     __syncthreads();
-    fft_tile<T, false>(s, g.lNy, B, twy, 0, tid, nthr);
+    fft_tile<T, false, SWZ>(s, g.lNy, B, pitch, twy, 0, tid, nthr);
     for (int idx = tid; idx < (B << g.lNy); idx += nthr) {
         const int b = idx >> g.lNy, ky = idx & (g.Ny - 1);
         const int l = l0 + b;
-        if (l < nlines) W2[(size_t)l * g.Ny + ky] = s[swz<RB>(pos_of_freq(ky, g.lNy) * B + b)];
+        if (l < nlines) W2[(size_t)l * g.Ny + ky] = s[taddr<SWZ, RB>(ky * pitch + b)];   // W2 keeps position (digit-reversed) order
     }
 }
 
-template <typename T>
-__global__ void __launch_bounds__(512) k_y_inv(Geo g, int B, int kx0, int nkx,
+template <typename T, bool SWZ>
+__global__ void __launch_bounds__(512) k_y_inv(Geo g, int B, int pitch, int kx0, int nkx,
                                                const typename cx_of<T>::type* __restrict__ W2,
                                                typename cx_of<T>::type* __restrict__ W1,
                                                const typename cx_of<T>::type* __restrict__ twy)
@@ -175,77 +175,200 @@ __global__ void __launch_bounds__(512) k_y_inv(Geo g, int B, int kx0, int nkx,
         const int l = l0 + b;
         C v = cmake<C>((T)0, (T)0);
         if (l < nlines) v = W2[(size_t)l * g.Ny + ky];
-        s[swz<RB>(pos_of_freq(ky, g.lNy) * B + b)] = v;
+        s[taddr<SWZ, RB>(ky * pitch + b)] = v;
     }
     __syncthreads();
-    fft_tile<T, true>(s, g.lNy, B, twy, 0, tid, nthr);
+    fft_tile<T, true, SWZ>(s, g.lNy, B, pitch, twy, 0, tid, nthr);
     const int lny = 31 - __clz(g.ny);
     for (int idx = tid; idx < (B << lny); idx += nthr) {
         const int b = idx >> lny, p = idx & (g.ny - 1);
         const int l = l0 + b;
         if (l < nlines) {
             const int z = l % g.nz, ck = l / g.nz, kxl = ck % nkx, c = ck / nkx;
-            W1[(((size_t)c * g.hx + kx0 + kxl) * g.nz + z) * g.ny + p] = s[swz<RB>(p * B + b)];
+            W1[(((size_t)c * g.hx + kx0 + kxl) * g.nz + z) * g.ny + p] = s[taddr<SWZ, RB>(p * pitch + b)];
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------ K3
-// tile = one kx plane x TY consecutive ky x all z x 3 components; smem s[Nz][3*TY].
-// H^_a = sum_b K^_ab M^_b, K^ real and symmetric (PAPER.md:322-326 KernelMultiplication;
-// :255-256 packed by y/z symmetry; parity signs DESIGN.md R1).  In place on the W2 slab.
+// z FFT . kernel multiplication . z IFFT "in the same routine".
+// tile = one kx plane x TY consecutive ky x all z x 3 components; smem s[Nz][3*TY] (batch fastest, so
+// every shared-memory access of a half warp is 16 consecutive slots: conflict free, no swizzle).
+//   first forward pass   reads W2 straight from global (only z < nz: the zero padding is synthesised)
+//   fused middle stage   last forward pass + H^_a = sum_b K^_ab M^_b + first inverse pass, in registers
+//   last inverse pass    writes z < nz straight back to W2 (the crop)
+// H^_a = sum_b K^_ab M^_b, K^ real and symmetric (PAPER.md:322-326 KernelMultiplication; :255-256 packed
+// by y/z symmetry; parity signs DESIGN.md R1).  In place on the W2 slab.
 template <typename T>
-__global__ void __launch_bounds__(512) k_z_mul(Geo g, int TY, int kx0, int nkx,
+struct KernelVals { T xx, yy, zz, xy, xz, yz; };
+
+// K is stored [comp][kx][kz'][py]: z packed over kz' = min(kz, Nz-kz) (sign applied here), y unpacked in the
+// position order of W2 with its parity sign already folded in at plan time.
+template <typename T>
+__device__ __forceinline__ KernelVals<T> load_kernel(const Geo& g, const T* __restrict__ K, size_t kcs, int kx, int py, int kz)
+{
+    const bool mz = (2 * kz > g.Nz);
+    const int kzp = mz ? g.Nz - kz : kz;
+    const size_t ko = ((size_t)kx * g.kpz + kzp) * g.kpitch + py;
+    KernelVals<T> v;
+    v.xx = __ldg(K + ko); v.yy = __ldg(K + kcs + ko); v.zz = __ldg(K + 2 * kcs + ko);
+    v.xy = __ldg(K + 3 * kcs + ko);
+    const T xz = __ldg(K + 4 * kcs + ko), yz = __ldg(K + 5 * kcs + ko);
+    v.xz = mz ? -xz : xz; v.yz = mz ? -yz : yz;
+    return v;
+}
+
+template <typename C, typename T>
+__device__ __forceinline__ void apply_kernel(const KernelVals<T>& k, C& mx, C& my, C& mz)
+{
+    const C kxx = cmake<C>(k.xx, k.xx), kyy = cmake<C>(k.yy, k.yy), kzz = cmake<C>(k.zz, k.zz);
+    const C kxy = cmake<C>(k.xy, k.xy), kxz = cmake<C>(k.xz, k.xz), kyz = cmake<C>(k.yz, k.yz);
+    const C hx = p_fma(kxz, mz, p_fma(kxy, my, p_mul(kxx, mx)));
+    const C hy = p_fma(kyz, mz, p_fma(kyy, my, p_mul(kxy, mx)));
+    const C hz = p_fma(kzz, mz, p_fma(kyz, my, p_mul(kxz, mx)));
+    mx = hx; my = hy; mz = hz;
+}
+
+// fused middle stage on the tile: radix 2^LR, stride 1
+template <typename T, int LR>
+__device__ __forceinline__ void k3_fused(const Geo& g, typename cx_of<T>::type* s, int TY, int kx, int ky0,
+                                         const T* __restrict__ K, size_t kcs, int tid, int nthr)
+{
+    using C = typename cx_of<T>::type;
+    constexpr int R = 1 << LR;
+    const int B = 3 * TY;
+    const int ty = tid % TY, i0 = tid / TY, istep = nthr / TY;
+    const int nbf = g.Nz >> LR;
+    for (int i = i0; i < nbf; i += istep) {
+        const int p0 = i << LR;
+        C a[3][R];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+#pragma unroll
+            for (int m = 0; m < R; ++m) a[c][m] = s[(p0 + m) * B + c * TY + ty];
+            dftR<LR, false, false>(a[c]);
+        }
+        const int kb = freq_of_pos(p0, g.lNz);
+#pragma unroll
+        for (int m = 0; m < R; ++m) {
+            const KernelVals<T> kv = load_kernel<T>(g, K, kcs, kx, ky0 + ty, kb + m * (g.Nz >> LR));
+            apply_kernel(kv, a[0][m], a[1][m], a[2][m]);
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            dftR<LR, true, false>(a[c]);
+#pragma unroll
+            for (int m = 0; m < R; ++m) s[(p0 + m) * B + c * TY + ty] = a[c][m];
+        }
+    }
+}
+
+// whole z transform in one radix-2^LR butterfly per (ky, component): Nz <= 8, no shared memory
+template <typename T, int LR>
+__device__ __forceinline__ void k3_single(const Geo& g, typename cx_of<T>::type* base, size_t cstride, int kx, int ky,
+                                          const T* __restrict__ K, size_t kcs)
+{
+    using C = typename cx_of<T>::type;
+    constexpr int R = 1 << LR;
+    C a[3][R];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) a[c][r] = (r < g.nz) ? base[c * cstride + (size_t)r * g.Ny] : cmake<C>((T)0, (T)0);
+        dftR<LR, false, false>(a[c]);
+    }
+#pragma unroll
+    for (int m = 0; m < R; ++m) {
+        const KernelVals<T> kv = load_kernel<T>(g, K, kcs, kx, ky, m);
+        apply_kernel(kv, a[0][m], a[1][m], a[2][m]);
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        dftR<LR, true, false>(a[c]);
+#pragma unroll
+        for (int r = 0; r < R; ++r) if (r < g.nz) base[c * cstride + (size_t)r * g.Ny] = a[c][r];
+    }
+}
+
+// Nz <= 8: one thread per ky column, no shared memory.  grid = nkx * Ny / TY, block >= TY.
+template <typename T>
+__global__ void __launch_bounds__(128) k_z_small(Geo g, int TY, int kx0, int nkx,
+                                                 typename cx_of<T>::type* __restrict__ W2,
+                                                 const T* __restrict__ K, size_t kcs)
+{
+    using C = typename cx_of<T>::type;
+    const int tid = threadIdx.x;
+    const int tilesY = g.Ny / TY;
+    const int kyt = blockIdx.x % tilesY, kxl = blockIdx.x / tilesY;
+    const int ky0 = kyt * TY;
+    const int kx = kx0 + kxl;
+    const size_t cstride = (size_t)nkx * g.nz * g.Ny;
+    if (tid >= TY) return;
+    C* col = W2 + ((size_t)kxl * g.nz) * g.Ny + ky0 + tid;
+    const int lNz = g.lNz;
+    if (lNz == 0) k3_single<T, 0>(g, col, cstride, kx, ky0 + tid, K, kcs);
+    else if (lNz == 1) k3_single<T, 1>(g, col, cstride, kx, ky0 + tid, K, kcs);
+    else if (lNz == 2) k3_single<T, 2>(g, col, cstride, kx, ky0 + tid, K, kcs);
+    else k3_single<T, 3>(g, col, cstride, kx, ky0 + tid, K, kcs);
+}
+
+// Nz >= 16.  LRF = log2 radix of the fused middle stage = the last pass of the schedule (Nz % 8 -> 1, 2; else 3).
+template <typename T, int LRF>
+__global__ void __launch_bounds__(512, ((LRF == 3 || sizeof(T) == 8) ? 1 : 2)) k_z_mul(Geo g, int TY, int kx0, int nkx,
                                                typename cx_of<T>::type* __restrict__ W2,
-                                               const T* __restrict__ K, size_t kcomp_stride,
+                                               const T* __restrict__ K, size_t kcs,
                                                const typename cx_of<T>::type* __restrict__ twz)
 {
     using C = typename cx_of<T>::type;
-    constexpr int RB = cx_of<T>::ROWBITS;
     C* s = reinterpret_cast<C*>(demag_smem);
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int tilesY = g.Ny / TY;
     const int kyt = blockIdx.x % tilesY, kxl = blockIdx.x / tilesY;
     const int ky0 = kyt * TY;
-    const int B = 3 * TY;
-    const int lTY = 31 - __clz(TY);
+    const int kx = kx0 + kxl;
     const size_t cstride = (size_t)nkx * g.nz * g.Ny;                 // component stride in the slab
     C* base = W2 + ((size_t)kxl * g.nz) * g.Ny + ky0;
-    for (int idx = tid; idx < 3 * g.Nz * TY; idx += nthr) {
-        const int ty = idx & (TY - 1), r = idx >> lTY;
-        const int z = r & (g.Nz - 1), c = r >> g.lNz;
-        C v = cmake<C>((T)0, (T)0);
-        if (z < g.nz) v = base[c * cstride + (size_t)z * g.Ny + ty];
-        s[swz<RB>(z * B + c * TY + ty)] = v;
+    const int lNz = g.lNz;
+    const int B = 3 * TY;
+    const int n8 = lNz / 3, rem = lNz % 3;
+    const int npass = n8 + (rem ? 1 : 0);
+    const int b = tid % B, i0 = tid / B, istep = nthr / B;       // nthr is a multiple of B (plan)
+    const int c = b / TY, ty = b - c * TY;
+    C* gcol = base + c * cstride + ty;
+    const bool padded = g.Nz != g.nz;
+    const int ls0 = lNz - 3, S0 = 1 << ls0;
+    // ---- first forward pass (radix 8, stride Nz/8) straight from global
+    for (int i = i0; i < S0; i += istep) {
+        C a[8];
+        if (padded) {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) a[r] = gcol[(size_t)(i + r * S0) * g.Ny];
+            dft8<false, true>(a);
+        } else {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) a[r] = gcol[(size_t)(i + r * S0) * g.Ny];
+            dft8<false, false>(a);
+        }
+        twiddle<3, false>(a, twz, i);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) s[(i + r * S0) * B + b] = a[r];
     }
     __syncthreads();
-    fft_tile<T, false>(s, g.lNz, B, twz, 0, tid, nthr);
-    const int kx = kx0 + kxl;
-    for (int idx = tid; idx < g.Nz * TY; idx += nthr) {
-        const int ty = idx & (TY - 1), p = idx >> lTY;
-        const int kz = freq_of_pos(p, g.lNz);
-        const int ky = ky0 + ty;
-        const bool my = (2 * ky > g.Ny), mz = (2 * kz > g.Nz);
-        const int kyp = my ? g.Ny - ky : ky, kzp = mz ? g.Nz - kz : kz;
-        const T sy = my ? (T)-1 : (T)1, sz = mz ? (T)-1 : (T)1;
-        const size_t ko = ((size_t)kx * g.kpz + kzp) * g.kpitch + kyp;
-        const T kxx = __ldg(K + ko), kyy = __ldg(K + kcomp_stride + ko), kzz = __ldg(K + 2 * kcomp_stride + ko);
-        const T kxy = sy * __ldg(K + 3 * kcomp_stride + ko);
-        const T kxz = sz * __ldg(K + 4 * kcomp_stride + ko);
-        const T kyz = sy * sz * __ldg(K + 5 * kcomp_stride + ko);
-        const int a0 = swz<RB>(p * B + ty), a1 = swz<RB>(p * B + TY + ty), a2 = swz<RB>(p * B + 2 * TY + ty);
-        const C mx = s[a0], my_ = s[a1], mz_ = s[a2];
-        s[a0] = cmake<C>(kxx * mx.x + kxy * my_.x + kxz * mz_.x, kxx * mx.y + kxy * my_.y + kxz * mz_.y);
-        s[a1] = cmake<C>(kxy * mx.x + kyy * my_.x + kyz * mz_.x, kxy * mx.y + kyy * my_.y + kyz * mz_.y);
-        s[a2] = cmake<C>(kxz * mx.x + kyz * my_.x + kzz * mz_.x, kxz * mx.y + kyz * my_.y + kzz * mz_.y);
-    }
+    // ---- middle forward passes (all radix 8); the last pass of the schedule is the fused stage
+    for (int k = 1; k <= npass - 2; ++k) { fft_pass<T, 3, false, false>(s, lNz, lNz - 3 * (k + 1), B, B, twz, 0, tid, nthr); __syncthreads(); }
+    k3_fused<T, LRF>(g, s, TY, kx, ky0, K, kcs, tid, nthr);
     __syncthreads();
-    fft_tile<T, true>(s, g.lNz, B, twz, 0, tid, nthr);
-    const int lnz = 31 - __clz(g.nz);
-    for (int idx = tid; idx < ((3 * TY) << lnz); idx += nthr) {
-        const int ty = idx & (TY - 1), r = idx >> lTY;
-        const int z = r & (g.nz - 1), c = r >> lnz;
-        base[c * cstride + (size_t)z * g.Ny + ty] = s[swz<RB>(z * B + c * TY + ty)];
+    for (int k = npass - 2; k >= 1; --k) { fft_pass<T, 3, true, false>(s, lNz, lNz - 3 * (k + 1), B, B, twz, 0, tid, nthr); __syncthreads(); }
+    // ---- last inverse pass (radix 8, stride Nz/8) straight to global, keeping z < nz (the crop)
+    for (int i = i0; i < S0; i += istep) {
+        C a[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) a[r] = s[(i + r * S0) * B + b];
+        twiddle<3, true>(a, twz, i);
+        dft8<true, false>(a);
+        const int nout = padded ? 4 : 8;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) if (r < nout) gcol[(size_t)(i + r * S0) * g.Ny] = a[r];
     }
 }
 
@@ -327,3 +450,5 @@ __global__ void __launch_bounds__(256) k_macro_scatter(int nx, int ny, int nz, i
 }
 
 }  // namespace demag
+
+#include "kernels_fast.cuh"

@@ -37,7 +37,7 @@ demag_status fail(demag_status st, const char* fmt, ...)
                         "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);   \
     } while (0)
 
-constexpr int kMaxSmem = 232448;          // 227 KB opt-in dynamic shared memory per CTA (sm_100)
+constexpr int kMaxSmem = 232448 - 1024;   // 227 KB opt-in shared memory per CTA (sm_100) minus room for static __shared__
 constexpr size_t kSlabBytes = 40u << 20;  // target size of the L2-resident W2 slab (L2 is ~126 MB)
 
 inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
@@ -61,10 +61,11 @@ struct demag_plan_s {
     void* Mc = nullptr; void* Hc = nullptr; size_t macro_bytes = 0;   // atomistic macrocell buffers
     bool has_kernel = false;
     // launch configuration
-    int R1, thr1, smem1;          // K1 / K5
-    int B2, thr2, smem2;          // K2 / K4
+    int R1, thr1, smem1, pitch1;  // K1 / K5   (pitch odd -> conflict-free transposing loads; B == 1 -> swizzle)
+    int B2, thr2, smem2, pitch2;  // K2 / K4
     int TY, thr3, smem3;          // K3
     int nkx_slab, nkx_auto;
+    bool fast1 = false, fast2 = false;   // kernels_fast.cuh variants of the x / y stages
 };
 
 namespace {
@@ -81,11 +82,21 @@ int pick_threads(long long elems)
 template <typename T>
 demag_status set_func_attrs()
 {
-    CUDA_TRY(cudaFuncSetAttribute(k_x_r2c<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
-    CUDA_TRY(cudaFuncSetAttribute(k_x_c2r<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
-    CUDA_TRY(cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
-    CUDA_TRY(cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
-    CUDA_TRY(cudaFuncSetAttribute(k_z_mul<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_x_r2c<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_x_c2r<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_fwd<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_inv<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_x_r2c<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_x_c2r<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_fwd<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_inv<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_x_r2c_f<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_x_c2r_f<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_fwd_f<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_y_inv_f<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_z_mul<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_z_mul<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+    CUDA_TRY(cudaFuncSetAttribute(k_z_mul<T, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
     return DEMAG_OK;
 }
 
@@ -112,39 +123,49 @@ void configure(demag_plan_s* p)
 {
     const Geo& g = p->g;
     const size_t csz = 2 * p->esz;
-    // K1 / K5: R rows of Lc complex.  R >= 4 keeps the transposed stores at >= 32 B (fp32) runs.
+    // K1 / K5: R rows of Lc complex, tile s[Lc][pitch].  R >= 4 keeps the transposed stores at >= 32 B runs.
     {
         const long long Lc = 1LL << g.lLc;
         int R = pow2_floor(std::max<long long>(1, (48 << 10) / (long long)(Lc * csz)));
         if (R < 4) R = 4;
         if (R > 16) R = 16;
-        while (R > 1 && (long long)R * Lc * csz > 200 << 10) R /= 2;
+        while (R > 1 && (long long)(R | 1) * Lc * csz > 200 << 10) R /= 2;
         if (R > g.ny) R = g.ny;
         p->R1 = R;
-        const long long elems = (long long)R * Lc;
+        p->pitch1 = R == 1 ? 1 : (R | 1);
+        p->fast1 = g.lLc >= 3 && R >= 2;
+        const long long elems = (long long)p->pitch1 * Lc;
         p->smem1 = (int)(((elems + 15) / 16 * 16) * csz);
-        p->thr1 = pick_threads(elems);
+        p->thr1 = pick_threads((long long)R * Lc);
     }
-    // K2 / K4: B lines of Ny complex, about 32 KB per tile
+    // K2 / K4: B lines of Ny complex, tile s[Ny][pitch]: the largest B in {16,8,4,2} whose tile is <= 100 KB
     {
-        int B = (int)std::max<long long>(1, (32 << 10) / (long long)(g.Ny * csz));
-        if (B > 16) B = 16;
+        int B = 16;
+        while (B > 1 && (long long)(B | 1) * g.Ny * csz > 100 << 10) B /= 2;
         const long long nlines_min = 3LL * g.nz;
-        if (B > nlines_min) B = (int)nlines_min;
+        while (B > nlines_min) B /= 2;
+        if (B < 1) B = 1;
         p->B2 = B;
-        const long long elems = (long long)B * g.Ny;
+        p->pitch2 = B == 1 ? 1 : (B | 1);
+        p->fast2 = g.lNy >= 3 && B >= 2;
+        const long long elems = (long long)p->pitch2 * g.Ny;
         p->smem2 = (int)(((elems + 15) / 16 * 16) * csz);
-        p->thr2 = pick_threads(elems);
+        p->thr2 = pick_threads((long long)B * g.Ny);
     }
-    // K3: TY ky columns x Nz x 3 components
-    {
+    // K3: TY ky columns x Nz x 3 components, tile s[Nz][3*TY]; block = a multiple of 3*TY threads
+    if (g.lNz <= 3) {                       // whole z transform in one butterfly per thread, no shared memory
+        int TY = std::min(g.Ny, 128);
+        p->TY = TY; p->smem3 = 0; p->thr3 = std::max(32, TY);
+    } else {
         int TY = 16;
         while (TY > 1 && (long long)TY * 3 * g.Nz * csz > 100 << 10) TY /= 2;
         if (TY > g.Ny) TY = g.Ny;
         p->TY = TY;
-        const long long elems = 3LL * TY * g.Nz;
-        p->smem3 = (int)(((elems + 15) / 16 * 16) * csz);
-        p->thr3 = pick_threads(elems);
+        const int B = 3 * TY;
+        p->smem3 = (int)((long long)B * g.Nz * csz);
+        const int S0 = g.Nz / 8;
+        const int gc = pow2_floor(std::max(1, std::min(S0, 512 / B)));
+        p->thr3 = B * gc;
     }
     // slab of kx planes whose W2 part stays L2-resident between K2, K3 and K4
     {
@@ -189,7 +210,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
     g.lLc = g.Nx >= 2 ? ilog2(g.Nx / 2) : 0;
     g.lNy = ilog2(g.Ny); g.lNz = ilog2(g.Nz);
     g.kpy = g.Ny / 2 + 1; g.kpz = g.Nz / 2 + 1;
-    g.kpitch = (g.kpy + 7) / 8 * 8;
+    g.kpitch = g.Ny;                          // kernel rows: y unpacked, position order
     p->h[0] = hx; p->h[1] = hy; p->h[2] = hz;
     p->pbc = pbc_flags; p->prec = precision;
     p->esz = precision == DEMAG_FP32 ? 4 : 8;
@@ -296,11 +317,11 @@ demag_status launch_sym_axis(const double* in, double* out, int n, int N, int pa
 }
 
 template <typename T>
-void launch_pack(const double* A, void* K, const Geo& g, double scale)
+void launch_pack(const double* A, void* K, const Geo& g, int par_y, double scale)
 {
-    const size_t n = (size_t)g.hx * g.kpz * g.kpy;
+    const size_t n = (size_t)g.hx * g.kpz * g.Ny;
     const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
-    k_pack_kernel<T><<<grid, 256>>>(A, (T*)K, g.hx, g.kpy, g.kpz, g.kpitch, scale);
+    k_pack_kernel<T><<<grid, 256>>>(A, (T*)K, g.hx, g.kpy, g.kpz, g.Ny, g.lNy, par_y, scale);
 }
 
 }  // namespace
@@ -344,8 +365,8 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
             // each odd axis contributes a factor i (X = i Im X): two odd axes -> -1.  Eq. (1)'s minus sign and
             // the inverse-transform normalisation 1/(Nx Ny Nz) are folded in here (R3).
             const double scale = (nodd == 2 ? -1.0 : 1.0) * (-1.0) / ((double)g.Nx * g.Ny * g.Nz);
-            if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, scale);
-            else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, scale);
+            if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
+            else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
             CUDA_TRY(cudaGetLastError());
         }
         CUDA_TRY(cudaDeviceSynchronize());
@@ -398,21 +419,33 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
         const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
         STAGE(0, (k_x_copy_fwd<T><<<grid, 256, 0, st>>>(3 * nc, M, W1)));
     } else {
-        STAGE(0, (k_x_r2c<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, M, W1, twx)));
+        if (p->fast1) STAGE(0, (k_x_r2c_f<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, M, W1, twx)));
+        else if (p->pitch1 == 1) STAGE(0, (k_x_r2c<T, true><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, M, W1, twx)));
+        else STAGE(0, (k_x_r2c<T, false><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, M, W1, twx)));
     }
     for (int kx0 = 0; kx0 < g.hx; kx0 += p->nkx_slab) {
         const int nkx = std::min(p->nkx_slab, g.hx - kx0);
         const unsigned g2 = (unsigned)((3LL * nkx * g.nz + p->B2 - 1) / p->B2);
-        STAGE(1, (k_y_fwd<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W1, W2, twy)));
-        STAGE(2, (k_z_mul<T><<<(unsigned)(nkx * (g.Ny / p->TY)), p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, (const T*)p->K,
-                                                                                         p->kcomp_stride, twz)));
-        STAGE(3, (k_y_inv<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, kx0, nkx, W2, W1, twy)));
+        if (p->fast2) STAGE(1, (k_y_fwd_f<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, p->pitch2, kx0, nkx, W1, W2, twy)));
+        else if (p->pitch2 == 1) STAGE(1, (k_y_fwd<T, true><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, p->pitch2, kx0, nkx, W1, W2, twy)));
+        else STAGE(1, (k_y_fwd<T, false><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, p->pitch2, kx0, nkx, W1, W2, twy)));
+        const unsigned g3 = (unsigned)(nkx * (g.Ny / p->TY));
+        const T* Kp = (const T*)p->K;
+        if (g.lNz <= 3) STAGE(2, (k_z_small<T><<<g3, p->thr3, 0, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride)));
+        else if (g.lNz % 3 == 1) STAGE(2, (k_z_mul<T, 1><<<g3, p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride, twz)));
+        else if (g.lNz % 3 == 2) STAGE(2, (k_z_mul<T, 2><<<g3, p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride, twz)));
+        else STAGE(2, (k_z_mul<T, 3><<<g3, p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride, twz)));
+        if (p->fast2) STAGE(3, (k_y_inv_f<T><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, p->pitch2, kx0, nkx, W2, W1, twy)));
+        else if (p->pitch2 == 1) STAGE(3, (k_y_inv<T, true><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, p->pitch2, kx0, nkx, W2, W1, twy)));
+        else STAGE(3, (k_y_inv<T, false><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, p->pitch2, kx0, nkx, W2, W1, twy)));
     }
     if (g.Nx == 1) {
         const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
         STAGE(4, (k_x_copy_inv<T><<<grid, 256, 0, st>>>(3 * nc, W1, H)));
     } else {
-        STAGE(4, (k_x_c2r<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, W1, H, twx)));
+        if (p->fast1) STAGE(4, (k_x_c2r_f<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, W1, H, twx)));
+        else if (p->pitch1 == 1) STAGE(4, (k_x_c2r<T, true><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, W1, H, twx)));
+        else STAGE(4, (k_x_c2r<T, false><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, W1, H, twx)));
     }
     CUDA_TRY(cudaGetLastError());
     return DEMAG_OK;
