@@ -170,19 +170,27 @@ template <int LR, bool INV, bool HALF_IN, typename C> __device__ __forceinline__
     if (LR == 3) dft8<INV, HALF_IN>(a); else if (LR == 2) dft4<INV, HALF_IN>(a); else if (LR == 1) dft2<INV, HALF_IN>(a);
 }
 
-// a[m] *= w^m (forward) or conj(w)^m (inverse), m = 1..R-1, w^m read / derived from the table at j*m
-template <int LR, bool INV, typename C>
+// a[m] *= w^m (forward) or conj(w)^m (inverse), m = 1..R-1, w^m read / derived from the table at j*m.
+// UNI: the index j is the same for (nearly) all lanes of a warp (lines-fastest thread mapping), so every power is
+// read directly (broadcast loads, one sector each); otherwise w, w^2, w^4 are read and the rest derived.
+template <int LR, bool INV, bool UNI, typename C>
 __device__ __forceinline__ void twiddle(C* a, const C* __restrict__ tw, int j)
 {
     if (LR == 3) {
-        const C w1 = __ldg(tw + j), w2 = __ldg(tw + 2 * j), w4 = __ldg(tw + 4 * j);
-        const C w3 = cmul(w1, w2), w5 = cmul(w1, w4), w6 = cmul(w2, w4), w7 = cmul(w3, w4);
+        C w1, w2, w3, w4, w5, w6, w7;
+        if (UNI) {
+            w1 = __ldg(tw + j); w2 = __ldg(tw + 2 * j); w3 = __ldg(tw + 3 * j); w4 = __ldg(tw + 4 * j);
+            w5 = __ldg(tw + 5 * j); w6 = __ldg(tw + 6 * j); w7 = __ldg(tw + 7 * j);
+        } else {
+            w1 = __ldg(tw + j); w2 = __ldg(tw + 2 * j); w4 = __ldg(tw + 4 * j);
+            w3 = cmul(w1, w2); w5 = cmul(w1, w4); w6 = cmul(w2, w4); w7 = cmul(w3, w4);
+        }
         if (!INV) { a[1] = cmul(a[1], w1); a[2] = cmul(a[2], w2); a[3] = cmul(a[3], w3); a[4] = cmul(a[4], w4);
                     a[5] = cmul(a[5], w5); a[6] = cmul(a[6], w6); a[7] = cmul(a[7], w7); }
         else      { a[1] = cmulc(a[1], w1); a[2] = cmulc(a[2], w2); a[3] = cmulc(a[3], w3); a[4] = cmulc(a[4], w4);
                     a[5] = cmulc(a[5], w5); a[6] = cmulc(a[6], w6); a[7] = cmulc(a[7], w7); }
     } else if (LR == 2) {
-        const C w1 = __ldg(tw + j), w2 = __ldg(tw + 2 * j); const C w3 = cmul(w1, w2);
+        const C w1 = __ldg(tw + j), w2 = __ldg(tw + 2 * j); const C w3 = UNI ? __ldg(tw + 3 * j) : cmul(w1, w2);
         if (!INV) { a[1] = cmul(a[1], w1); a[2] = cmul(a[2], w2); a[3] = cmul(a[3], w3); }
         else      { a[1] = cmulc(a[1], w1); a[2] = cmulc(a[2], w2); a[3] = cmulc(a[3], w3); }
     } else if (LR == 1) {
@@ -218,9 +226,9 @@ __device__ __forceinline__ void fft_pass(typename cx_of<T>::type* s, int log2L, 
         for (int r = 0; r < R; ++r) a[r] = s[taddr<SWZ, RB>(q0 + r * stride)];
         if (!INV) {
             dftR<LR, false, false>(a);
-            if (ls > 0) twiddle<LR, false>(a, tw, lo << ltw);
+            if (ls > 0) twiddle<LR, false, !SWZ>(a, tw, lo << ltw);
         } else {
-            if (ls > 0) twiddle<LR, true>(a, tw, lo << ltw);
+            if (ls > 0) twiddle<LR, true, !SWZ>(a, tw, lo << ltw);
             dftR<LR, true, false>(a);
         }
 #pragma unroll

@@ -349,7 +349,7 @@ __global__ void __launch_bounds__(512, ((LRF == 3 || sizeof(T) == 8) ? 1 : 2)) k
             for (int r = 0; r < 8; ++r) a[r] = gcol[(size_t)(i + r * S0) * g.Ny];
             dft8<false, false>(a);
         }
-        twiddle<3, false>(a, twz, i);
+        twiddle<3, false, true>(a, twz, i);
 #pragma unroll
         for (int r = 0; r < 8; ++r) s[(i + r * S0) * B + b] = a[r];
     }
@@ -364,7 +364,7 @@ __global__ void __launch_bounds__(512, ((LRF == 3 || sizeof(T) == 8) ? 1 : 2)) k
         C a[8];
 #pragma unroll
         for (int r = 0; r < 8; ++r) a[r] = s[(i + r * S0) * B + b];
-        twiddle<3, true>(a, twz, i);
+        twiddle<3, true, true>(a, twz, i);
         dft8<true, false>(a);
         const int nout = padded ? 4 : 8;
 #pragma unroll

@@ -27,7 +27,7 @@ __device__ __forceinline__ void pass_first_fwd(typename cx_of<T>::type* s, int l
 #pragma unroll
         for (int r = 0; r < (HALF ? 4 : 8); ++r) a[r] = ld(b, i + r * S0);
         dft8<false, HALF>(a);
-        twiddle<3, false>(a, tw, i << lt);
+        twiddle<3, false, false>(a, tw, i << lt);
         C* d = s + i * pitch + b;
         const int st = S0 * pitch;
 #pragma unroll
@@ -50,7 +50,7 @@ __device__ __forceinline__ void pass_last_inv(typename cx_of<T>::type* s, int lL
         const int st = S0 * pitch;
 #pragma unroll
         for (int r = 0; r < 8; ++r) a[r] = d[r * st];
-        twiddle<3, true>(a, tw, i << lt);
+        twiddle<3, true, false>(a, tw, i << lt);
         dft8<true, false>(a);
 #pragma unroll
         for (int r = 0; r < 8; ++r) if (r < 4 || !half_out) stf(b, i + r * S0, a[r]);

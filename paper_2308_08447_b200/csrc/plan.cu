@@ -13,6 +13,7 @@
 #include "../../include/demag.h"
 #include "builder.cuh"
 #include "kernels.cuh"
+#include "kernels_z.cuh"
 
 using namespace demag;
 
@@ -38,7 +39,7 @@ demag_status fail(demag_status st, const char* fmt, ...)
     } while (0)
 
 constexpr int kMaxSmem = 232448 - 1024;   // 227 KB opt-in shared memory per CTA (sm_100) minus room for static __shared__
-constexpr size_t kSlabBytes = 40u << 20;  // target size of the L2-resident W2 slab (L2 is ~126 MB)
+constexpr size_t kSlabBytes = 128u << 20;  // target size of the L2-resident W2 slab (L2 is ~126 MB)
 
 inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 inline int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
@@ -66,6 +67,7 @@ struct demag_plan_s {
     int TY, thr3, smem3;          // K3
     int nkx_slab, nkx_auto;
     bool fast1 = false, fast2 = false;   // kernels_fast.cuh variants of the x / y stages
+    bool z_spec = false;                 // kernels_z.cuh compile-time specialised z stage
 };
 
 namespace {
@@ -119,6 +121,37 @@ demag_status make_twiddles(int N, void** out, size_t* bytes)
     return DEMAG_OK;
 }
 
+// Compile-time specialised z stage (kernels_z.cuh) for (log2 Nz, TY) in {(4..8, 16), (9, 8)}.
+// mode 0: set the shared-memory attribute (plan time); mode 1: launch.  Returns false if no specialisation matches.
+template <typename T, int LNZ, int TY, int NT>
+bool z_c_do(int mode, const Geo& g, unsigned grid, cudaStream_t st, int kx0, int nkx, typename cx_of<T>::type* W2,
+            const T* K, size_t kcs, const typename cx_of<T>::type* twz, cudaError_t* err)
+{
+    constexpr int smem = (1 << LNZ) * 3 * TY * (int)sizeof(typename cx_of<T>::type);
+    if (mode == 0) *err = cudaFuncSetAttribute(k_z_mul_c<T, LNZ, TY, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    else k_z_mul_c<T, LNZ, TY, NT><<<grid, NT, smem, st>>>(g, kx0, nkx, W2, K, kcs, twz);
+    return true;
+}
+template <typename T>
+bool z_c_dispatch(int mode, const Geo& g, int TY, unsigned grid, cudaStream_t st, int kx0, int nkx,
+                  typename cx_of<T>::type* W2, const T* K, size_t kcs, const typename cx_of<T>::type* twz, cudaError_t* err)
+{
+    if (TY == 16) {
+        switch (g.lNz) {
+        case 4: return z_c_do<T, 4, 16, 96>(mode, g, grid, st, kx0, nkx, W2, K, kcs, twz, err);
+        case 5: return z_c_do<T, 5, 16, 192>(mode, g, grid, st, kx0, nkx, W2, K, kcs, twz, err);
+        case 6: return z_c_do<T, 6, 16, 384>(mode, g, grid, st, kx0, nkx, W2, K, kcs, twz, err);
+        case 7: return z_c_do<T, 7, 16, 384>(mode, g, grid, st, kx0, nkx, W2, K, kcs, twz, err);
+        case 8: if (sizeof(T) == 4) return z_c_do<T, 8, 16, 384>(mode, g, grid, st, kx0, nkx, W2, K, kcs, twz, err); break;
+        default: break;
+        }
+    } else if (TY == 8) {
+        if (g.lNz == 9 && sizeof(T) == 4) return z_c_do<T, 9, 8, 384>(mode, g, grid, st, kx0, nkx, W2, K, kcs, twz, err);
+        if (g.lNz == 8 && sizeof(T) == 8) return z_c_do<T, 8, 8, 384>(mode, g, grid, st, kx0, nkx, W2, K, kcs, twz, err);
+    }
+    return false;
+}
+
 void configure(demag_plan_s* p)
 {
     const Geo& g = p->g;
@@ -141,7 +174,9 @@ void configure(demag_plan_s* p)
     // K2 / K4: B lines of Ny complex, tile s[Ny][pitch]: the largest B in {16,8,4,2} whose tile is <= 100 KB
     {
         int B = 16;
-        while (B > 1 && (long long)(B | 1) * g.Ny * csz > 100 << 10) B /= 2;
+        long long lim = 100 << 10;
+        if (const char* e = getenv("DEMAG_B2_KB")) lim = (long long)atoi(e) << 10;      // tuning override
+        while (B > 1 && (long long)(B | 1) * g.Ny * csz > lim) B /= 2;
         const long long nlines_min = 3LL * g.nz;
         while (B > nlines_min) B /= 2;
         if (B < 1) B = 1;
@@ -158,6 +193,7 @@ void configure(demag_plan_s* p)
         p->TY = TY; p->smem3 = 0; p->thr3 = std::max(32, TY);
     } else {
         int TY = 16;
+        if (const char* e = getenv("DEMAG_TY")) TY = atoi(e);       // tuning override (experiments only)
         while (TY > 1 && (long long)TY * 3 * g.Nz * csz > 100 << 10) TY /= 2;
         if (TY > g.Ny) TY = g.Ny;
         p->TY = TY;
@@ -170,7 +206,9 @@ void configure(demag_plan_s* p)
     // slab of kx planes whose W2 part stays L2-resident between K2, K3 and K4
     {
         const size_t per_kx = (size_t)3 * g.nz * g.Ny * csz;
-        long long n = (long long)(kSlabBytes / per_kx);
+        size_t slab_bytes = kSlabBytes;
+        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoi(e) << 20;   // tuning override
+        long long n = (long long)(slab_bytes / per_kx);
         if (n < 1) n = 1;
         if (n > g.hx) n = g.hx;
         p->nkx_auto = (int)n;
@@ -228,6 +266,14 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         if (precision == DEMAG_FP32) { demag_status s = set_func_attrs<float>(); if (s) return s; }
         else { demag_status s = set_func_attrs<double>(); if (s) return s; }
         CUDA_TRY(cudaFuncSetAttribute(k_sym_axis, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+        {
+            cudaError_t zerr = cudaSuccess;
+            if (getenv("DEMAG_NO_ZSPEC")) p->z_spec = false; else
+            p->z_spec = precision == DEMAG_FP32
+                ? z_c_dispatch<float>(0, g, p->TY, 0, nullptr, 0, 0, nullptr, nullptr, 0, nullptr, &zerr)
+                : z_c_dispatch<double>(0, g, p->TY, 0, nullptr, 0, 0, nullptr, nullptr, 0, nullptr, &zerr);
+            CUDA_TRY(zerr);
+        }
         CUDA_TRY(cudaMalloc(&p->W1, p->w1_bytes));
         CUDA_TRY(cudaMalloc(&p->W2, p->w2_bytes));
         CUDA_TRY(cudaMalloc(&p->K, p->k_bytes));
@@ -431,7 +477,9 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
         else STAGE(1, (k_y_fwd<T, false><<<g2, p->thr2, p->smem2, st>>>(g, p->B2, p->pitch2, kx0, nkx, W1, W2, twy)));
         const unsigned g3 = (unsigned)(nkx * (g.Ny / p->TY));
         const T* Kp = (const T*)p->K;
-        if (g.lNz <= 3) STAGE(2, (k_z_small<T><<<g3, p->thr3, 0, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride)));
+        cudaError_t zerr = cudaSuccess;
+        if (p->z_spec) STAGE(2, (z_c_dispatch<T>(1, g, p->TY, g3, st, kx0, nkx, W2, Kp, p->kcomp_stride, twz, &zerr)));
+        else if (g.lNz <= 3) STAGE(2, (k_z_small<T><<<g3, p->thr3, 0, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride)));
         else if (g.lNz % 3 == 1) STAGE(2, (k_z_mul<T, 1><<<g3, p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride, twz)));
         else if (g.lNz % 3 == 2) STAGE(2, (k_z_mul<T, 2><<<g3, p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride, twz)));
         else STAGE(2, (k_z_mul<T, 3><<<g3, p->thr3, p->smem3, st>>>(g, p->TY, kx0, nkx, W2, Kp, p->kcomp_stride, twz)));
