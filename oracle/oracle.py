@@ -198,7 +198,14 @@ def fft_conv(T, M, P=None) -> np.ndarray:
     nz, ny, nx = M.shape[1:]
     Px, Py, Pz = P if P is not None else padded_shape((nx, ny, nz))
     s = (Pz, Py, Px)
-    Mh = [np.fft.rfftn(M[b], s=s, axes=(0, 1, 2)) for b in range(3)]
+    try:                                   # same routine family (pocketfft), threaded
+        import scipy.fft as _fft
+        rfftn = lambda x: _fft.rfftn(x, s=s, axes=(0, 1, 2), workers=-1)
+        irfftn = lambda x: _fft.irfftn(x, s=s, axes=(0, 1, 2), workers=-1)
+    except ImportError:
+        rfftn = lambda x: np.fft.rfftn(x, s=s, axes=(0, 1, 2))
+        irfftn = lambda x: np.fft.irfftn(x, s=s, axes=(0, 1, 2))
+    Mh = [rfftn(M[b]) for b in range(3)]
     H = np.empty_like(M)
     Kh = {}
     for a in range(3):
@@ -206,9 +213,9 @@ def fft_conv(T, M, P=None) -> np.ndarray:
         for b in range(3):
             c = int(COMP[a, b])
             if c not in Kh:
-                Kh[c] = np.fft.rfftn(_padded_one(T[c], c, (Px, Py, Pz)), s=s, axes=(0, 1, 2))
+                Kh[c] = rfftn(_padded_one(T[c], c, (Px, Py, Pz)))
             acc = acc + Kh[c] * Mh[b]
-        H[a] = -np.fft.irfftn(acc, s=s, axes=(0, 1, 2))[:nz, :ny, :nx]
+        H[a] = -irfftn(acc)[:nz, :ny, :nx]
     return H
 
 

@@ -1,0 +1,132 @@
+"""Parity at BASELINE.json's full sizes (configs 2-5), in the launch configuration bench.py times.
+
+The oracle cannot afford n_c^2 pairs here, so it evaluates Eq. (1) by direct fp64 summation at seeded
+sample cells (O-S: corners, face/edge centres, body centre, random cells), each computed one by one; for
+configs 2 and 3 the whole field is also compared with the library-FFT cross-check O-C.  The oracle's N is
+pushed through demag_set_kernel (R5 "convolution parity"): 2e-5 (fp32) / 1e-11 (fp64) of Ms.
+"""
+import numpy as np
+import pytest
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+TOL32, TOL64 = 2e-5, 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2308_08447_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _need_host_gb(gb):
+    import psutil
+    if psutil.virtual_memory().available < gb * 2 ** 30:
+        pytest.skip(f"needs ~{gb} GB of host memory for the oracle")
+
+
+def _sampled_check(torch, B, oracle, cfg, M, precs, nsamp, full_field):
+    from paper_2308_08447_b200 import workloads as W
+    T = oracle.tensor_table(cfg.n, cfg.h)
+    cells = W.sample_cells(cfg.n, nsamp, cfg.seed)
+    M64 = M.astype(np.float64)
+    Hs = oracle.direct_sum_sampled(T, M64, cells)                 # [nsamp][3], Eq. (1) one cell at a time
+    Hfull = oracle.fft_conv(T, M64) if full_field else None
+    if Hfull is not None:                                         # the cross-check agrees with Eq. (1) where sampled
+        assert np.abs(Hfull.reshape(3, -1)[:, cells].T - Hs).max() / cfg.Ms < 1e-12
+    out = {}
+    for prec in precs:
+        dt = torch.float32 if prec == 0 else torch.float64
+        tol = TOL32 if prec == 0 else TOL64
+        with B.Plan(cfg.n, cfg.h, 0, prec) as p:
+            p.set_kernel(T)
+            Md = torch.from_numpy(M).to("cuda", dt)
+            Hd = torch.full_like(Md, float("nan"))
+            p.apply(Md, Hd)
+            torch.cuda.synchronize()
+            assert not torch.isnan(Hd).any()
+            got = Hd.reshape(3, -1)[:, torch.from_numpy(cells).cuda()].T.cpu().numpy().astype(np.float64)
+            err = np.abs(got - Hs).max() / cfg.Ms
+            assert err <= tol, (cfg.name, prec, err)
+            out[prec] = err
+            if Hfull is not None:
+                errf = np.abs(Hd.cpu().numpy().astype(np.float64) - Hfull).max() / cfg.Ms
+                assert errf <= tol, (cfg.name, prec, "full field", errf)
+            # properties that hold at any size: energy >= 0, M untouched
+            E = torch.zeros(1, dtype=torch.float64, device="cuda")
+            p.energy(Md, Hd, E)
+            torch.cuda.synchronize()
+            assert E.item() > 0
+            assert torch.equal(Md.cpu(), torch.from_numpy(M).to(dt))
+            del Md, Hd
+        torch.cuda.empty_cache()
+    return out
+
+
+def test_config2_film_1024x1024x1(torch, B, oracle):
+    from paper_2308_08447_b200 import workloads as W
+    cfg = W.CONFIGS["C2"]
+    M = W.make_magnetisation(cfg)
+    _sampled_check(torch, B, oracle, cfg, M, (0, 1), 256, full_field=True)
+
+
+def test_config3_256x256x64_fp32_and_fp64(torch, B, oracle):
+    from paper_2308_08447_b200 import workloads as W
+    _need_host_gb(24)
+    cfg = W.CONFIGS["C3"]
+    M = W.make_magnetisation(cfg)            # fp32; the fp64 plan gets the same values widened
+    _sampled_check(torch, B, oracle, cfg, M, (0, 1), 256, full_field=True)
+
+
+def test_config4_4096x4096x8(torch, B, oracle):
+    from paper_2308_08447_b200 import workloads as W
+    _need_host_gb(40)
+    cfg = W.CONFIGS["C4"]
+    M = W.make_magnetisation(cfg)
+    _sampled_check(torch, B, oracle, cfg, M, (0,), 48, full_field=False)
+
+
+def test_config5_atomistic_1024cubed(torch, B, oracle):
+    """1024^3 spins -> 4x4x4 macrocells -> 256^3 mesh -> field scattered back per spin (Eq. (9))."""
+    from paper_2308_08447_b200 import workloads as W
+    _need_host_gb(24)
+    if torch.cuda.get_device_properties(0).total_memory < 60 * 2 ** 30:
+        pytest.skip("needs ~45 GB of device memory")
+    cfg = W.CONFIGS["C5"]
+    c, a, mu_s = cfg.macro, cfg.a, cfg.mu_s
+    n = cfg.n
+    L = tuple(v * k for v, k in zip(n, c))
+    S = W.random_spins_torch(L, cfg.seed)                                   # device, 12.9 GB
+    # oracle side: average the spins in fp64 on the host, slab by slab (Eq. (9))
+    Mref = np.empty((3, n[2], n[1], n[0]))
+    for Z in range(n[2]):
+        slab = S[:, Z * c[2]:(Z + 1) * c[2]].cpu().numpy()
+        Mref[:, Z:Z + 1] = oracle.macrocell_average(slab, c, mu_s, a)
+    T = oracle.tensor_table(n, cfg.h)
+    cells = W.sample_cells(n, 64, cfg.seed)
+    Href = oracle.direct_sum_sampled(T, Mref, cells)                        # [64][3]
+    with B.Plan(n, cfg.h, 0, B.DEMAG_FP32) as p:
+        p.set_kernel(T)
+        Hs = torch.full_like(S, float("nan"))
+        p.apply_atomistic(S, Hs, c, mu_s, a)
+        torch.cuda.synchronize()
+        worst = 0.0
+        for s_, i in enumerate(cells):
+            ix, iy, iz = int(i % n[0]), int((i // n[0]) % n[1]), int(i // (n[0] * n[1]))
+            blk = Hs[:, iz * c[2]:(iz + 1) * c[2], iy * c[1]:(iy + 1) * c[1], ix * c[0]:(ix + 1) * c[0]].cpu().numpy()
+            assert np.all(blk == blk[:, :1, :1, :1])                         # every spin of the cell: same bits
+            worst = max(worst, np.abs(blk[:, 0, 0, 0].astype(np.float64) - Href[s_]).max() / cfg.Ms)
+        assert worst <= TOL32, worst
+        # one whole spin layer: no NaN left, piecewise constant over 4x4 blocks
+        layer = Hs[:, 5].cpu().numpy()
+        assert not np.isnan(layer).any()
+        assert np.array_equal(layer, np.repeat(np.repeat(layer[:, ::c[1], ::c[0]], c[1], axis=1), c[0], axis=2))
