@@ -109,6 +109,12 @@ demag_status demag_apply_profiled(demag_plan_t plan, const void* M_dev, void* H_
 /* Number of kernel launches one demag_apply enqueues with the current settings. */
 int demag_launches_per_apply(demag_plan_t plan);
 
+/* Which kernel family demag_apply uses for this plan: 1 = the compile-time specialised two-lines-per-thread
+ * kernels (all axes zero padded, sizes in their instantiated range), 0 = the size-generic kernels.  Both compute
+ * the same convolution (Appendix A).  The environment variable DEMAG_PATH=generic, read by
+ * demag_plan_create, forces 0 (used by the tests to cover both families). */
+int demag_path(demag_plan_t plan);
+
 /* Last error message of the calling thread ("" if none). */
 const char* demag_last_error(void);
 

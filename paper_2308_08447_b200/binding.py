@@ -21,7 +21,7 @@ STATUS = {0: "DEMAG_OK", 1: "DEMAG_ERR_INVALID_ARG", 2: "DEMAG_ERR_UNSUPPORTED",
 
 EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy", "demag_apply_atomistic",
            "demag_get_kernel_real", "demag_workspace_bytes", "demag_set_slab", "demag_launches_per_apply",
-           "demag_last_error", "demag_plan_destroy", "demag_apply_profiled"]
+           "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path"]
 
 
 class DemagError(RuntimeError):
@@ -54,6 +54,8 @@ def lib():
         L.demag_set_slab.argtypes = [vp, i]
         L.demag_launches_per_apply.argtypes = [vp]
         L.demag_launches_per_apply.restype = i
+        L.demag_path.argtypes = [vp]
+        L.demag_path.restype = i
         L.demag_last_error.restype = ctypes.c_char_p
         L.demag_plan_destroy.argtypes = [vp]
         for name in EXPORTS:
@@ -131,6 +133,10 @@ def demag_launches_per_apply(plan) -> int:
     return int(lib().demag_launches_per_apply(plan))
 
 
+def demag_path(plan) -> int:
+    return int(lib().demag_path(plan))
+
+
 def demag_plan_destroy(plan):
     _check(lib().demag_plan_destroy(plan))
 
@@ -166,6 +172,9 @@ class Plan:
 
     def launches_per_apply(self):
         return demag_launches_per_apply(self.handle)
+
+    def path(self):
+        return demag_path(self.handle)
 
     def set_slab(self, k):
         demag_set_slab(self.handle, k)

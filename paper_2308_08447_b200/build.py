@@ -7,7 +7,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "plan.cu")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("plan.cu", "kernels.cuh", "kernels_fast.cuh", "kernels_z.cuh", "fft_core.cuh", "builder.cuh")] + \
+DEPS = [os.path.join(HERE, "csrc", f) for f in ("plan.cu", "kernels.cuh", "kernels_fast.cuh", "kernels_z.cuh", "fft_core.cuh", "builder.cuh", "soa_core.cuh", "kernels_v2.cuh", "v2_host.cuh")] + \
        [os.path.join(os.path.dirname(HERE), "include", "demag.h")]
 LIB = os.path.join(HERE, "libdemag_b200.so")
 

@@ -1,0 +1,525 @@
+// kernels_v2.cuh -- the fast hot path of demag_apply: compile-time specialised kernels that process TWO lines
+// per thread in packed fp32 (soa_core.cuh).  Same mathematics and execution order as kernels.cuh
+// (x R2C -> y FFT -> z FFT . kernel multiplication . z IFFT -> y IFFT -> x C2R), different
+// data layout of the private workspaces:
+//
+//   W1v [3][hq][nz][ny] quads   one quad = x-frequencies (k, Lc-k) of one (y,z): the pair the Hermitian split of
+//                               the real transform produces / consumes together (hq = Lc/2 + 1, Lc = Nx/2 = nx)
+//   W2v [3][nq][nz][Ny] quads   slab of nq pairs; y in the digit-reversed "position order" the forward passes
+//                               leave behind (the stored kernel spectrum uses the same order: nothing is permuted)
+//   Kv  [hq][Nz/2+1][Ny] KQ     the six real components for the two frequencies of the pair, z packed by symmetry
+//                               (PAPER.md:255-256), the y parity sign, -1/(Nx Ny Nz) and the 1/2 of the real
+//                               split folded in at plan time
+//
+// Every kernel is templated on log2 of its transform length, its tile and its block size, so that every
+// shared-memory offset is an immediate; twiddles come from per-pass tables (dup format, [m-1][lo]).
+#pragma once
+#include "soa_core.cuh"
+
+namespace demag {
+namespace v2 {
+
+extern __shared__ __align__(32) unsigned char smem_v2[];
+
+struct GeoV {
+    int nx, ny, nz;      // mesh
+    int Ny, Nz;          // padded (2 ny, 2 nz)
+    int Lc;              // complex length of the packed real x transform = nx (Nx = 2 nx)
+    int hq;              // number of (k, Lc-k) pairs = Lc/2 + 1
+    int kpz;             // Nz/2 + 1
+};
+
+template <typename T> struct TwSet { const CQ<T>* p[6]; };   // per-pass twiddle tables (NULL for stride-1 passes)
+
+template <typename T> struct alignas(4 * sizeof(T)) KQ {     // kernel spectrum at one (q, kz', py): pairs over the two kx
+    typename vec2<T>::type xx, yy, zz, xy, xz, yz;
+};
+
+// ---- 128-bit quad access ----------------------------------------------------------------------------
+__device__ __forceinline__ CQ<float> ldq(const CQ<float>* p)
+{
+    const float4 v = *reinterpret_cast<const float4*>(p);
+    CQ<float> r; r.re = make_float2(v.x, v.y); r.im = make_float2(v.z, v.w); return r;
+}
+__device__ __forceinline__ void stq(CQ<float>* p, CQ<float> a)
+{
+    *reinterpret_cast<float4*>(p) = make_float4(a.re.x, a.re.y, a.im.x, a.im.y);
+}
+__device__ __forceinline__ CQ<float> ldgq(const CQ<float>* p)
+{
+    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+    CQ<float> r; r.re = make_float2(v.x, v.y); r.im = make_float2(v.z, v.w); return r;
+}
+__device__ __forceinline__ CQ<double> ldq(const CQ<double>* p)
+{
+    const double2* q = reinterpret_cast<const double2*>(p);
+    CQ<double> r; r.re = q[0]; r.im = q[1]; return r;
+}
+__device__ __forceinline__ void stq(CQ<double>* p, CQ<double> a)
+{
+    double2* q = reinterpret_cast<double2*>(p);
+    q[0] = a.re; q[1] = a.im;
+}
+__device__ __forceinline__ CQ<double> ldgq(const CQ<double>* p)
+{
+    const double2* q = reinterpret_cast<const double2*>(p);
+    CQ<double> r; r.re = __ldg(q); r.im = __ldg(q + 1); return r;
+}
+
+// twiddles of one butterfly: w^(lo m), m = 1..R-1, from the pass table [m-1][lo]
+template <int LR, int LS, typename T>
+__device__ __forceinline__ void load_tw(CQ<T>* w, const CQ<T>* __restrict__ tab, int lo)
+{
+#pragma unroll
+    for (int m = 1; m < (1 << LR); ++m) w[m] = ldgq(tab + ((m - 1) << LS) + lo);
+}
+template <int LR, bool INV, typename T>
+__device__ __forceinline__ void apply_tw(CQ<T>* a, const CQ<T>* w)
+{
+#pragma unroll
+    for (int m = 1; m < (1 << LR); ++m) a[m] = ctw<INV>(a[m], w[m]);
+}
+
+// ---- one in-place pass over a shared-memory tile s[p][PITCH], lines fastest ---------------------------------
+// pass J of schedule SC on lines of length 2^LL; BL lines (quads) per tile; NT threads.
+template <typename T, int LL, int POL, int J, bool INV, int BL, int PITCH, int NT>
+__device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab, int tid)
+{
+    constexpr Sched SC = make_sched(LL, POL);
+    constexpr int LR = SC.lr[J], LS = SC.ls[J], R = 1 << LR, S = 1 << LS;
+    constexpr int NBF = 1 << (LL - LR);            // butterflies per line
+    constexpr int TOT = NBF * BL;
+    constexpr int ITER = (TOT + NT - 1) / NT;
+    constexpr bool HOIST = (LS > 0) && (NT % BL == 0) && ((NT / BL) % S == 0) && ITER > 1;
+    CQ<T> w[R];
+    if (HOIST) load_tw<LR, LS>(w, tab, (tid / BL) & (S - 1));
+#pragma unroll(ITER <= 2 ? ITER : 1)
+    for (int k = 0; k < ITER; ++k) {
+        const int t = tid + k * NT;
+        if (TOT % NT != 0 && t >= TOT) break;
+        const int b = t % BL, i = t / BL;
+        const int lo = i & (S - 1);
+        const int p0 = ((i >> LS) << (LS + LR)) + lo;
+        CQ<T>* d = s + p0 * PITCH + b;
+        CQ<T> a[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * S * PITCH);
+        if (!INV) {
+            dftR<LR, false, false>(a);
+            if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, lo); apply_tw<LR, false>(a, w); }
+        } else {
+            if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, lo); apply_tw<LR, true>(a, w); }
+            dftR<LR, true, false>(a);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) stq(d + r * S * PITCH, a[r]);
+    }
+}
+// forward passes J..J1-1 (each followed by a barrier) / inverse passes J-1 down to J0
+template <typename T, int LL, int POL, int J, int J1, int BL, int PITCH, int NT> struct FwdPasses {
+    static __device__ __forceinline__ void run(CQ<T>* s, const TwSet<T>& tw, int tid)
+    {
+        pass_ss<T, LL, POL, J, false, BL, PITCH, NT>(s, tw.p[J], tid);
+        __syncthreads();
+        FwdPasses<T, LL, POL, J + 1, J1, BL, PITCH, NT>::run(s, tw, tid);
+    }
+};
+template <typename T, int LL, int POL, int J1, int BL, int PITCH, int NT> struct FwdPasses<T, LL, POL, J1, J1, BL, PITCH, NT> {
+    static __device__ __forceinline__ void run(CQ<T>*, const TwSet<T>&, int) {}
+};
+template <typename T, int LL, int POL, int J0, int J, int BL, int PITCH, int NT> struct InvPasses {   // runs J-1, J-2, .., J0
+    static __device__ __forceinline__ void run(CQ<T>* s, const TwSet<T>& tw, int tid)
+    {
+        pass_ss<T, LL, POL, J - 1, true, BL, PITCH, NT>(s, tw.p[J - 1], tid);
+        __syncthreads();
+        InvPasses<T, LL, POL, J0, J - 1, BL, PITCH, NT>::run(s, tw, tid);
+    }
+};
+template <typename T, int LL, int POL, int J0, int BL, int PITCH, int NT> struct InvPasses<T, LL, POL, J0, J0, BL, PITCH, NT> {
+    static __device__ __forceinline__ void run(CQ<T>*, const TwSet<T>&, int) {}
+};
+
+// position of frequency k for schedule (LL, POL), at run time (a few shifts and masks)
+template <int LL, int POL> __device__ __forceinline__ int pos_of_freq_rt(int k)
+{
+    constexpr Sched SC = make_sched(LL, POL);
+    int p = 0, w = 0;
+#pragma unroll
+    for (int j = 0; j < SC.n; ++j) {
+        p += ((k >> w) & ((1 << SC.lr[j]) - 1)) << SC.ls[j];
+        w += SC.lr[j];
+    }
+    return p;
+}
+template <int LL, int POL> __device__ __forceinline__ int freq_of_pos_rt(int p)
+{
+    constexpr Sched SC = make_sched(LL, POL);
+    int k = 0, w = 0;
+#pragma unroll
+    for (int j = 0; j < SC.n; ++j) {
+        k += ((p >> SC.ls[j]) & ((1 << SC.lr[j]) - 1)) << w;
+        w += SC.lr[j];
+    }
+    return k;
+}
+
+// first forward pass (pass 0) with the inputs coming from ld(line, point) and the upper half of every line zero
+// (the padding); threads walk the point index fastest.  Results go to the tile.
+// LF = false: threads walk the point index fastest (lines contiguous in memory); LF = true: lines fastest.
+template <typename T, int LL, int POL, int BL, int PITCH, int NT, bool LF, typename LD>
+__device__ __forceinline__ void pass_first(CQ<T>* s, const CQ<T>* __restrict__ tab, int tid, LD ld)
+{
+    constexpr Sched SC = make_sched(LL, POL);
+    constexpr int LR = SC.lr[0], LS = SC.ls[0], R = 1 << LR, S = 1 << LS;
+    constexpr int TOT = S * BL;
+    constexpr int ITER = (TOT + NT - 1) / NT;
+    constexpr bool HOIST = (LS > 0) && ITER > 1 && (LF ? (NT % BL == 0 && (NT / BL) % S == 0) : (NT % S == 0));
+    CQ<T> w[R];
+    if (HOIST) load_tw<LR, LS>(w, tab, LF ? ((tid / BL) & (S - 1)) : (tid & (S - 1)));
+#pragma unroll(ITER <= 2 ? ITER : 1)
+    for (int k = 0; k < ITER; ++k) {
+        const int t = tid + k * NT;
+        if (TOT % NT != 0 && t >= TOT) break;
+        const int i = LF ? ((t / BL) & (S - 1)) : (t & (S - 1)), b = LF ? (t % BL) : (t >> LS);
+        CQ<T> a[R];
+        if (R > 1) {
+#pragma unroll
+            for (int r = 0; r < R / 2; ++r) a[r] = ld(b, i + r * S);
+        } else a[0] = ld(b, i);
+        dftR<LR, false, true>(a);
+        if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, false>(a, w); }
+        CQ<T>* d = s + i * PITCH + b;
+#pragma unroll
+        for (int r = 0; r < R; ++r) stq(d + r * S * PITCH, a[r]);
+    }
+}
+// last inverse pass (pass 0 backwards): outputs r < R/2 (the crop) go to st(line, point, value)
+template <typename T, int LL, int POL, int BL, int PITCH, int NT, bool LF, typename ST>
+__device__ __forceinline__ void pass_last(const CQ<T>* s, const CQ<T>* __restrict__ tab, int tid, ST st)
+{
+    constexpr Sched SC = make_sched(LL, POL);
+    constexpr int LR = SC.lr[0], LS = SC.ls[0], R = 1 << LR, S = 1 << LS;
+    constexpr int TOT = S * BL;
+    constexpr int ITER = (TOT + NT - 1) / NT;
+    constexpr bool HOIST = (LS > 0) && ITER > 1 && (LF ? (NT % BL == 0 && (NT / BL) % S == 0) : (NT % S == 0));
+    CQ<T> w[R];
+    if (HOIST) load_tw<LR, LS>(w, tab, LF ? ((tid / BL) & (S - 1)) : (tid & (S - 1)));
+#pragma unroll(ITER <= 2 ? ITER : 1)
+    for (int k = 0; k < ITER; ++k) {
+        const int t = tid + k * NT;
+        if (TOT % NT != 0 && t >= TOT) break;
+        const int i = LF ? ((t / BL) & (S - 1)) : (t & (S - 1)), b = LF ? (t % BL) : (t >> LS);
+        const CQ<T>* d = s + i * PITCH + b;
+        CQ<T> a[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * S * PITCH);
+        if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, true>(a, w); }
+        dftR<LR, true, false>(a);
+#pragma unroll
+        for (int r = 0; r < R / 2; ++r) st(b, i + r * S, a[r]);
+    }
+}
+
+// =========================================================================================== K2v / K4v: y stage
+// lines l = (c*nq + ql)*nz + z of the slab [q0, q0+nq); a tile = BP consecutive lines (quads: two x-frequencies each).
+__device__ __forceinline__ long long w1v_line_offset(const GeoV& g, int l, int q0, int nq)
+{
+    const int z = l % g.nz, ck = l / g.nz, ql = ck % nq, c = ck / nq;
+    return (((long long)c * g.hq + q0 + ql) * g.nz + z) * g.ny;
+}
+
+// y forward FFT, zero padding synthesised (PAPER.md:309-315 yFFT): W1v -> W2v (position order)
+template <typename T, int LNY, int POL, int BP, int NT>
+__global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
+                                               CQ<T>* __restrict__ W2, TwSet<T> tw)
+{
+    constexpr int NY = 1 << LNY, PITCH = BP | 1;
+    constexpr Sched SC = make_sched(LNY, POL);
+    CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
+    __shared__ long long loff[BP];
+    const int tid = threadIdx.x;
+    const int nlines = 3 * nq * g.nz;
+    const int l0 = blockIdx.x * BP;
+    if (tid < BP) loff[tid] = (l0 + tid < nlines) ? w1v_line_offset(g, l0 + tid, q0, nq) : -1;
+    __syncthreads();
+    auto ld = [&](int b, int p) { const long long o = loff[b]; return o >= 0 ? ldgq(W1 + o + p) : cq_zero<T>(); };
+    pass_first<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, ld);
+    __syncthreads();
+    FwdPasses<T, LNY, POL, 1, SC.n, BP, PITCH, NT>::run(s, tw, tid);
+    CQ<T>* dst = W2 + (size_t)l0 * NY;
+    const int nvalid = min(BP, nlines - l0);
+#pragma unroll 4
+    for (int idx = tid; idx < (nvalid << LNY); idx += NT) {
+        const int b = idx >> LNY, p = idx & (NY - 1);
+        stq(dst + idx, ldq(s + p * PITCH + b));
+    }
+}
+
+// y inverse FFT fused with the crop: W2v -> W1v
+template <typename T, int LNY, int POL, int BP, int NT>
+__global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
+                                               CQ<T>* __restrict__ W1, TwSet<T> tw)
+{
+    constexpr int NY = 1 << LNY, PITCH = BP | 1;
+    constexpr Sched SC = make_sched(LNY, POL);
+    CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
+    __shared__ long long loff[BP];
+    const int tid = threadIdx.x;
+    const int nlines = 3 * nq * g.nz;
+    const int l0 = blockIdx.x * BP;
+    if (tid < BP) loff[tid] = (l0 + tid < nlines) ? w1v_line_offset(g, l0 + tid, q0, nq) : -1;
+    const CQ<T>* src = W2 + (size_t)l0 * NY;
+    const int nvalid = min(BP, nlines - l0);
+#pragma unroll 4
+    for (int idx = tid; idx < (BP << LNY); idx += NT) {
+        const int b = idx >> LNY, p = idx & (NY - 1);
+        stq(s + p * PITCH + b, b < nvalid ? ldgq(src + idx) : cq_zero<T>());
+    }
+    __syncthreads();
+    InvPasses<T, LNY, POL, 1, SC.n, BP, PITCH, NT>::run(s, tw, tid);
+    auto st = [&](int b, int p, CQ<T> v) { const long long o = loff[b]; if (o >= 0) stq(W1 + o + p, v); };
+    pass_last<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, st);
+}
+
+// =========================================================================================== K3v: z stage
+// z FFT . kernel multiplication . z IFFT "in the same routine" (PAPER.md:343; :316-326 zFFT, KernelMultiplication).
+template <typename T> __device__ __forceinline__ KQ<T> ldk(const KQ<T>* p);
+template <> __device__ __forceinline__ KQ<float> ldk<float>(const KQ<float>* p)
+{
+    const float4* q = reinterpret_cast<const float4*>(p);
+    const float4 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2);
+    KQ<float> k;
+    k.xx = make_float2(a.x, a.y); k.yy = make_float2(a.z, a.w); k.zz = make_float2(b.x, b.y);
+    k.xy = make_float2(b.z, b.w); k.xz = make_float2(c.x, c.y); k.yz = make_float2(c.z, c.w);
+    return k;
+}
+template <> __device__ __forceinline__ KQ<double> ldk<double>(const KQ<double>* p)
+{
+    const double2* q = reinterpret_cast<const double2*>(p);
+    KQ<double> k;
+    k.xx = __ldg(q); k.yy = __ldg(q + 1); k.zz = __ldg(q + 2); k.xy = __ldg(q + 3); k.xz = __ldg(q + 4); k.yz = __ldg(q + 5);
+    return k;
+}
+// H^_a = sum_b K^_ab M^_b, K^ real and symmetric.  SGN: sign of the z-odd components xz, yz
+// (+1 direct, -1 mirrored kz > Nz/2, 0 = run-time sign sg).
+template <int SGN, typename T>
+__device__ __forceinline__ void apply_kernel(const KQ<T>& k, CQ<T>& mx, CQ<T>& my, CQ<T>& mz, T sg)
+{
+    typename vec2<T>::type kxz = k.xz, kyz = k.yz;
+    if (SGN < 0) { kxz = vneg(kxz); kyz = vneg(kyz); }
+    if (SGN == 0) { kxz = vmul(kxz, vdup(sg)); kyz = vmul(kyz, vdup(sg)); }
+    CQ<T> hx, hy, hz;
+    hx.re = vfma(kxz, mz.re, vfma(k.xy, my.re, vmul(k.xx, mx.re)));
+    hx.im = vfma(kxz, mz.im, vfma(k.xy, my.im, vmul(k.xx, mx.im)));
+    hy.re = vfma(kyz, mz.re, vfma(k.yy, my.re, vmul(k.xy, mx.re)));
+    hy.im = vfma(kyz, mz.im, vfma(k.yy, my.im, vmul(k.xy, mx.im)));
+    hz.re = vfma(k.zz, mz.re, vfma(kyz, my.re, vmul(kxz, mx.re)));
+    hz.im = vfma(k.zz, mz.im, vfma(kyz, my.im, vmul(kxz, mx.im)));
+    mx = hx; my = hy; mz = hz;
+}
+
+// multiply the RF points of one fused butterfly (positions p0..p0+RF-1 <-> kz = f0 + m Nz/RF)
+template <typename T, int LNZ, int LRF, int M> struct MulPoints {
+    static __device__ __forceinline__ void run(CQ<T> (*a)[1 << LRF], const KQ<T>* __restrict__ Kcol, int Ny, int f0)
+    {
+        constexpr int NZ = 1 << LNZ, RF = 1 << LRF, W = NZ >> LRF;
+        const int kz = f0 + M * W;
+        if (RF == 1 || 2 * M < RF) {
+            apply_kernel<1>(ldk(Kcol + (size_t)kz * Ny), a[0][M], a[1][M], a[2][M], (T)1);
+        } else if (2 * M > RF) {
+            apply_kernel<-1>(ldk(Kcol + (size_t)(NZ - kz) * Ny), a[0][M], a[1][M], a[2][M], (T)1);
+        } else {
+            const bool mir = f0 > 0;
+            apply_kernel<0>(ldk(Kcol + (size_t)(mir ? NZ - kz : kz) * Ny), a[0][M], a[1][M], a[2][M], mir ? (T)-1 : (T)1);
+        }
+        MulPoints<T, LNZ, LRF, M + 1>::run(a, Kcol, Ny, f0);
+    }
+};
+template <typename T, int LNZ, int LRF> struct MulPoints<T, LNZ, LRF, (1 << LRF)> {
+    static __device__ __forceinline__ void run(CQ<T> (*)[1 << LRF], const KQ<T>* __restrict__, int, int) {}
+};
+
+// Nz >= 16 (at least two passes).  Tile = one pair plane ql x TY consecutive py x all z x 3 components:
+// shared s[Nz][3 TY] quads, lines fastest everywhere (a warp's accesses are consecutive quads: conflict free).
+template <typename T, int LNZ, int POL, int TY, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const KQ<T>* __restrict__ K, TwSet<T> tw)
+{
+    constexpr int NZ = 1 << LNZ, B = 3 * TY;
+    constexpr Sched SC = make_sched(LNZ, POL);
+    constexpr int NP = SC.n, LRF = SC.lr[NP - 1], RF = 1 << LRF;
+    static_assert(NP >= 2 && NT % TY == 0, "k_z_v: needs >= 2 passes");
+    CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
+    const int tid = threadIdx.x;
+    const int tilesY = g.Ny / TY;
+    const int pyt = blockIdx.x % tilesY, ql = blockIdx.x / tilesY;
+    const int py0 = pyt * TY;
+    const size_t cstride = (size_t)nq * g.nz * g.Ny;
+    CQ<T>* base = W2 + (size_t)ql * g.nz * g.Ny + py0;
+    const int Ny = g.Ny;
+    auto ld = [&](int b, int z) { const int c = b / TY, ty = b - c * TY; return ldq(base + c * cstride + (size_t)z * Ny + ty); };
+    pass_first<T, LNZ, POL, B, B, NT, true>(s, tw.p[0], tid, ld);
+    __syncthreads();
+    FwdPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
+    {   // fused: last forward pass . multiply . first inverse pass; item = (butterfly i, column ty), 3 components
+        constexpr int NBF = NZ >> LRF, TOT = NBF * TY, ITER = (TOT + NT - 1) / NT;
+        const KQ<T>* Kq = K + (size_t)(q0 + ql) * g.kpz * Ny + py0;
+#pragma unroll 1
+        for (int k = 0; k < ITER; ++k) {
+            const int t = tid + k * NT;
+            if (TOT % NT != 0 && t >= TOT) break;
+            const int ty = t % TY, i = t / TY;
+            const int p0 = i << LRF;
+            CQ<T> a[3][RF];
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+#pragma unroll
+                for (int m = 0; m < RF; ++m) a[cc][m] = ldq(s + (p0 + m) * B + cc * TY + ty);
+                dftR<LRF, false, false>(a[cc]);
+            }
+            const int f0 = freq_of_pos_rt<LNZ, POL>(p0);
+            MulPoints<T, LNZ, LRF, 0>::run(a, Kq + ty, Ny, f0);
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+                dftR<LRF, true, false>(a[cc]);
+#pragma unroll
+                for (int m = 0; m < RF; ++m) stq(s + (p0 + m) * B + cc * TY + ty, a[cc][m]);
+            }
+        }
+    }
+    __syncthreads();
+    InvPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
+    auto st = [&](int b, int z, CQ<T> v) { const int c = b / TY, ty = b - c * TY; stq(base + c * cstride + (size_t)z * Ny + ty, v); };
+    pass_last<T, LNZ, POL, B, B, NT, true>(s, tw.p[0], tid, st);
+}
+
+// Nz <= 8: the whole z transform of a column is one butterfly per component in registers; no shared memory.
+// grid = nq * Ny / 128 (or fewer columns per block if Ny < 128), block = min(Ny, 128).
+template <typename T, int LNZ>
+__global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2, const KQ<T>* __restrict__ K)
+{
+    constexpr int RF = 1 << LNZ;
+    const int cols = blockDim.x;
+    const int tilesY = g.Ny / cols;
+    const int pyt = blockIdx.x % tilesY, ql = blockIdx.x / tilesY;
+    const int py = pyt * cols + threadIdx.x;
+    const size_t cstride = (size_t)nq * g.nz * g.Ny;
+    CQ<T>* col = W2 + (size_t)ql * g.nz * g.Ny + py;
+    const int Ny = g.Ny;
+    CQ<T> a[3][RF];
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+#pragma unroll
+        for (int m = 0; m < (RF > 1 ? RF / 2 : 1); ++m) a[cc][m] = ldq(col + cc * cstride + (size_t)m * Ny);
+        dftR<LNZ, false, true>(a[cc]);
+    }
+    MulPoints<T, LNZ, LNZ, 0>::run(a, K + (size_t)(q0 + ql) * g.kpz * Ny + py, Ny, 0);
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+        dftR<LNZ, true, false>(a[cc]);
+#pragma unroll
+        for (int m = 0; m < (RF > 1 ? RF / 2 : 1); ++m) stq(col + cc * cstride + (size_t)m * Ny, a[cc][m]);
+    }
+}
+
+// =========================================================================================== K1v / K5v: x stage
+// A tile = RP pairs of consecutive y rows of one (component, z); the two rows of a pair are the two lines of a quad.
+// The real rows are transformed as packed complex sequences z[m] = x[2m] + i x[2m+1] of length Lc (upper half
+// zero: the padding), then split into the real transform's bins k and Lc-k together:
+//   2 X[k] = A - i w^k D,  2 X[Lc-k] = conj(A + i w^k D),  A = Z[k] + conj Z[Lc-k],  D = Z[k] - conj Z[Lc-k],
+// w = exp(-2 pi i / 2Lc).  The factor 2 is folded into the stored kernel spectrum.
+
+// x R2C FFT fused with the zero padding and the transposition to y-contiguous storage
+// (PAPER.md:35, :296-300 xFFT_R2C; :343 "xy transposition ... to avoid strided y FFTs"):  M -> W1v
+template <typename T, int LLC, int POL, int RP, int NT>
+__global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
+                                               TwSet<T> tw, const CQ<T>* __restrict__ twpost)
+{
+    using V = typename vec2<T>::type;
+    constexpr int LC = 1 << LLC, PITCH = RP | 1;
+    constexpr Sched SC = make_sched(LLC, POL);
+    CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
+    const int tid = threadIdx.x;
+    const int tilesY = g.ny / (2 * RP);
+    const int ty = blockIdx.x % tilesY, cz = blockIdx.x / tilesY;
+    const int y0 = ty * 2 * RP;
+    const int nx = g.nx;
+    const T* rows = M + ((size_t)cz * g.ny + y0) * nx;
+    auto ld = [&](int b, int m) {
+        const V r0 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b) * nx + 2 * m));
+        const V r1 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b + 1) * nx + 2 * m));
+        CQ<T> q; q.re.x = r0.x; q.re.y = r1.x; q.im.x = r0.y; q.im.y = r1.y; return q;
+    };
+    pass_first<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, ld);
+    __syncthreads();
+    FwdPasses<T, LLC, POL, 1, SC.n, RP, PITCH, NT>::run(s, tw, tid);
+    const int c = cz / g.nz, z = cz - c * g.nz;
+    const size_t plane = (size_t)g.nz * g.ny;
+    CQ<T>* out = W1 + ((size_t)c * g.hq * g.nz + z) * g.ny + y0;
+    constexpr int TOT = (LC / 2 + 1) * RP;
+#pragma unroll 2
+    for (int t = tid; t < TOT; t += NT) {
+        const int b = t % RP, k = t / RP;
+        const CQ<T> Zk = ldq(s + pos_of_freq_rt<LLC, POL>(k) * PITCH + b);
+        const CQ<T> Zm = ldq(s + pos_of_freq_rt<LLC, POL>((LC - k) & (LC - 1)) * PITCH + b);
+        const CQ<T> w = ldgq(twpost + k);
+        CQ<T> D; D.re = vsub(Zk.re, Zm.re); D.im = vadd(Zk.im, Zm.im);
+        const V A = vadd(Zk.re, Zm.re), Bm = vsub(Zk.im, Zm.im);
+        const CQ<T> u = cmul(D, w);
+        const V xkr = vadd(A, u.im), xki = vsub(Bm, u.re), xmr = vsub(A, u.im), xmi = vneg(vadd(Bm, u.re));
+        CQ<T> o0, o1;
+        o0.re.x = xkr.x; o0.re.y = xmr.x; o0.im.x = xki.x; o0.im.y = xmi.x;
+        o1.re.x = xkr.y; o1.re.y = xmr.y; o1.im.x = xki.y; o1.im.y = xmi.y;
+        CQ<T>* d = out + (size_t)k * plane + 2 * b;
+        stq(d, o0); stq(d + 1, o1);
+    }
+}
+
+// x C2R FFT fused with the crop; writes H:  W1v -> H
+//   2 Z[k] = A + i u,  2 Z[Lc-k] = conj(A - i u),  A = X[k] + conj X[Lc-k],  u = conj(w^k) (X[k] - conj X[Lc-k])
+template <typename T, int LLC, int POL, int RP, int NT>
+__global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict__ W1, T* __restrict__ H,
+                                               TwSet<T> tw, const CQ<T>* __restrict__ twpost)
+{
+    using V = typename vec2<T>::type;
+    constexpr int LC = 1 << LLC, PITCH = RP | 1;
+    constexpr Sched SC = make_sched(LLC, POL);
+    CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
+    const int tid = threadIdx.x;
+    const int tilesY = g.ny / (2 * RP);
+    const int ty = blockIdx.x % tilesY, cz = blockIdx.x / tilesY;
+    const int y0 = ty * 2 * RP;
+    const int c = cz / g.nz, z = cz - c * g.nz;
+    const size_t plane = (size_t)g.nz * g.ny;
+    const CQ<T>* in = W1 + ((size_t)c * g.hq * g.nz + z) * g.ny + y0;
+    constexpr int TOT = (LC / 2 + 1) * RP;
+#pragma unroll 2
+    for (int t = tid; t < TOT; t += NT) {
+        const int b = t % RP, k = t / RP;
+        const CQ<T>* d = in + (size_t)k * plane + 2 * b;
+        const CQ<T> Q0 = ldgq(d), Q1 = ldgq(d + 1);
+        V xkr, xmr, xki, xmi;
+        xkr.x = Q0.re.x; xkr.y = Q1.re.x; xmr.x = Q0.re.y; xmr.y = Q1.re.y;
+        xki.x = Q0.im.x; xki.y = Q1.im.x; xmi.x = Q0.im.y; xmi.y = Q1.im.y;
+        const V Ar = vadd(xkr, xmr), Ai = vsub(xki, xmi);
+        CQ<T> D; D.re = vsub(xkr, xmr); D.im = vadd(xki, xmi);
+        const CQ<T> u = cmulc(D, ldgq(twpost + k));
+        CQ<T> Zk, Zm;
+        Zk.re = vsub(Ar, u.im); Zk.im = vadd(Ai, u.re);
+        Zm.re = vadd(Ar, u.im); Zm.im = vsub(u.re, Ai);
+        stq(s + pos_of_freq_rt<LLC, POL>(k) * PITCH + b, Zk);
+        if (k != 0 && 2 * k != LC) stq(s + pos_of_freq_rt<LLC, POL>(LC - k) * PITCH + b, Zm);
+    }
+    __syncthreads();
+    InvPasses<T, LLC, POL, 1, SC.n, RP, PITCH, NT>::run(s, tw, tid);
+    const int nx = g.nx;
+    T* rows = H + ((size_t)cz * g.ny + y0) * nx;
+    auto st = [&](int b, int m, CQ<T> v) {
+        V r0, r1; r0.x = v.re.x; r0.y = v.im.x; r1.x = v.re.y; r1.y = v.im.y;
+        *reinterpret_cast<V*>(rows + (size_t)(2 * b) * nx + 2 * m) = r0;
+        *reinterpret_cast<V*>(rows + (size_t)(2 * b + 1) * nx + 2 * m) = r1;
+    };
+    pass_last<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, st);
+}
+
+}  // namespace v2
+}  // namespace demag

@@ -14,6 +14,7 @@
 #include "builder.cuh"
 #include "kernels.cuh"
 #include "kernels_z.cuh"
+#include "v2_host.cuh"
 
 using namespace demag;
 
@@ -68,6 +69,12 @@ struct demag_plan_s {
     int nkx_slab, nkx_auto;
     bool fast1 = false, fast2 = false;   // kernels_fast.cuh variants of the x / y stages
     bool z_spec = false;                 // kernels_z.cuh compile-time specialised z stage
+    // fast path (kernels_v2.cuh): pair layout of W1 / W2 / K, per-pass twiddle tables
+    bool v2 = false;
+    int nq_slab = 0, nq_auto = 0;        // (k, Lc-k) pair planes per L2-resident slab
+    v2::Ctx<float> cf; v2::Ctx<double> cd;
+    v2::AxisTables<float> tf[3]; v2::AxisTables<double> td[3];
+    int* ypos2freq = nullptr;
 };
 
 namespace {
@@ -262,6 +269,28 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
     p->w2_bytes = (size_t)3 * p->nkx_auto * g.nz * g.Ny * csz;
     p->kcomp_stride = (size_t)g.hx * g.kpz * g.kpitch;
     p->k_bytes = 6 * p->kcomp_stride * p->esz;
+    {
+        const char* path = getenv("DEMAG_PATH");           // "generic" forces the size-generic kernels (tests, A/B timing)
+        p->v2 = !(path && !strcmp(path, "generic")) && pbc_flags == 0 &&
+                v2::supported(nx, ny, nz, g.Nx, g.Ny, g.Nz, g.lLc, g.lNy, g.lNz, p->esz, kMaxSmem);
+    }
+    if (p->v2) {
+        v2::GeoV gv;
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz;
+        p->cf.g = gv; p->cd.g = gv;
+        p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
+        const size_t qsz = 4 * p->esz;                      // one quad
+        const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;
+        size_t slab_bytes = kSlabBytes;
+        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoi(e) << 20;
+        long long n = (long long)(slab_bytes / per_q);
+        if (n < 1) n = 1;
+        if (n > gv.hq) n = gv.hq;
+        p->nq_auto = p->nq_slab = (int)n;
+        p->w1_bytes = (size_t)3 * gv.hq * g.nz * g.ny * qsz;
+        p->w2_bytes = (size_t)p->nq_auto * per_q;
+        p->k_bytes = (size_t)gv.hq * g.kpz * g.Ny * 12 * p->esz;
+    }
     auto alloc_all = [&]() -> demag_status {
         if (precision == DEMAG_FP32) { demag_status s = set_func_attrs<float>(); if (s) return s; }
         else { demag_status s = set_func_attrs<double>(); if (s) return s; }
@@ -273,6 +302,42 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
                 ? z_c_dispatch<float>(0, g, p->TY, 0, nullptr, 0, 0, nullptr, nullptr, 0, nullptr, &zerr)
                 : z_c_dispatch<double>(0, g, p->TY, 0, nullptr, 0, 0, nullptr, nullptr, 0, nullptr, &zerr);
             CUDA_TRY(zerr);
+        }
+        if (p->v2) {
+            const int LL[3] = {g.lLc, g.lNy, g.lNz};
+            const int POL[3] = {v2::x_pol(g.lLc), v2::y_pol(g.lNy), v2::z_pol(g.lNz)};
+            cudaError_t verr = cudaSuccess;
+            if (precision == DEMAG_FP32) {
+                for (int a = 0; a < 3; ++a) {
+                    CUDA_TRY(v2::build_axis_tables<float>(LL[a], POL[a], a == 0 ? nx : 0, &p->tf[a], a == 0 ? &p->cf.twpost : nullptr));
+                    p->tw_bytes += p->tf[a].bytes;
+                }
+                p->cf.twx = p->tf[0].set; p->cf.twy = p->tf[1].set; p->cf.twz = p->tf[2].set;
+                v2::x_fwd<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::x_inv<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::y_fwd<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::y_inv<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::z_mul<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+            } else {
+                for (int a = 0; a < 3; ++a) {
+                    CUDA_TRY(v2::build_axis_tables<double>(LL[a], POL[a], a == 0 ? nx : 0, &p->td[a], a == 0 ? &p->cd.twpost : nullptr));
+                    p->tw_bytes += p->td[a].bytes;
+                }
+                p->cd.twx = p->td[0].set; p->cd.twy = p->td[1].set; p->cd.twz = p->td[2].set;
+                v2::x_fwd<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::x_inv<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::y_fwd<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::y_inv<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                v2::z_mul<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+            }
+            {   // y position -> frequency map of the y schedule, for the plan-time pack
+                const v2::Sched sc = v2::make_sched(g.lNy, v2::y_pol(g.lNy));
+                std::vector<int> h((size_t)g.Ny);
+                for (int q = 0; q < g.Ny; ++q) h[q] = v2::sched_freq_of_pos(sc, q);
+                CUDA_TRY(cudaMalloc(&p->ypos2freq, sizeof(int) * (size_t)g.Ny));
+                CUDA_TRY(cudaMemcpy(p->ypos2freq, h.data(), sizeof(int) * (size_t)g.Ny, cudaMemcpyHostToDevice));
+                p->tw_bytes += sizeof(int) * (size_t)g.Ny;
+            }
         }
         CUDA_TRY(cudaMalloc(&p->W1, p->w1_bytes));
         CUDA_TRY(cudaMalloc(&p->W2, p->w2_bytes));
@@ -298,6 +363,8 @@ demag_status demag_plan_destroy(demag_plan_t p)
     cudaFree(p->W1); cudaFree(p->W2); cudaFree(p->K);
     for (int a = 0; a < 3; ++a) cudaFree(p->tw[a]);
     cudaFree(p->Mc); cudaFree(p->Hc);
+    for (int a = 0; a < 3; ++a) { cudaFree(p->tf[a].dev); cudaFree(p->td[a].dev); }
+    cudaFree(p->ypos2freq);
     delete p;
     return DEMAG_OK;
 }
@@ -312,6 +379,12 @@ demag_status demag_set_slab(demag_plan_t p, int kx_per_slab)
 {
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
     if (kx_per_slab < 0) return fail(DEMAG_ERR_INVALID_ARG, "kx_per_slab < 0");
+    if (p->v2) {                                // fast path: the slab unit is a (k, Lc-k) pair plane
+        int n = kx_per_slab == 0 ? p->nq_auto : kx_per_slab;
+        if (n > p->nq_auto) n = p->nq_auto;
+        p->nq_slab = n;
+        return DEMAG_OK;
+    }
     int n = kx_per_slab == 0 ? p->nkx_auto : kx_per_slab;
     if (n > p->nkx_auto) n = p->nkx_auto;      // the W2 slab was sized for nkx_auto planes
     p->nkx_slab = n;
@@ -321,9 +394,11 @@ demag_status demag_set_slab(demag_plan_t p, int kx_per_slab)
 int demag_launches_per_apply(demag_plan_t p)
 {
     if (!p) return 0;
-    const int nslab = (p->g.hx + p->nkx_slab - 1) / p->nkx_slab;
+    const int nslab = p->v2 ? (p->cf.g.hq + p->nq_slab - 1) / p->nq_slab : (p->g.hx + p->nkx_slab - 1) / p->nkx_slab;
     return 2 + 3 * nslab;
 }
+
+int demag_path(demag_plan_t p) { return p && p->v2 ? 1 : 0; }
 
 }  // extern "C"
 
@@ -411,7 +486,16 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
             // each odd axis contributes a factor i (X = i Im X): two odd axes -> -1.  Eq. (1)'s minus sign and
             // the inverse-transform normalisation 1/(Nx Ny Nz) are folded in here (R3).
             const double scale = (nodd == 2 ? -1.0 : 1.0) * (-1.0) / ((double)g.Nx * g.Ny * g.Nz);
-            if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
+            if (p->v2) {    // pair layout; the real split of the x transform hands over 2 X[k]: fold the 1/2 here
+                const v2::GeoV& gv = p->cf.g;
+                const size_t n = (size_t)gv.hq * g.kpz * g.Ny;
+                const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
+                if (p->prec == DEMAG_FP32)
+                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, p->ypos2freq, par[c][1], 0.5 * scale);
+                else
+                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, p->ypos2freq, par[c][1], 0.5 * scale);
+            }
+            else if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
             else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
             CUDA_TRY(cudaGetLastError());
         }
@@ -453,6 +537,10 @@ struct StageTimer {
 };
 #define STAGE(s, launch) do { if (tm) tm->begin(s); launch; if (tm) tm->end(); } while (0)
 
+template <typename T> const v2::Ctx<T>& v2_ctx(const demag_plan_s* p);
+template <> const v2::Ctx<float>& v2_ctx<float>(const demag_plan_s* p) { return p->cf; }
+template <> const v2::Ctx<double>& v2_ctx<double>(const demag_plan_s* p) { return p->cd; }
+
 template <typename T>
 demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr)
 {
@@ -461,6 +549,22 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
     C* W1 = (C*)p->W1; C* W2 = (C*)p->W2;
     const C* twx = (const C*)p->tw[0]; const C* twy = (const C*)p->tw[1]; const C* twz = (const C*)p->tw[2];
     const size_t nc = (size_t)g.nx * g.ny * g.nz;
+    if (p->v2) {
+        const v2::Ctx<T>& cx = v2_ctx<T>(p);
+        v2::CQ<T>* V1 = (v2::CQ<T>*)p->W1; v2::CQ<T>* V2 = (v2::CQ<T>*)p->W2;
+        const v2::KQ<T>* Kv = (const v2::KQ<T>*)p->K;
+        cudaError_t verr = cudaSuccess;
+        STAGE(0, (v2::x_fwd<T>(1, cx, st, M, V1, &verr)));
+        for (int q0 = 0; q0 < cx.g.hq; q0 += p->nq_slab) {
+            const int nq = std::min(p->nq_slab, cx.g.hq - q0);
+            STAGE(1, (v2::y_fwd<T>(1, cx, st, q0, nq, V1, V2, &verr)));
+            STAGE(2, (v2::z_mul<T>(1, cx, st, q0, nq, V2, Kv, &verr)));
+            STAGE(3, (v2::y_inv<T>(1, cx, st, q0, nq, V2, V1, &verr)));
+        }
+        STAGE(4, (v2::x_inv<T>(1, cx, st, V1, H, &verr)));
+        CUDA_TRY(cudaGetLastError());
+        return DEMAG_OK;
+    }
     if (g.Nx == 1) {
         const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
         STAGE(0, (k_x_copy_fwd<T><<<grid, 256, 0, st>>>(3 * nc, M, W1)));

@@ -1,0 +1,237 @@
+// v2_host.cuh -- host side of the fast path (kernels_v2.cuh): per-size launch configurations, twiddle tables,
+// the plan-time pack of the kernel spectrum into the pair layout, and the launchers demag_apply calls.
+#pragma once
+#include <math.h>
+#include <vector>
+#include "kernels_v2.cuh"
+
+namespace demag {
+namespace v2 {
+
+// ---- launch configurations (compile-time, by log2 transform length) ---------------------------------------
+// x stage (K1v / K5v): radix policy, row pairs per tile, threads
+template <int LLC> struct XCfg { static constexpr int POL = 1, RP = 8, NT = 64; };
+template <> struct XCfg<8>  { static constexpr int POL = 2, RP = 8, NT = 128; };
+template <> struct XCfg<9>  { static constexpr int POL = 1, RP = 8, NT = 256; };
+template <> struct XCfg<10> { static constexpr int POL = 1, RP = 4, NT = 256; };
+template <> struct XCfg<11> { static constexpr int POL = 1, RP = 2, NT = 256; };
+template <> struct XCfg<12> { static constexpr int POL = 1, RP = 1, NT = 256; };
+// y stage (K2v / K4v): radix policy, line pairs per tile, threads
+template <int LNY> struct YCfg { static constexpr int POL = 1, BP = 8, NT = 64; };
+template <> struct YCfg<8>  { static constexpr int POL = 1, BP = 8, NT = 128; };
+template <> struct YCfg<9>  { static constexpr int POL = 1, BP = 8, NT = 256; };
+template <> struct YCfg<10> { static constexpr int POL = 1, BP = 4, NT = 256; };
+template <> struct YCfg<11> { static constexpr int POL = 1, BP = 2, NT = 256; };
+template <> struct YCfg<12> { static constexpr int POL = 1, BP = 1, NT = 256; };
+template <> struct YCfg<13> { static constexpr int POL = 1, BP = 1, NT = 512; };
+// z stage (K3v): radix policy (the LAST pass is the fused one), ky columns per tile, threads, min blocks per SM
+template <int LNZ> struct ZCfg { static constexpr int POL = 1, TY = 16, NT = 64, MINB = 1; };
+template <> struct ZCfg<4>  { static constexpr int POL = 0, TY = 32, NT = 128, MINB = 1; };   // 8 . 2
+template <> struct ZCfg<5>  { static constexpr int POL = 1, TY = 16, NT = 64,  MINB = 1; };   // 4 . 8
+template <> struct ZCfg<6>  { static constexpr int POL = 1, TY = 16, NT = 128, MINB = 1; };   // 8 . 8
+template <> struct ZCfg<7>  { static constexpr int POL = 1, TY = 8,  NT = 128, MINB = 1; };   // 16 . 8
+template <> struct ZCfg<8>  { static constexpr int POL = 1, TY = 4,  NT = 64,  MINB = 1; };   // 4 . 8 . 8
+template <> struct ZCfg<9>  { static constexpr int POL = 1, TY = 4,  NT = 256, MINB = 1; };   // 8 . 8 . 8
+template <> struct ZCfg<10> { static constexpr int POL = 1, TY = 2,  NT = 128, MINB = 1; };   // 16 . 8 . 8
+template <> struct ZCfg<11> { static constexpr int POL = 1, TY = 1,  NT = 64,  MINB = 1; };   // 4 . 8 . 8 . 8
+
+constexpr int kXMin = 4, kXMax = 12, kYMin = 4, kYMax = 13, kZMin = 2, kZMax = 11;
+
+inline int x_rp(int lLc)
+{
+    switch (lLc) { case 10: return XCfg<10>::RP; case 11: return XCfg<11>::RP; case 12: return XCfg<12>::RP; default: return 8; }
+}
+inline int x_pol(int lLc) { return lLc == 8 ? XCfg<8>::POL : 1; }
+inline int y_pol(int) { return 1; }
+inline int z_pol(int lNz) { return lNz == 4 ? ZCfg<4>::POL : 1; }
+inline int z_ty(int lNz)
+{
+    switch (lNz) {
+    case 2: case 3: return 1;
+    case 4: return ZCfg<4>::TY; case 5: return ZCfg<5>::TY; case 6: return ZCfg<6>::TY; case 7: return ZCfg<7>::TY;
+    case 8: return ZCfg<8>::TY; case 9: return ZCfg<9>::TY; case 10: return ZCfg<10>::TY; case 11: return ZCfg<11>::TY;
+    default: return 1 << 30;
+    }
+}
+
+// Can the fast path run this geometry?  (all axes zero padded, sizes inside the instantiated range, tiles divide)
+inline bool supported(int nx, int ny, int nz, int Nx, int Ny, int Nz, int lLc, int lNy, int lNz, size_t esz, int max_smem)
+{
+    if (Nx != 2 * nx || Ny != 2 * ny || Nz != 2 * nz) return false;
+    if (lLc < kXMin || lLc > kXMax || lNy < kYMin || lNy > kYMax || lNz < kZMin || lNz > kZMax) return false;
+    if (ny % (2 * x_rp(lLc)) != 0) return false;
+    if (lNz >= 4 && Ny % z_ty(lNz) != 0) return false;
+    if (lNz < 4 && Ny < 32) return false;
+    // shared memory of the y tile (the largest): Ny * (BP|1) quads
+    const int bp = lNy <= 9 ? 8 : lNy == 10 ? 4 : lNy == 11 ? 2 : 1;
+    if ((size_t)Ny * (bp | 1) * 4 * esz > (size_t)max_smem) return false;
+    if ((size_t)nx * (x_rp(lLc) | 1) * 4 * esz > (size_t)max_smem) return false;
+    if ((size_t)Nz * 3 * z_ty(lNz) * 4 * esz > (size_t)max_smem && lNz >= 4) return false;
+    return true;
+}
+
+// ---- twiddle tables ------------------------------------------------------------------------------------
+// pass j of schedule (LL, POL): entries [(m-1) S + lo] = exp(-2 pi i lo m / (R S)), m = 1..R-1, lo = 0..S-1, stored as
+// quads {wr, wr, wi, wi}.  All passes of one axis live in one device buffer.
+template <typename T>
+struct AxisTables {
+    void* dev = nullptr;
+    size_t bytes = 0;
+    TwSet<T> set;
+};
+template <typename T>
+cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>* out, const CQ<T>** post)
+{
+    const Sched sc = make_sched(LL, POL);
+    std::vector<T> h;
+    size_t off[6] = {0, 0, 0, 0, 0, 0};
+    bool has[6] = {false, false, false, false, false, false};
+    const long double tp = 6.283185307179586476925286766559005768L;
+    for (int j = 0; j < sc.n; ++j) {
+        const int R = 1 << sc.lr[j], S = 1 << sc.ls[j];
+        if (S == 1) continue;
+        has[j] = true; off[j] = h.size();
+        for (int m = 1; m < R; ++m)
+            for (int lo = 0; lo < S; ++lo) {
+                const long double a = tp * (long double)lo * (long double)m / ((long double)R * (long double)S);
+                const T wr = (T)cosl(a), wi = (T)(-sinl(a));
+                h.push_back(wr); h.push_back(wr); h.push_back(wi); h.push_back(wi);
+            }
+    }
+    size_t post_off = h.size();
+    if (extra_post_Lc > 0) {     // w^k = exp(-2 pi i k / (2 Lc)), k = 0..Lc/2 (the real-transform split)
+        for (int k = 0; k <= extra_post_Lc / 2; ++k) {
+            const long double a = tp * (long double)k / (2.0L * (long double)extra_post_Lc);
+            T wr = (T)cosl(a), wi = (T)(-sinl(a));
+            if (2 * k == extra_post_Lc) { wr = 0; wi = -1; }
+            h.push_back(wr); h.push_back(wr); h.push_back(wi); h.push_back(wi);
+        }
+    }
+    if (h.empty()) h.resize(4, (T)0);
+    out->bytes = h.size() * sizeof(T);
+    cudaError_t e = cudaMalloc(&out->dev, out->bytes);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpy(out->dev, h.data(), out->bytes, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e;
+    for (int j = 0; j < 6; ++j) out->set.p[j] = has[j] ? reinterpret_cast<const CQ<T>*>((const T*)out->dev + off[j]) : nullptr;
+    if (post) *post = extra_post_Lc > 0 ? reinterpret_cast<const CQ<T>*>((const T*)out->dev + post_off) : nullptr;
+    return cudaSuccess;
+}
+
+// ---- plan-time pack of the transformed tensor into the pair layout -----------------------------------------
+// A = real 3D transform of one component, [kz'][ky'][kx] (kx = 0..Lc).  Kv[q][kz'][py] component comp, lines (q, Lc-q).
+// ypos2freq[py] = y frequency stored at W2v position py (the y schedule's digit reversal).
+template <typename T>
+__global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv, int comp, int Lc, int hq, int kpy, int kpz,
+                                int Ny, const int* __restrict__ ypos2freq, int par_y, double scale)
+{
+    const size_t n = (size_t)hq * kpz * Ny;
+    const int hx = Lc + 1;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int py = (int)(i % Ny), kz = (int)((i / Ny) % kpz), q = (int)(i / ((size_t)Ny * kpz));
+        const int ky = ypos2freq[py];
+        const bool my = 2 * ky > Ny;
+        const int kyp = my ? Ny - ky : ky;
+        const double sg = (my && par_y < 0) ? -1.0 : 1.0;
+        const double* row = A + ((size_t)kz * kpy + kyp) * hx;
+        Kv[i * 12 + comp * 2 + 0] = (T)(sg * scale * row[q]);
+        Kv[i * 12 + comp * 2 + 1] = (T)(sg * scale * row[Lc - q]);
+    }
+}
+
+// ---- launchers ---------------------------------------------------------------------------------------------
+template <typename T> struct Ctx {
+    GeoV g;
+    int lLc, lNy, lNz;
+    TwSet<T> twx, twy, twz;
+    const CQ<T>* twpost;
+};
+
+#define V2_CASE_X(L, KERN, ...)                                                                                     \
+    case L: {                                                                                                        \
+        using C = XCfg<L>;                                                                                           \
+        constexpr int smem = (1 << L) * (C::RP | 1) * (int)sizeof(CQ<T>);                                            \
+        if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::RP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+        else KERN<T, L, C::POL, C::RP, C::NT><<<3u * c.g.nz * (c.g.ny / (2 * C::RP)), C::NT, smem, st>>>(__VA_ARGS__); \
+        return true;                                                                                                 \
+    }
+
+// mode 0: set the shared-memory attribute (plan time); mode 1: launch
+template <typename T>
+bool x_fwd(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cudaError_t* err)
+{
+    switch (c.lLc) {
+        V2_CASE_X(4, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
+        V2_CASE_X(6, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
+        V2_CASE_X(8, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
+        V2_CASE_X(10, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
+        V2_CASE_X(12, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
+    default: return false;
+    }
+}
+template <typename T>
+bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cudaError_t* err)
+{
+    switch (c.lLc) {
+        V2_CASE_X(4, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(5, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
+        V2_CASE_X(6, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(7, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
+        V2_CASE_X(8, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(9, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
+        V2_CASE_X(10, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(11, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
+        V2_CASE_X(12, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
+    default: return false;
+    }
+}
+
+#define V2_CASE_Y(L, KERN, A, B) case L: V2_BODY_Y(L, KERN, A, B)
+#define V2_BODY_Y(L, KERN, A, B)                                                                                    \
+    {                                                                                                                \
+        using C = YCfg<L>;                                                                                           \
+        constexpr int smem = (1 << L) * (C::BP | 1) * (int)sizeof(CQ<T>);                                            \
+        if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::BP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+        else KERN<T, L, C::POL, C::BP, C::NT><<<(unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st>>>(c.g, q0, nq, A, B, c.twy); \
+        return true;                                                                                                 \
+    }
+template <typename T>
+bool y_fwd(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W1, CQ<T>* W2, cudaError_t* err)
+{
+    switch (c.lNy) {
+        V2_CASE_Y(4, k_y_fwd_v, W1, W2) V2_CASE_Y(5, k_y_fwd_v, W1, W2) V2_CASE_Y(6, k_y_fwd_v, W1, W2) V2_CASE_Y(7, k_y_fwd_v, W1, W2)
+        V2_CASE_Y(8, k_y_fwd_v, W1, W2) V2_CASE_Y(9, k_y_fwd_v, W1, W2) V2_CASE_Y(10, k_y_fwd_v, W1, W2) V2_CASE_Y(11, k_y_fwd_v, W1, W2)
+        V2_CASE_Y(12, k_y_fwd_v, W1, W2)
+    case 13: if constexpr (sizeof(T) == 4) V2_BODY_Y(13, k_y_fwd_v, W1, W2) else return false;
+    default: return false;
+    }
+}
+template <typename T>
+bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W2, CQ<T>* W1, cudaError_t* err)
+{
+    switch (c.lNy) {
+        V2_CASE_Y(4, k_y_inv_v, W2, W1) V2_CASE_Y(5, k_y_inv_v, W2, W1) V2_CASE_Y(6, k_y_inv_v, W2, W1) V2_CASE_Y(7, k_y_inv_v, W2, W1)
+        V2_CASE_Y(8, k_y_inv_v, W2, W1) V2_CASE_Y(9, k_y_inv_v, W2, W1) V2_CASE_Y(10, k_y_inv_v, W2, W1) V2_CASE_Y(11, k_y_inv_v, W2, W1)
+        V2_CASE_Y(12, k_y_inv_v, W2, W1)
+    case 13: if constexpr (sizeof(T) == 4) V2_BODY_Y(13, k_y_inv_v, W2, W1) else return false;
+    default: return false;
+    }
+}
+
+#define V2_CASE_Z(L)                                                                                                \
+    case L: {                                                                                                        \
+        using C = ZCfg<L>;                                                                                           \
+        constexpr int smem = (1 << L) * 3 * C::TY * (int)sizeof(CQ<T>);                                              \
+        if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+        else k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB><<<(unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st>>>(c.g, q0, nq, W2, K, c.twz); \
+        return true;                                                                                                 \
+    }
+template <typename T>
+bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2, const KQ<T>* K, cudaError_t* err)
+{
+    switch (c.lNz) {
+    case 2: if (mode) k_z1_v<T, 2><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
+    case 3: if (mode) k_z1_v<T, 3><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
+        V2_CASE_Z(4) V2_CASE_Z(5) V2_CASE_Z(6) V2_CASE_Z(7) V2_CASE_Z(8) V2_CASE_Z(9) V2_CASE_Z(10) V2_CASE_Z(11)
+    default: return false;
+    }
+}
+
+}  // namespace v2
+}  // namespace demag

@@ -1,0 +1,124 @@
+"""Parity of the compile-time specialised kernel family (kernels_v2.cuh, demag_path() == 1) against the fp64
+oracle, one case per instantiated transform length of every stage, plus agreement with the size-generic family.
+
+Tolerances as everywhere (BASELINE.json north_star): 2e-5 (fp32) / 1e-11 (fp64) of Ms, the oracle's tensor
+pushed through demag_set_kernel.
+"""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL32 = 2e-5
+TOL64 = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2308_08447_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _run(torch, B, n, h, T, M, prec, expect_path=None, slab=0):
+    dt = torch.float32 if prec == 0 else torch.float64
+    with B.Plan(n, h, 0, prec) as p:
+        if expect_path is not None:
+            assert p.path() == expect_path, f"plan for {n} took kernel family {p.path()}"
+        p.set_kernel(T)
+        if slab:
+            p.set_slab(slab)
+        Md = torch.from_numpy(np.ascontiguousarray(M)).to("cuda", dt)
+        Hd = torch.full_like(Md, float("nan"))
+        p.apply(Md, Hd)
+        torch.cuda.synchronize()
+        assert not torch.isnan(Hd).any()
+        return Hd.cpu().numpy().astype(np.float64)
+
+
+def _reference(oracle, n, h, M):
+    """Full field: Eq. (1) by direct summation when small, else the NumPy-FFT cross-check O-C, itself checked
+    against Eq. (1) at sampled cells."""
+    from paper_2308_08447_b200 import workloads as W
+    T = oracle.tensor_table(n, h)
+    M64 = M.astype(np.float64)
+    if np.prod(n) <= 4096:
+        return T, oracle.direct_sum(T, M64)
+    ref = oracle.fft_conv(T, M64)
+    cells = W.sample_cells(n, 48, 7)
+    Hs = oracle.direct_sum_sampled(T, M64, cells)
+    assert np.abs(ref.reshape(3, -1)[:, cells].T - Hs).max() / 8e5 < 1e-12
+    return T, ref
+
+
+# one shape per x length (Lc = nx = 16 .. 4096), per y length (Ny = 32 .. 8192), per z length (Nz = 4 .. 2048);
+# the other two axes small but spanning several tiles / a ragged last tile where the stage allows it
+X_SHAPES = [(16, 16, 2), (32, 16, 4), (64, 32, 2), (128, 16, 2), (256, 48 // 3 * 2, 2), (512, 16, 2), (1024, 16, 2),
+            (2048, 16, 2), (4096, 16, 2)]
+Y_SHAPES = [(16, 16, 4), (16, 32, 2), (32, 64, 2), (16, 128, 2), (16, 256, 4), (16, 512, 2), (16, 1024, 2),
+            (16, 2048, 2), (16, 4096, 2)]
+Z_SHAPES = [(16, 16, 2), (16, 16, 4), (16, 16, 8), (16, 16, 16), (16, 32, 32), (16, 16, 64), (16, 16, 128),
+            (16, 16, 256), (16, 16, 512), (16, 16, 1024)]
+SHAPES = sorted(set(X_SHAPES + Y_SHAPES + Z_SHAPES + [(64, 64, 8), (32, 48 // 3 * 2, 16), (256, 64, 16)]))
+
+
+@pytest.mark.parametrize("n", SHAPES)
+@pytest.mark.parametrize("prec", [0, 1])
+def test_fast_family_against_oracle(torch, B, oracle, n, prec):
+    from paper_2308_08447_b200 import workloads as W
+    if prec == 1 and 2 * n[1] > 4096:
+        pytest.skip("fp64 fast path stops at Ny = 4096 (shared memory)")
+    h = (2e-9, 3e-9, 1.5e-9)
+    Ms = 8e5
+    M = W.random_unit_vectors(n, Ms, 300 + sum(n))
+    T, ref = _reference(oracle, n, h, M)
+    H = _run(torch, B, n, h, T, M, prec, expect_path=1)
+    err = np.abs(H - ref).max() / Ms
+    assert err <= (TOL32 if prec == 0 else TOL64), err
+
+
+@pytest.mark.parametrize("n", [(64, 32, 4), (128, 64, 16), (32, 16, 64)])
+def test_fast_and_generic_families_agree(torch, B, oracle, n, monkeypatch):
+    from paper_2308_08447_b200 import workloads as W
+    h = (2e-9, 2e-9, 2e-9)
+    Ms = 8e5
+    M = W.random_unit_vectors(n, Ms, 11)
+    T = oracle.tensor_table(n, h)
+    Hf = _run(torch, B, n, h, T, M, 1, expect_path=1)
+    monkeypatch.setenv("DEMAG_PATH", "generic")
+    Hg = _run(torch, B, n, h, T, M, 1, expect_path=0)
+    monkeypatch.delenv("DEMAG_PATH")
+    assert np.abs(Hf - Hg).max() / Ms <= 1e-12
+
+
+@pytest.mark.parametrize("slab", [1, 2, 5])
+def test_fast_family_slab_size_does_not_change_result(torch, B, oracle, slab):
+    from paper_2308_08447_b200 import workloads as W
+    n, h = (32, 16, 8), (2e-9, 2e-9, 2e-9)
+    M = W.random_unit_vectors(n, 8e5, 5)
+    T = oracle.tensor_table(n, h)
+    H0 = _run(torch, B, n, h, T, M, 0, expect_path=1)
+    H1 = _run(torch, B, n, h, T, M, 0, expect_path=1, slab=slab)
+    assert np.array_equal(H0, H1)
+
+
+def test_fast_family_impulse_returns_tensor_column(torch, B, oracle):
+    """A single magnetised cell reads the stored kernel back through the whole pipeline: H_a(i) = -N_ab(i-j) M_b."""
+    n, h = (32, 16, 8), (2e-9, 3e-9, 1e-9)
+    T = oracle.tensor_table(n, h)
+    for (jx, jy, jz), comp in [((0, 0, 0), 0), ((31, 15, 7), 1), ((13, 6, 2), 2)]:
+        M = np.zeros((3,) + n[::-1], dtype=np.float32)
+        M[comp, jz, jy, jx] = 1.0
+        ref = oracle.direct_sum(T, M.astype(np.float64))
+        H = _run(torch, B, n, h, T, M, 1, expect_path=1)
+        assert np.abs(H - ref).max() <= 1e-13
