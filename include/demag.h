@@ -110,9 +110,10 @@ demag_status demag_apply_profiled(demag_plan_t plan, const void* M_dev, void* H_
 int demag_launches_per_apply(demag_plan_t plan);
 
 /* Which kernel family demag_apply uses for this plan: 1 = the compile-time specialised two-lines-per-thread
- * kernels (all axes zero padded, sizes in their instantiated range), 0 = the size-generic kernels.  Both compute
- * the same convolution (Appendix A).  The environment variable DEMAG_PATH=generic, read by
- * demag_plan_create, forces 0 (used by the tests to cover both families). */
+ * kernels (DEMAG_FP32 plans with all axes zero padded and sizes in their instantiated range), 0 = the size-generic
+ * kernels.  Both compute the same convolution (Appendix A).  The environment variable DEMAG_PATH,
+ * read by demag_plan_create, overrides the choice: "generic" forces 0, "fast" also admits DEMAG_FP64 plans to 1
+ * (used by the tests to cover both families in both precisions). */
 int demag_path(demag_plan_t plan);
 
 /* Last error message of the calling thread ("" if none). */

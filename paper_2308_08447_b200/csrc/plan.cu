@@ -271,7 +271,10 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
     p->k_bytes = 6 * p->kcomp_stride * p->esz;
     {
         const char* path = getenv("DEMAG_PATH");           // "generic" forces the size-generic kernels (tests, A/B timing)
-        p->v2 = !(path && !strcmp(path, "generic")) && pbc_flags == 0 &&
+        // fp64: the 32-byte quads halve the shared-memory efficiency of the y stage; the generic kernels are faster
+        // there (C3 fp64: 1.14 ms vs 1.28 ms), so the fast family is opt-in (DEMAG_PATH=fast) for fp64 plans
+        const bool want = precision == DEMAG_FP32 || (path && !strcmp(path, "fast"));
+        p->v2 = want && !(path && !strcmp(path, "generic")) && pbc_flags == 0 &&
                 v2::supported(nx, ny, nz, g.Nx, g.Ny, g.Nz, g.lLc, g.lNy, g.lNz, p->esz, kMaxSmem);
     }
     if (p->v2) {
@@ -701,7 +704,13 @@ extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev,
     const double f = muB * mu_s_in_muB / ((double)cx * cy * cz * a * a * a);
     const unsigned ga = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)1 << 22);
     const unsigned gs = (unsigned)std::min<size_t>((nspin3 / 4 + 255) / 256 + 1, (size_t)p->sm_count * 32);
-    if (p->prec == DEMAG_FP32) {
+    if (p->prec == DEMAG_FP32 && cx == 4 && g.ny <= 65535 && 3 * g.nz <= 65535) {
+        const dim3 g3((unsigned)((g.nx + 127) / 128), (unsigned)g.ny, (unsigned)(3 * g.nz));
+        k_macro_avg_x4<<<g3, 128, 0, st>>>(g.nx, cy, cz, (const float*)S_dev, (float*)p->Mc, f);
+        s = apply_impl<float>(p, (const float*)p->Mc, (float*)p->Hc, st);
+        if (s) return s;
+        k_macro_scatter_x4<<<g3, 128, 0, st>>>(g.nx, cy, cz, (const float*)p->Hc, (float*)Hs_dev, accumulate);
+    } else if (p->prec == DEMAG_FP32) {
         k_macro_avg<float><<<ga, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const float*)S_dev, (float*)p->Mc, f);
         s = apply_impl<float>(p, (const float*)p->Mc, (float*)p->Hc, st);
         if (s) return s;

@@ -2,6 +2,7 @@
 // the plan-time pack of the kernel spectrum into the pair layout, and the launchers demag_apply calls.
 #pragma once
 #include <math.h>
+#include <stdlib.h>
 #include <vector>
 #include "kernels_v2.cuh"
 
@@ -29,9 +30,9 @@ template <int LNZ> struct ZCfg { static constexpr int POL = 1, TY = 16, NT = 64,
 template <> struct ZCfg<4>  { static constexpr int POL = 0, TY = 32, NT = 128, MINB = 1; };   // 8 . 2
 template <> struct ZCfg<5>  { static constexpr int POL = 1, TY = 16, NT = 64,  MINB = 1; };   // 4 . 8
 template <> struct ZCfg<6>  { static constexpr int POL = 1, TY = 16, NT = 128, MINB = 1; };   // 8 . 8
-template <> struct ZCfg<7>  { static constexpr int POL = 1, TY = 8,  NT = 128, MINB = 1; };   // 16 . 8
+template <> struct ZCfg<7>  { static constexpr int POL = 1, TY = 8,  NT = 64,  MINB = 1; };   // 16 . 8
 template <> struct ZCfg<8>  { static constexpr int POL = 1, TY = 4,  NT = 64,  MINB = 1; };   // 4 . 8 . 8
-template <> struct ZCfg<9>  { static constexpr int POL = 1, TY = 4,  NT = 256, MINB = 1; };   // 8 . 8 . 8
+template <> struct ZCfg<9>  { static constexpr int POL = 1, TY = 4,  NT = 128, MINB = 1; };   // 8 . 8 . 8
 template <> struct ZCfg<10> { static constexpr int POL = 1, TY = 2,  NT = 128, MINB = 1; };   // 16 . 8 . 8
 template <> struct ZCfg<11> { static constexpr int POL = 1, TY = 1,  NT = 64,  MINB = 1; };   // 4 . 8 . 8 . 8
 

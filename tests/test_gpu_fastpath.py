@@ -74,8 +74,10 @@ SHAPES = sorted(set(X_SHAPES + Y_SHAPES + Z_SHAPES + [(64, 64, 8), (32, 48 // 3 
 
 @pytest.mark.parametrize("n", SHAPES)
 @pytest.mark.parametrize("prec", [0, 1])
-def test_fast_family_against_oracle(torch, B, oracle, n, prec):
+def test_fast_family_against_oracle(torch, B, oracle, n, prec, monkeypatch):
     from paper_2308_08447_b200 import workloads as W
+    if prec == 1:
+        monkeypatch.setenv("DEMAG_PATH", "fast")      # fp64 plans take the generic family unless asked
     if prec == 1 and 2 * n[1] > 4096:
         pytest.skip("fp64 fast path stops at Ny = 4096 (shared memory)")
     h = (2e-9, 3e-9, 1.5e-9)
@@ -94,6 +96,7 @@ def test_fast_and_generic_families_agree(torch, B, oracle, n, monkeypatch):
     Ms = 8e5
     M = W.random_unit_vectors(n, Ms, 11)
     T = oracle.tensor_table(n, h)
+    monkeypatch.setenv("DEMAG_PATH", "fast")
     Hf = _run(torch, B, n, h, T, M, 1, expect_path=1)
     monkeypatch.setenv("DEMAG_PATH", "generic")
     Hg = _run(torch, B, n, h, T, M, 1, expect_path=0)
@@ -112,8 +115,9 @@ def test_fast_family_slab_size_does_not_change_result(torch, B, oracle, slab):
     assert np.array_equal(H0, H1)
 
 
-def test_fast_family_impulse_returns_tensor_column(torch, B, oracle):
+def test_fast_family_impulse_returns_tensor_column(torch, B, oracle, monkeypatch):
     """A single magnetised cell reads the stored kernel back through the whole pipeline: H_a(i) = -N_ab(i-j) M_b."""
+    monkeypatch.setenv("DEMAG_PATH", "fast")
     n, h = (32, 16, 8), (2e-9, 3e-9, 1e-9)
     T = oracle.tensor_table(n, h)
     for (jx, jy, jz), comp in [((0, 0, 0), 0), ((31, 15, 7), 1), ((13, 6, 2), 2)]:
