@@ -38,6 +38,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3", help="C1..C5, suffix d = fp64 (e.g. C3d)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
 
@@ -144,6 +145,23 @@ class ClockSampler:
         return out
 
 
+# ----------------------------------------------------------------------------------------------- multi-rank plumbing
+def allreduce_max(vals, device, world):
+    """Max over ranks of a list of floats (device times): the timing rule of the bench contract.  The path does not
+    shard without an exchange (replicas only), so this is the ONLY collective of a run."""
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor(list(vals), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return tt.tolist()
+
+
+def aggregate_throughput(world, units_per_rank, steps, ms_total_max):
+    """Whole-job units/s of `world` independent replicas that each did `steps` steps of `units_per_rank` units."""
+    return world * units_per_rank * steps / (ms_total_max * 1e-3)
+
+
 # ----------------------------------------------------------------------------------------------- our arm
 def stage_bytes(n, esz):
     """Algorithmic HBM bytes of each stage of the 5-pass separable structure (T2):
@@ -159,6 +177,61 @@ def stage_bytes(n, esz):
 
 
 STAGE_NAMES = ["k_x_r2c", "k_y_fwd", "k_z_mul", "k_y_inv", "k_x_c2r"]
+
+
+def cufft_baseline(torch, n, dt, dev, reps=10):
+    """cuFFT-based convolution on the same GPU (torch.fft), timing only (random real kernel spectrum): the comparator
+    north_star names; never on the product path.  (i) naive: materialise the padded field, rfftn, multiply, irfftn,
+    crop; (ii) pruned: per-axis transforms with the padding given as n= and slicing between axes (the paper's
+    single-GPU scheme).  Returns ms of each (median over `reps`)."""
+    nx, ny, nz = n
+    P = [v if v == 1 else 2 * v for v in n]
+    Nx, Ny, Nz = P
+    hx = Nx // 2 + 1
+    cdt = torch.complex64 if dt == torch.float32 else torch.complex128
+    need = (3 * Nz * Ny * hx * (8 if dt == torch.float32 else 16)) * 3 + 6 * Nz * Ny * hx * (4 if dt == torch.float32 else 8)
+    free, _ = torch.cuda.mem_get_info()
+    if need > 0.6 * free:
+        return None
+    M = torch.randn((3, nz, ny, nx), dtype=dt, device=dev)
+    K = torch.randn((6, Nz, Ny, hx), dtype=dt, device=dev)
+
+    def mult(Z):
+        zx, zy, zz = Z[0], Z[1], Z[2]
+        return torch.stack((K[0] * zx + K[3] * zy + K[4] * zz, K[3] * zx + K[1] * zy + K[5] * zz,
+                            K[4] * zx + K[5] * zy + K[2] * zz))
+
+    def naive():
+        Mp = torch.zeros((3, Nz, Ny, Nx), dtype=dt, device=dev)
+        Mp[:, :nz, :ny, :nx] = M
+        Z = torch.fft.rfftn(Mp, dim=(-3, -2, -1))
+        return torch.fft.irfftn(mult(Z), s=(Nz, Ny, Nx), dim=(-3, -2, -1))[:, :nz, :ny, :nx]
+
+    def pruned():
+        X = torch.fft.rfft(M, n=Nx, dim=-1) if Nx > 1 else M.to(cdt)
+        Y = torch.fft.fft(X, n=Ny, dim=-2) if Ny > 1 else X
+        Z = torch.fft.fft(Y, n=Nz, dim=-3) if Nz > 1 else Y
+        Hh = mult(Z)
+        Hh = torch.fft.ifft(Hh, dim=-3)[:, :nz] if Nz > 1 else Hh
+        Hh = torch.fft.ifft(Hh, dim=-2)[:, :, :ny] if Ny > 1 else Hh
+        return torch.fft.irfft(Hh, n=Nx, dim=-1)[..., :nx] if Nx > 1 else Hh.real
+
+    out = {}
+    for name, fn in (("naive", naive), ("pruned", pruned)):
+        try:
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(reps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record(); torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            out[name + "_ms"] = statistics.median(ts)
+        except torch.cuda.OutOfMemoryError:
+            out[name + "_ms"] = None
+        torch.cuda.empty_cache()
+    return out
 
 
 def run_ours(args, cfg, fp64):
@@ -285,11 +358,12 @@ def run_ours(args, cfg, fp64):
     st_ms /= reps
     launches_per_step = plan.launches_per_apply() + (2 if atom else 0)
 
+    cufft = None
+    if rank == 0 and not atom and not args.no_cufft:
+        cufft = cufft_baseline(torch, n, dt, dev)
+
     # ---- reduce over ranks: max time
-    tt = torch.tensor([ms_total, ms_hot, t_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms_total, ms_hot, t_e2e = tt.tolist()
+    ms_total, ms_hot, t_e2e = allreduce_max([ms_total, ms_hot, t_e2e], dev, world)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -304,7 +378,7 @@ def run_ours(args, cfg, fp64):
     sb = stage_bytes(n, esz)
     dom = int(np.argmax(st_ms))
     achieved = sb[dom] / (st_ms[dom] * 1e-3) / 1e9
-    value = world * nc * args.steps / (ms_total * 1e-3) / 1e9
+    value = aggregate_throughput(world, nc, args.steps, ms_total) / 1e9
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -312,7 +386,8 @@ def run_ours(args, cfg, fp64):
         "config": {"workload": workload_name(cfg, fp64), "mesh": list(n), "cells": nc, "padded": [v if v == 1 else 2 * v for v in n],
                    "l2": "flushed between timed steps (256 MB write outside each step's event pair)",
                    "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-                   "kernel": "built-in Newell tensor (demag_set_kernel(NULL))"},
+                   "kernel": "built-in Newell tensor (demag_set_kernel(NULL))",
+                   "kernel_family": "fast (kernels_v2.cuh)" if plan.path() == 1 else "generic (kernels.cuh)"},
         "conv_per_s": world * args.steps / (ms_total * 1e-3),
         "hot_ms_per_step": ms_hot, "hot_value": world * nc / (ms_hot * 1e-3) / 1e9,
         "e2e": {"value": world * nc * args.steps / t_e2e / 1e9, "unit": UNIT,
@@ -330,6 +405,11 @@ def run_ours(args, cfg, fp64):
                               "frac_of_peak": sum(sb) / (ms_total / args.steps) / 1e6 / peak},
         "plan_build_s": t_plan, "input_gen_s": t_inputs, "workspace_bytes": plan.workspace_bytes(),
     }
+    if cufft:
+        best = min(v for v in cufft.values() if v)
+        cufft.update(best_ms=best, ours_over_cufft=best / (ms_total / args.steps),
+                     note="torch.fft (cuFFT) convolution of the same shape on the same GPU, L2 not flushed, timing only")
+        line["cufft"] = cufft
     if atom:
         line["spins_per_s_G"] = world * units * args.steps / (ms_total * 1e-3) / 1e9
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
