@@ -7,9 +7,10 @@
 //                               the real transform produces / consumes together (hq = Lc/2 + 1, Lc = Nx/2 = nx)
 //   W2v [3][nq][nz][Ny] quads   slab of nq pairs; y in the digit-reversed "position order" the forward passes
 //                               leave behind (the stored kernel spectrum uses the same order: nothing is permuted)
-//   Kv  [hq][Nz/2+1][Ny] KQ     the six real components for the two frequencies of the pair, z packed by symmetry
-//                               (PAPER.md:255-256), the y parity sign, -1/(Nx Ny Nz) and the 1/2 of the real
-//                               split folded in at plan time
+//   Kv  [hq][Ny/KT][Nz/2+1][chunk][KT]  the six real components for the two frequencies of the pair, z packed by
+//                               symmetry, the y parity sign, -1/(Nx Ny Nz) and the 1/2 of the
+//                               real split folded in at plan time; tiled by KT consecutive py (the z kernel's
+//                               tile) and split into 16-byte chunks so that a warp's load is contiguous
 //
 // Every kernel is templated on log2 of its transform length, its tile and its block size, so that every
 // shared-memory offset is an immediate; twiddles come from per-pass tables (dup format, [m-1][lo]).
@@ -283,21 +284,23 @@ __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ
 
 // =========================================================================================== K3v: z stage
 // z FFT . kernel multiplication . z IFFT "in the same routine" (PAPER.md:343; :316-326 zFFT, KernelMultiplication).
-template <typename T> __device__ __forceinline__ KQ<T> ldk(const KQ<T>* p);
-template <> __device__ __forceinline__ KQ<float> ldk<float>(const KQ<float>* p)
+// One (q, kz', py) entry is NCH chunks of 16 bytes, chunk j of column ty at p[j * KT]:
+// fp32: 3 chunks {xx0,xx1,yy0,yy1} {zz0,zz1,xy0,xy1} {xz0,xz1,yz0,yz1};  fp64: 6 chunks, one component pair each.
+template <typename T> struct kchunks;
+template <> struct kchunks<float>  { static constexpr int N = 3; using V = float4; };
+template <> struct kchunks<double> { static constexpr int N = 6; using V = double2; };
+template <int KT> __device__ __forceinline__ KQ<float> ldk(const float4* p)
 {
-    const float4* q = reinterpret_cast<const float4*>(p);
-    const float4 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2);
+    const float4 a = __ldg(p), b = __ldg(p + KT), c = __ldg(p + 2 * KT);
     KQ<float> k;
     k.xx = make_float2(a.x, a.y); k.yy = make_float2(a.z, a.w); k.zz = make_float2(b.x, b.y);
     k.xy = make_float2(b.z, b.w); k.xz = make_float2(c.x, c.y); k.yz = make_float2(c.z, c.w);
     return k;
 }
-template <> __device__ __forceinline__ KQ<double> ldk<double>(const KQ<double>* p)
+template <int KT> __device__ __forceinline__ KQ<double> ldk(const double2* p)
 {
-    const double2* q = reinterpret_cast<const double2*>(p);
     KQ<double> k;
-    k.xx = __ldg(q); k.yy = __ldg(q + 1); k.zz = __ldg(q + 2); k.xy = __ldg(q + 3); k.xz = __ldg(q + 4); k.yz = __ldg(q + 5);
+    k.xx = __ldg(p); k.yy = __ldg(p + KT); k.zz = __ldg(p + 2 * KT); k.xy = __ldg(p + 3 * KT); k.xz = __ldg(p + 4 * KT); k.yz = __ldg(p + 5 * KT);
     return k;
 }
 // H^_a = sum_b K^_ab M^_b, K^ real and symmetric.  SGN: sign of the z-odd components xz, yz
@@ -318,31 +321,34 @@ __device__ __forceinline__ void apply_kernel(const KQ<T>& k, CQ<T>& mx, CQ<T>& m
     mx = hx; my = hy; mz = hz;
 }
 
-// multiply the RF points of one fused butterfly (positions p0..p0+RF-1 <-> kz = f0 + m Nz/RF)
-template <typename T, int LNZ, int LRF, int M> struct MulPoints {
-    static __device__ __forceinline__ void run(CQ<T> (*a)[1 << LRF], const KQ<T>* __restrict__ Kcol, int Ny, int f0)
+// multiply the RF points of one fused butterfly (positions p0..p0+RF-1 <-> kz = f0 + m Nz/RF); Kcol = this column's
+// first chunk at kz' = 0, rows kz' are kchunks<T>::N * KT vectors apart
+template <typename T, int LNZ, int LRF, int KT, int M> struct MulPoints {
+    using KV = typename kchunks<T>::V;
+    static __device__ __forceinline__ void run(CQ<T> (*a)[1 << LRF], const KV* __restrict__ Kcol, int f0)
     {
-        constexpr int NZ = 1 << LNZ, RF = 1 << LRF, W = NZ >> LRF;
+        constexpr int NZ = 1 << LNZ, RF = 1 << LRF, W = NZ >> LRF, ROW = kchunks<T>::N * KT;
         const int kz = f0 + M * W;
         if (RF == 1 || 2 * M < RF) {
-            apply_kernel<1>(ldk(Kcol + (size_t)kz * Ny), a[0][M], a[1][M], a[2][M], (T)1);
+            apply_kernel<1>(ldk<KT>(Kcol + kz * ROW), a[0][M], a[1][M], a[2][M], (T)1);
         } else if (2 * M > RF) {
-            apply_kernel<-1>(ldk(Kcol + (size_t)(NZ - kz) * Ny), a[0][M], a[1][M], a[2][M], (T)1);
+            apply_kernel<-1>(ldk<KT>(Kcol + (NZ - kz) * ROW), a[0][M], a[1][M], a[2][M], (T)1);
         } else {
             const bool mir = f0 > 0;
-            apply_kernel<0>(ldk(Kcol + (size_t)(mir ? NZ - kz : kz) * Ny), a[0][M], a[1][M], a[2][M], mir ? (T)-1 : (T)1);
+            apply_kernel<0>(ldk<KT>(Kcol + (mir ? NZ - kz : kz) * ROW), a[0][M], a[1][M], a[2][M], mir ? (T)-1 : (T)1);
         }
-        MulPoints<T, LNZ, LRF, M + 1>::run(a, Kcol, Ny, f0);
+        MulPoints<T, LNZ, LRF, KT, M + 1>::run(a, Kcol, f0);
     }
 };
-template <typename T, int LNZ, int LRF> struct MulPoints<T, LNZ, LRF, (1 << LRF)> {
-    static __device__ __forceinline__ void run(CQ<T> (*)[1 << LRF], const KQ<T>* __restrict__, int, int) {}
+template <typename T, int LNZ, int LRF, int KT> struct MulPoints<T, LNZ, LRF, KT, (1 << LRF)> {
+    using KV = typename kchunks<T>::V;
+    static __device__ __forceinline__ void run(CQ<T> (*)[1 << LRF], const KV* __restrict__, int) {}
 };
 
 // Nz >= 16 (at least two passes).  Tile = one pair plane ql x TY consecutive py x all z x 3 components:
 // shared s[Nz][3 TY] quads, lines fastest everywhere (a warp's accesses are consecutive quads: conflict free).
 template <typename T, int LNZ, int POL, int TY, int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const KQ<T>* __restrict__ K, TwSet<T> tw)
+__global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K, TwSet<T> tw)
 {
     constexpr int NZ = 1 << LNZ, B = 3 * TY;
     constexpr Sched SC = make_sched(LNZ, POL);
@@ -362,7 +368,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     FwdPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
     {   // fused: last forward pass . multiply . first inverse pass; item = (butterfly i, column ty), 3 components
         constexpr int NBF = NZ >> LRF, TOT = NBF * TY, ITER = (TOT + NT - 1) / NT;
-        const KQ<T>* Kq = K + (size_t)(q0 + ql) * g.kpz * Ny + py0;
+        const typename kchunks<T>::V* Kq = K + ((size_t)(q0 + ql) * tilesY + pyt) * g.kpz * (kchunks<T>::N * TY);   // KT == TY
 #pragma unroll 1
         for (int k = 0; k < ITER; ++k) {
             const int t = tid + k * NT;
@@ -377,7 +383,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
                 dftR<LRF, false, false>(a[cc]);
             }
             const int f0 = freq_of_pos_rt<LNZ, POL>(p0);
-            MulPoints<T, LNZ, LRF, 0>::run(a, Kq + ty, Ny, f0);
+            MulPoints<T, LNZ, LRF, TY, 0>::run(a, Kq + ty, f0);
 #pragma unroll
             for (int cc = 0; cc < 3; ++cc) {
                 dftR<LRF, true, false>(a[cc]);
@@ -395,7 +401,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
 // Nz <= 8: the whole z transform of a column is one butterfly per component in registers; no shared memory.
 // grid = nq * Ny / 128 (or fewer columns per block if Ny < 128), block = min(Ny, 128).
 template <typename T, int LNZ>
-__global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2, const KQ<T>* __restrict__ K)
+__global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K)
 {
     constexpr int RF = 1 << LNZ;
     const int cols = blockDim.x;
@@ -412,7 +418,7 @@ __global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2,
         for (int m = 0; m < (RF > 1 ? RF / 2 : 1); ++m) a[cc][m] = ldq(col + cc * cstride + (size_t)m * Ny);
         dftR<LNZ, false, true>(a[cc]);
     }
-    MulPoints<T, LNZ, LNZ, 0>::run(a, K + (size_t)(q0 + ql) * g.kpz * Ny + py, Ny, 0);
+    MulPoints<T, LNZ, LNZ, 32, 0>::run(a, K + ((size_t)(q0 + ql) * (Ny / 32) + py / 32) * g.kpz * (kchunks<T>::N * 32) + (py & 31), 0);   // KT = 32
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc) {
         dftR<LNZ, true, false>(a[cc]);

@@ -494,9 +494,9 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
                 const size_t n = (size_t)gv.hq * g.kpz * g.Ny;
                 const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
                 if (p->prec == DEMAG_FP32)
-                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, p->ypos2freq, par[c][1], 0.5 * scale);
+                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale);
                 else
-                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, p->ypos2freq, par[c][1], 0.5 * scale);
+                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale);
             }
             else if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
             else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
@@ -555,7 +555,7 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
     if (p->v2) {
         const v2::Ctx<T>& cx = v2_ctx<T>(p);
         v2::CQ<T>* V1 = (v2::CQ<T>*)p->W1; v2::CQ<T>* V2 = (v2::CQ<T>*)p->W2;
-        const v2::KQ<T>* Kv = (const v2::KQ<T>*)p->K;
+        const typename v2::kchunks<T>::V* Kv = (const typename v2::kchunks<T>::V*)p->K;
         cudaError_t verr = cudaSuccess;
         STAGE(0, (v2::x_fwd<T>(1, cx, st, M, V1, &verr)));
         for (int q0 = 0; q0 < cx.g.hq; q0 += p->nq_slab) {

@@ -120,14 +120,18 @@ cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>*
 }
 
 // ---- plan-time pack of the transformed tensor into the pair layout -----------------------------------------
-// A = real 3D transform of one component, [kz'][ky'][kx] (kx = 0..Lc).  Kv[q][kz'][py] component comp, lines (q, Lc-q).
-// ypos2freq[py] = y frequency stored at W2v position py (the y schedule's digit reversal).
+// A = real 3D transform of one component, [kz'][ky'][kx] (kx = 0..Lc).  Kv[q][py / KT][kz'][chunk][py % KT], lines
+// (q, Lc-q) (kernels_v2.cuh "kchunks").  ypos2freq[py] = y frequency stored at W2v position py (the y schedule's
+// digit reversal).  KT = the z kernel's tile width (z_kt()).
+inline int z_kt(int lNz) { return lNz >= 4 ? z_ty(lNz) : 32; }
 template <typename T>
 __global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv, int comp, int Lc, int hq, int kpy, int kpz,
-                                int Ny, const int* __restrict__ ypos2freq, int par_y, double scale)
+                                int Ny, int KT, const int* __restrict__ ypos2freq, int par_y, double scale)
 {
     const size_t n = (size_t)hq * kpz * Ny;
     const int hx = Lc + 1;
+    constexpr int U = 16 / (int)sizeof(T), NCH = 12 / U;          // values per 16-byte chunk, chunks per entry
+    const int j = sizeof(T) == 4 ? comp / 2 : comp, off = sizeof(T) == 4 ? (comp % 2) * 2 : 0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const int py = (int)(i % Ny), kz = (int)((i / Ny) % kpz), q = (int)(i / ((size_t)Ny * kpz));
         const int ky = ypos2freq[py];
@@ -135,8 +139,10 @@ __global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv
         const int kyp = my ? Ny - ky : ky;
         const double sg = (my && par_y < 0) ? -1.0 : 1.0;
         const double* row = A + ((size_t)kz * kpy + kyp) * hx;
-        Kv[i * 12 + comp * 2 + 0] = (T)(sg * scale * row[q]);
-        Kv[i * 12 + comp * 2 + 1] = (T)(sg * scale * row[Lc - q]);
+        const size_t tile_row = ((size_t)q * (Ny / KT) + py / KT) * kpz + kz;
+        T* d = Kv + ((tile_row * NCH + j) * KT + py % KT) * U + off;
+        d[0] = (T)(sg * scale * row[q]);
+        d[1] = (T)(sg * scale * row[Lc - q]);
     }
 }
 
@@ -224,7 +230,7 @@ bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<
         return true;                                                                                                 \
     }
 template <typename T>
-bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2, const KQ<T>* K, cudaError_t* err)
+bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* K, cudaError_t* err)
 {
     switch (c.lNz) {
     case 2: if (mode) k_z1_v<T, 2><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
