@@ -48,7 +48,7 @@ inline int z_pol(int lNz) { return lNz == 4 ? ZCfg<4>::POL : 1; }
 inline int z_ty(int lNz)
 {
     switch (lNz) {
-    case 2: case 3: return 1;
+    case 0: case 2: case 3: return 1;
     case 4: return ZCfg<4>::TY; case 5: return ZCfg<5>::TY; case 6: return ZCfg<6>::TY; case 7: return ZCfg<7>::TY;
     case 8: return ZCfg<8>::TY; case 9: return ZCfg<9>::TY; case 10: return ZCfg<10>::TY; case 11: return ZCfg<11>::TY;
     default: return 1 << 30;
@@ -58,8 +58,9 @@ inline int z_ty(int lNz)
 // Can the fast path run this geometry?  (all axes zero padded, sizes inside the instantiated range, tiles divide)
 inline bool supported(int nx, int ny, int nz, int Nx, int Ny, int Nz, int lLc, int lNy, int lNz, size_t esz, int max_smem)
 {
-    if (Nx != 2 * nx || Ny != 2 * ny || Nz != 2 * nz) return false;
-    if (lLc < kXMin || lLc > kXMax || lNy < kYMin || lNy > kYMax || lNz < kZMin || lNz > kZMax) return false;
+    const bool film = nz == 1 && Nz == 1;          // a one-cell-thick mesh has no z transform (R6): multiply only
+    if (Nx != 2 * nx || Ny != 2 * ny || (Nz != 2 * nz && !film)) return false;
+    if (lLc < kXMin || lLc > kXMax || lNy < kYMin || lNy > kYMax || ((lNz < kZMin || lNz > kZMax) && !film)) return false;
     if (ny % (2 * x_rp(lLc)) != 0) return false;
     if (lNz >= 4 && Ny % z_ty(lNz) != 0) return false;
     if (lNz < 4 && Ny < 32) return false;
@@ -233,6 +234,7 @@ template <typename T>
 bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* K, cudaError_t* err)
 {
     switch (c.lNz) {
+    case 0: if (mode) k_z1_v<T, 0><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
     case 2: if (mode) k_z1_v<T, 2><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
     case 3: if (mode) k_z1_v<T, 3><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
         V2_CASE_Z(4) V2_CASE_Z(5) V2_CASE_Z(6) V2_CASE_Z(7) V2_CASE_Z(8) V2_CASE_Z(9) V2_CASE_Z(10) V2_CASE_Z(11)

@@ -69,7 +69,8 @@ Y_SHAPES = [(16, 16, 4), (16, 32, 2), (32, 64, 2), (16, 128, 2), (16, 256, 4), (
             (16, 2048, 2), (16, 4096, 2)]
 Z_SHAPES = [(16, 16, 2), (16, 16, 4), (16, 16, 8), (16, 16, 16), (16, 32, 32), (16, 16, 64), (16, 16, 128),
             (16, 16, 256), (16, 16, 512), (16, 16, 1024)]
-SHAPES = sorted(set(X_SHAPES + Y_SHAPES + Z_SHAPES + [(64, 64, 8), (32, 48 // 3 * 2, 16), (256, 64, 16)]))
+FILM_SHAPES = [(16, 16, 1), (64, 128, 1), (256, 32, 1)]          # nz = 1: no z transform, multiply only (row a3')
+SHAPES = sorted(set(X_SHAPES + Y_SHAPES + Z_SHAPES + FILM_SHAPES + [(64, 64, 8), (32, 48 // 3 * 2, 16), (256, 64, 16)]))
 
 
 @pytest.mark.parametrize("n", SHAPES)
