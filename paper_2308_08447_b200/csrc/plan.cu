@@ -40,7 +40,9 @@ demag_status fail(demag_status st, const char* fmt, ...)
     } while (0)
 
 constexpr int kMaxSmem = 232448 - 1024;   // 227 KB opt-in shared memory per CTA (sm_100) minus room for static __shared__
-constexpr size_t kSlabBytes = 128u << 20;  // target size of the L2-resident W2 slab (L2 is ~126 MB)
+constexpr size_t kSlabBytes = (size_t)16 << 30;   // cap of the W2 workspace: larger meshes run the y/z stages slab by slab.
+                                                  // (Measured on B200: the kernels are not DRAM bound, an L2-sized slab only adds launches and
+                                                  //  partial waves -- C3 426 us at 128 MB vs 401 us unslabbed -- so the cap is a memory cap.)
 
 inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 inline int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
@@ -214,7 +216,7 @@ void configure(demag_plan_s* p)
     {
         const size_t per_kx = (size_t)3 * g.nz * g.Ny * csz;
         size_t slab_bytes = kSlabBytes;
-        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoi(e) << 20;   // tuning override
+        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoll(e) << 20;   // tuning override
         long long n = (long long)(slab_bytes / per_kx);
         if (n < 1) n = 1;
         if (n > g.hx) n = g.hx;
@@ -285,7 +287,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         const size_t qsz = 4 * p->esz;                      // one quad
         const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;
         size_t slab_bytes = kSlabBytes;
-        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoi(e) << 20;
+        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoll(e) << 20;
         long long n = (long long)(slab_bytes / per_q);
         if (n < 1) n = 1;
         if (n > gv.hq) n = gv.hq;
