@@ -10,8 +10,11 @@
  * x R2C FFT -> y FFT -> z FFT -> multiply with the transformed tensor -> inverse z, y -> x C2R.
  *
  * Conventions (readings R3, R6, R8):
- *   - mesh of nx*ny*nz cuboid cells of size hx*hy*hz metres; every n_a is a power of two, n_a <= 4096;
- *   - an axis is zero-padded to N_a = 2 n_a unless n_a == 1 or its PBC flag is set (then N_a = n_a);
+ *   - mesh of nx*ny*nz cuboid cells of size hx*hy*hz metres, 1 <= n_a <= 4096;
+ *   - an axis is zero-padded to N_a = 2 m_a, m_a = the next power of two >= n_a (an exact linear convolution needs
+ *     N_a >= 2 n_a - 1), unless n_a == 1 or its PBC flag is set (then N_a = n_a, and a periodic
+ *     n_a must itself be a power of two).  A mesh whose sizes are not all powers of two is embedded, with zeros,
+ *     in the m_x*m_y*m_z mesh inside the plan (two extra copies per apply, same result);
  *   - M, H: planar device arrays [3][nz][ny][nx], x fastest, components x,y,z, in A/m,
  *     float (DEMAG_FP32) or double (DEMAG_FP64), 16-byte aligned, not aliased;
  *   - tensor component order: xx, yy, zz, xy, xz, yz; N is dimensionless;
@@ -39,7 +42,7 @@ typedef struct demag_plan_s* demag_plan_t;            /* opaque; owned by the li
 typedef enum {
     DEMAG_OK = 0,
     DEMAG_ERR_INVALID_ARG = 1,   /* NULL / misaligned / aliased pointer, non-positive size          */
-    DEMAG_ERR_UNSUPPORTED = 2,   /* size not a power of two or > 4096, built-in tensor with PBC ...  */
+    DEMAG_ERR_UNSUPPORTED = 2,   /* size > 4096, periodic size not a power of two, built-in tensor + PBC */
     DEMAG_ERR_ALLOC = 3,         /* cudaMalloc / malloc failed                                       */
     DEMAG_ERR_CUDA = 4,          /* a CUDA runtime call or launch failed (see demag_last_error)      */
     DEMAG_ERR_NO_KERNEL = 5      /* demag_apply before demag_set_kernel                              */

@@ -47,6 +47,7 @@ constexpr size_t kSlabBytes = (size_t)16 << 30;   // cap of the W2 workspace: la
 inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 inline int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
 inline int pow2_floor(long long v) { int p = 1; while (2LL * p <= v) p *= 2; return p; }
+inline int pow2_ceil(int v) { int p = 1; while (p < v) p *= 2; return p; }
 
 }  // namespace
 
@@ -77,6 +78,10 @@ struct demag_plan_s {
     v2::Ctx<float> cf; v2::Ctx<double> cd;
     v2::AxisTables<float> tf[3]; v2::AxisTables<double> td[3];
     int* ypos2freq = nullptr;
+    // general mesh sizes: the caller's mesh on[] is embedded (zeros) in the power-of-two mesh g.n* the transforms run on
+    int on[3] = {0, 0, 0};
+    bool embed = false;
+    void* Mp = nullptr; void* Hp = nullptr;
 };
 
 namespace {
@@ -242,12 +247,18 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         return fail(DEMAG_ERR_INVALID_ARG, "cell sizes must be positive and finite");
     if (precision != DEMAG_FP32 && precision != DEMAG_FP64) return fail(DEMAG_ERR_INVALID_ARG, "bad precision");
     if (pbc_flags & ~7u) return fail(DEMAG_ERR_INVALID_ARG, "bad pbc_flags");
-    if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz))
-        return fail(DEMAG_ERR_UNSUPPORTED, "mesh sizes must be powers of two (got %d x %d x %d)", nx, ny, nz);
     if (nx > 4096 || ny > 4096 || nz > 4096) return fail(DEMAG_ERR_UNSUPPORTED, "mesh sizes must be <= 4096");
+    if (((pbc_flags & DEMAG_PBC_X) && !is_pow2(nx)) || ((pbc_flags & DEMAG_PBC_Y) && !is_pow2(ny)) ||
+        ((pbc_flags & DEMAG_PBC_Z) && !is_pow2(nz)))
+        return fail(DEMAG_ERR_UNSUPPORTED, "a periodic axis cannot be padded: its size must be a power of two (got %d x %d x %d)", nx, ny, nz);
 
     demag_plan_s* p = new (std::nothrow) demag_plan_s();
     if (!p) return fail(DEMAG_ERR_ALLOC, "out of host memory");
+    // General sizes (R10): the transforms need power-of-two lengths N_a >= 2 n_a - 1 for an exact linear
+    // convolution, so the mesh is embedded, with zeros, in the mesh of the next powers of two.
+    p->on[0] = nx; p->on[1] = ny; p->on[2] = nz;
+    nx = pow2_ceil(nx); ny = pow2_ceil(ny); nz = pow2_ceil(nz);
+    p->embed = nx != p->on[0] || ny != p->on[1] || nz != p->on[2];
     Geo& g = p->g;
     g.nx = nx; g.ny = ny; g.nz = nz;
     g.Nx = (nx == 1 || (pbc_flags & DEMAG_PBC_X)) ? nx : 2 * nx;
@@ -344,6 +355,12 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
                 p->tw_bytes += sizeof(int) * (size_t)g.Ny;
             }
         }
+        if (p->embed) {
+            const size_t b = (size_t)3 * nx * ny * nz * p->esz;
+            CUDA_TRY(cudaMalloc(&p->Mp, b));
+            CUDA_TRY(cudaMalloc(&p->Hp, b));
+            p->macro_bytes += 2 * b;
+        }
         CUDA_TRY(cudaMalloc(&p->W1, p->w1_bytes));
         CUDA_TRY(cudaMalloc(&p->W2, p->w2_bytes));
         CUDA_TRY(cudaMalloc(&p->K, p->k_bytes));
@@ -367,7 +384,7 @@ demag_status demag_plan_destroy(demag_plan_t p)
     if (!p) return DEMAG_OK;
     cudaFree(p->W1); cudaFree(p->W2); cudaFree(p->K);
     for (int a = 0; a < 3; ++a) cudaFree(p->tw[a]);
-    cudaFree(p->Mc); cudaFree(p->Hc);
+    cudaFree(p->Mc); cudaFree(p->Hc); cudaFree(p->Mp); cudaFree(p->Hp);
     for (int a = 0; a < 3; ++a) { cudaFree(p->tf[a].dev); cudaFree(p->td[a].dev); }
     cudaFree(p->ypos2freq);
     delete p;
@@ -400,7 +417,7 @@ int demag_launches_per_apply(demag_plan_t p)
 {
     if (!p) return 0;
     const int nslab = p->v2 ? (p->cf.g.hq + p->nq_slab - 1) / p->nq_slab : (p->g.hx + p->nkx_slab - 1) / p->nkx_slab;
-    return 2 + 3 * nslab;
+    return 2 + 3 * nslab + (p->embed ? 2 : 0);
 }
 
 int demag_path(demag_plan_t p) { return p && p->v2 ? 1 : 0; }
@@ -474,7 +491,18 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
         for (int a = 0; a < 3; ++a) { demag_status s = make_twiddles<double2>(N[a], (void**)&tw64[a], &dummy); if (s) return s; }
         for (int c = 0; c < 6; ++c) {
             const double* src;
-            if (N6_host) { CUDA_TRY(cudaMemcpy(A, N6_host + c * nc, nc * sizeof(double), cudaMemcpyHostToDevice)); src = A; }
+            if (N6_host && !p->embed) { CUDA_TRY(cudaMemcpy(A, N6_host + c * nc, nc * sizeof(double), cudaMemcpyHostToDevice)); src = A; }
+            else if (N6_host) {   // caller's table covers offsets 0 <= d_a < on[a]; larger offsets never meet a cell: zero
+                const size_t onc = (size_t)p->on[0] * p->on[1] * p->on[2];
+                CUDA_TRY(cudaMemset(A, 0, nc * sizeof(double)));
+                cudaMemcpy3DParms cp = {};
+                cp.srcPtr = make_cudaPitchedPtr((void*)(N6_host + c * onc), p->on[0] * sizeof(double), p->on[0], p->on[1]);
+                cp.dstPtr = make_cudaPitchedPtr(A, g.nx * sizeof(double), g.nx, g.ny);
+                cp.extent = make_cudaExtent(p->on[0] * sizeof(double), p->on[1], p->on[2]);
+                cp.kind = cudaMemcpyHostToDevice;
+                CUDA_TRY(cudaMemcpy3D(&cp));
+                src = A;
+            }
             else src = Tdev + c * nc;
             demag_status s;
             // x: rows (z,y); y: lines (z; kx); z: lines (ky,kx)
@@ -523,7 +551,19 @@ extern "C" demag_status demag_get_kernel_real(demag_plan_t p, double* N6_host)
     demag_status st = build_table_dev(p, &T);
     if (st) return st;
     const size_t nc = (size_t)p->g.nx * p->g.ny * p->g.nz;
-    cudaError_t e = cudaMemcpy(N6_host, T, 6 * nc * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaError_t e = cudaSuccess;
+    if (!p->embed) e = cudaMemcpy(N6_host, T, 6 * nc * sizeof(double), cudaMemcpyDeviceToHost);
+    else {
+        const size_t onc = (size_t)p->on[0] * p->on[1] * p->on[2];
+        for (int c = 0; c < 6 && e == cudaSuccess; ++c) {
+            cudaMemcpy3DParms cp = {};
+            cp.srcPtr = make_cudaPitchedPtr(T + c * nc, p->g.nx * sizeof(double), p->g.nx, p->g.ny);
+            cp.dstPtr = make_cudaPitchedPtr(N6_host + c * onc, p->on[0] * sizeof(double), p->on[0], p->on[1]);
+            cp.extent = make_cudaExtent(p->on[0] * sizeof(double), p->on[1], p->on[2]);
+            cp.kind = cudaMemcpyDeviceToHost;
+            e = cudaMemcpy3D(&cp);
+        }
+    }
     cudaFree(T);
     if (e != cudaSuccess) return fail(DEMAG_ERR_CUDA, "copy back: %s", cudaGetErrorString(e));
     return DEMAG_OK;
@@ -608,6 +648,40 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
     return DEMAG_OK;
 }
 
+// caller's mesh <-> embedding power-of-two mesh (only for plans with embed == true)
+template <typename T>
+__global__ void __launch_bounds__(256) k_embed(int onx, int ony, int onz, int nx, int ny, int nz, const T* __restrict__ M, T* __restrict__ Mp)
+{
+    const int y = blockIdx.y, cz = blockIdx.z, c = cz / nz, z = cz - c * nz;
+    const bool in = y < ony && z < onz;
+    const T* src = M + (((size_t)c * onz + z) * ony + y) * onx;
+    T* dst = Mp + (((size_t)c * nz + z) * ny + y) * nx;
+    for (int x = blockIdx.x * 256 + threadIdx.x; x < nx; x += gridDim.x * 256) dst[x] = (in && x < onx) ? src[x] : (T)0;
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_crop(int onx, int ony, int onz, int nx, int ny, int nz, const T* __restrict__ Hp, T* __restrict__ H)
+{
+    const int y = blockIdx.y, cz = blockIdx.z, c = cz / onz, z = cz - c * onz;
+    const T* src = Hp + (((size_t)c * nz + z) * ny + y) * nx;
+    T* dst = H + (((size_t)c * onz + z) * ony + y) * onx;
+    for (int x = blockIdx.x * 256 + threadIdx.x; x < onx; x += gridDim.x * 256) dst[x] = src[x];
+}
+// demag_apply on the caller's mesh
+template <typename T>
+demag_status apply_outer(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr)
+{
+    if (!p->embed) return apply_impl<T>(p, M, H, st, tm);
+    const Geo& g = p->g;
+    k_embed<T><<<dim3((unsigned)((g.nx + 255) / 256), (unsigned)g.ny, (unsigned)(3 * g.nz)), 256, 0, st>>>(
+        p->on[0], p->on[1], p->on[2], g.nx, g.ny, g.nz, M, (T*)p->Mp);
+    demag_status s = apply_impl<T>(p, (const T*)p->Mp, (T*)p->Hp, st, tm);
+    if (s) return s;
+    k_crop<T><<<dim3((unsigned)((p->on[0] + 255) / 256), (unsigned)p->on[1], (unsigned)(3 * p->on[2])), 256, 0, st>>>(
+        p->on[0], p->on[1], p->on[2], g.nx, g.ny, g.nz, (const T*)p->Hp, H);
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}
+
 demag_status check_apply_args(demag_plan_s* p, const void* a, const void* b, size_t bytes)
 {
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
@@ -624,13 +698,13 @@ extern "C" demag_status demag_apply(demag_plan_t p, const void* M_dev, void* H_d
 {
     g_err[0] = 0;
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
-    const size_t bytes = (size_t)3 * p->g.nx * p->g.ny * p->g.nz * p->esz;
+    const size_t bytes = (size_t)3 * p->on[0] * p->on[1] * p->on[2] * p->esz;
     demag_status s = check_apply_args(p, M_dev, H_dev, bytes);
     if (s) return s;
     if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    return p->prec == DEMAG_FP32 ? apply_impl<float>(p, (const float*)M_dev, (float*)H_dev, st)
-                                 : apply_impl<double>(p, (const double*)M_dev, (double*)H_dev, st);
+    return p->prec == DEMAG_FP32 ? apply_outer<float>(p, (const float*)M_dev, (float*)H_dev, st)
+                                 : apply_outer<double>(p, (const double*)M_dev, (double*)H_dev, st);
 }
 
 extern "C" demag_status demag_apply_profiled(demag_plan_t p, const void* M_dev, void* H_dev, void* cuda_stream,
@@ -638,14 +712,14 @@ extern "C" demag_status demag_apply_profiled(demag_plan_t p, const void* M_dev, 
 {
     g_err[0] = 0;
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
-    const size_t bytes = (size_t)3 * p->g.nx * p->g.ny * p->g.nz * p->esz;
+    const size_t bytes = (size_t)3 * p->on[0] * p->on[1] * p->on[2] * p->esz;
     demag_status s = check_apply_args(p, M_dev, H_dev, bytes);
     if (s) return s;
     if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
     StageTimer tm;
     tm.st = (cudaStream_t)cuda_stream;
-    s = p->prec == DEMAG_FP32 ? apply_impl<float>(p, (const float*)M_dev, (float*)H_dev, tm.st, &tm)
-                              : apply_impl<double>(p, (const double*)M_dev, (double*)H_dev, tm.st, &tm);
+    s = p->prec == DEMAG_FP32 ? apply_outer<float>(p, (const float*)M_dev, (float*)H_dev, tm.st, &tm)
+                              : apply_outer<double>(p, (const double*)M_dev, (double*)H_dev, tm.st, &tm);
     cudaError_t e = cudaStreamSynchronize(tm.st);
     float ms[5] = {0, 0, 0, 0, 0};
     int cnt[5] = {0, 0, 0, 0, 0};
@@ -668,7 +742,7 @@ extern "C" demag_status demag_energy(demag_plan_t p, const void* M_dev, const vo
     if (!p || !M_dev || !H_dev || !E_dev) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
     if ((uintptr_t)E_dev & 7) return fail(DEMAG_ERR_INVALID_ARG, "E_dev must be 8-byte aligned");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t n3 = (size_t)3 * p->g.nx * p->g.ny * p->g.nz;
+    const size_t n3 = (size_t)3 * p->on[0] * p->on[1] * p->on[2];
     const double mu0 = 4.0e-7 * 3.14159265358979323846;
     const double scale = -0.5 * mu0 * p->h[0] * p->h[1] * p->h[2];
     CUDA_TRY(cudaMemsetAsync(E_dev, 0, sizeof(double), st));
@@ -686,7 +760,7 @@ extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev,
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
     if (cx < 1 || cy < 1 || cz < 1 || !(a > 0) || !isfinite(mu_s_in_muB))
         return fail(DEMAG_ERR_INVALID_ARG, "bad macrocell / lattice arguments");
-    const Geo& g = p->g;
+    struct { int nx, ny, nz; } g = {p->on[0], p->on[1], p->on[2]};     // the caller's macrocell mesh
     const double want[3] = {cx * a, cy * a, cz * a};
     for (int i = 0; i < 3; ++i)
         if (fabs(want[i] - p->h[i]) > 1e-9 * p->h[i])
@@ -699,7 +773,7 @@ extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev,
     if (!p->Mc) {   // first atomistic call on this plan: allocate the two macrocell buffers (documented)
         CUDA_TRY(cudaMalloc(&p->Mc, 3 * nc * p->esz));
         CUDA_TRY(cudaMalloc(&p->Hc, 3 * nc * p->esz));
-        p->macro_bytes = 6 * nc * p->esz;
+        p->macro_bytes += 6 * nc * p->esz;
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const double muB = 9.2740100783e-24;
@@ -709,17 +783,17 @@ extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev,
     if (p->prec == DEMAG_FP32 && cx == 4 && g.ny <= 65535 && 3 * g.nz <= 65535) {
         const dim3 g3((unsigned)((g.nx + 127) / 128), (unsigned)g.ny, (unsigned)(3 * g.nz));
         k_macro_avg_x4<<<g3, 128, 0, st>>>(g.nx, cy, cz, (const float*)S_dev, (float*)p->Mc, f);
-        s = apply_impl<float>(p, (const float*)p->Mc, (float*)p->Hc, st);
+        s = apply_outer<float>(p, (const float*)p->Mc, (float*)p->Hc, st);
         if (s) return s;
         k_macro_scatter_x4<<<g3, 128, 0, st>>>(g.nx, cy, cz, (const float*)p->Hc, (float*)Hs_dev, accumulate);
     } else if (p->prec == DEMAG_FP32) {
         k_macro_avg<float><<<ga, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const float*)S_dev, (float*)p->Mc, f);
-        s = apply_impl<float>(p, (const float*)p->Mc, (float*)p->Hc, st);
+        s = apply_outer<float>(p, (const float*)p->Mc, (float*)p->Hc, st);
         if (s) return s;
         k_macro_scatter<float><<<gs, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const float*)p->Hc, (float*)Hs_dev, accumulate);
     } else {
         k_macro_avg<double><<<ga, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const double*)S_dev, (double*)p->Mc, f);
-        s = apply_impl<double>(p, (const double*)p->Mc, (double*)p->Hc, st);
+        s = apply_outer<double>(p, (const double*)p->Mc, (double*)p->Hc, st);
         if (s) return s;
         k_macro_scatter<double><<<gs, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const double*)p->Hc, (double*)Hs_dev, accumulate);
     }

@@ -122,6 +122,56 @@ def test_linearity(torch, B, oracle):
     assert np.abs(H3 - (2.0 * H1 - 3.0 * H2)).max() < 1e-12
 
 
+# --------------------------------------------------------------------------------- general mesh sizes
+GENERAL = [(12, 10, 3), (7, 1, 1), (1, 9, 5), (48, 48, 1), (33, 17, 9), (100, 36, 5), (65, 16, 2)]
+
+
+@pytest.mark.parametrize("n", GENERAL)
+@pytest.mark.parametrize("prec", [0, 1])
+def test_general_mesh_sizes(torch, B, oracle, n, prec):
+    """DESIGN.md R10: sizes that are not powers of two (the paper's own meshes) are embedded in the
+    next power-of-two mesh; the result is the same Eq. (1) sum (padding >= 2n - 1 is exact)."""
+    h = (2e-9, 3e-9, 1e-9)
+    Ms = 8e5
+    M = rand_M(n, Ms, 500 + sum(n))
+    T = oracle.tensor_table(n, h)
+    ref = oracle.direct_sum(T, M.astype(np.float64)) if np.prod(n) <= 6000 else oracle.fft_conv(T, M.astype(np.float64))
+    H = run_gpu(torch, B, n, h, T, M, prec)
+    assert np.abs(H - ref).max() / Ms <= (TOL32 if prec == 0 else TOL64)
+    Hb = run_gpu(torch, B, n, h, None, M, prec, builtin=True)      # built-in tensor on the embedding mesh
+    assert np.abs(Hb - ref).max() / Ms <= (TOL32 if prec == 0 else 1e-9)
+
+
+def test_general_mesh_builder_table_energy_atomistic(torch, B, oracle):
+    n, h, Ms = (12, 10, 3), (2e-9, 3e-9, 1e-9), 8e5
+    with B.Plan(n, h, 0, B.DEMAG_FP64) as p:
+        assert np.abs(p.get_kernel_real() - oracle.tensor_table(n, h)).max() <= 1e-10
+        M = rand_M(n, Ms, 9).astype(np.float64)
+        T = oracle.tensor_table(n, h)
+        p.set_kernel(T)
+        Md = torch.from_numpy(M).cuda(); Hd = torch.empty_like(Md)
+        E = torch.zeros(1, dtype=torch.float64, device="cuda")
+        p.apply(Md, Hd); p.energy(Md, Hd, E); torch.cuda.synchronize()
+        ref = oracle.direct_sum(T, M)
+        Eref = oracle.energy(M, ref, h)
+        assert abs(E.item() - Eref) <= 1e-10 * abs(Eref)
+    # atomistic on a lattice whose macrocell mesh is 6 x 4 x 2
+    from paper_2308_08447_b200 import workloads as W
+    c, a, mu_s = (2, 2, 2), 0.3e-9, 2.0
+    L = (12, 8, 4)
+    S = W.random_spins_numpy(L, 77).astype(np.float64)
+    nm, hm = (6, 4, 2), tuple(ci * a for ci in c)
+    Tm = oracle.tensor_table(nm, hm)
+    Mref = oracle.macrocell_average(S, c, mu_s, a)
+    Href = oracle.macrocell_scatter(oracle.direct_sum(Tm, Mref), c)
+    with B.Plan(nm, hm, 0, B.DEMAG_FP64) as p:
+        p.set_kernel(Tm)
+        Sd = torch.from_numpy(S).cuda(); Hs = torch.empty_like(Sd)
+        p.apply_atomistic(Sd, Hs, c, mu_s, a)
+        torch.cuda.synchronize()
+        assert np.abs(Hs.cpu().numpy() - Href).max() / np.abs(Mref).max() <= 1e-11
+
+
 # --------------------------------------------------------------------------------- tensor builder
 @pytest.mark.parametrize("n,h", [((64, 32, 4), (2e-9, 2e-9, 1e-9)), ((128, 128, 1), (2e-9, 2e-9, 1e-9)),
                                  ((32, 32, 32), (3e-9, 3e-9, 3e-9)), ((256, 8, 2), (1e-9, 1.5e-9, 0.5e-9))])
@@ -214,8 +264,8 @@ def test_error_paths(torch, B):
         B.demag_plan_create(0, 4, 4, 1e-9, 1e-9, 1e-9)
     assert e.value.status == 1
     with pytest.raises(B.DemagError) as e:
-        B.demag_plan_create(12, 4, 4, 1e-9, 1e-9, 1e-9)
-    assert e.value.status == 2
+        B.demag_plan_create(12, 4, 4, 1e-9, 1e-9, 1e-9, B.DEMAG_PBC_X)
+    assert e.value.status == 2                          # a periodic axis cannot be padded
     with pytest.raises(B.DemagError) as e:
         B.demag_plan_create(8192, 4, 4, 1e-9, 1e-9, 1e-9)
     assert e.value.status == 2
