@@ -17,6 +17,7 @@
 #pragma once
 #include "soa_core.cuh"
 
+
 namespace demag {
 namespace v2 {
 
@@ -65,6 +66,22 @@ __device__ __forceinline__ CQ<double> ldgq(const CQ<double>* p)
 {
     const double2* q = reinterpret_cast<const double2*>(p);
     CQ<double> r; r.re = __ldg(q); r.im = __ldg(q + 1); return r;
+}
+
+// streaming global access of the field / workspace data (read once, written once per kernel): do not allocate in L1,
+// which is left to the twiddle tables and the kernel spectrum
+__device__ __forceinline__ CQ<float> ldsq(const CQ<float>* p)
+{
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    CQ<float> r; r.re = make_float2(v.x, v.y); r.im = make_float2(v.z, v.w); return r;
+}
+__device__ __forceinline__ CQ<double> ldsq(const CQ<double>* p)
+{
+    CQ<double> r;
+    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(r.re.x), "=d"(r.re.y) : "l"(p));
+    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(r.im.x), "=d"(r.im.y) : "l"(reinterpret_cast<const double2*>(p) + 1));
+    return r;
 }
 
 // twiddles of one butterfly: w^(lo m), m = 1..R-1, from the pass table [m-1][lo]
@@ -243,7 +260,7 @@ __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ
     const int l0 = blockIdx.x * BP;
     if (tid < BP) loff[tid] = (l0 + tid < nlines) ? w1v_line_offset(g, l0 + tid, q0, nq) : -1;
     __syncthreads();
-    auto ld = [&](int b, int p) { const long long o = loff[b]; return o >= 0 ? ldgq(W1 + o + p) : cq_zero<T>(); };
+    auto ld = [&](int b, int p) { const long long o = loff[b]; return o >= 0 ? ldsq(W1 + o + p) : cq_zero<T>(); };
     pass_first<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, ld);
     __syncthreads();
     FwdPasses<T, LNY, POL, 1, SC.n, BP, PITCH, NT>::run(s, tw, tid);
@@ -274,7 +291,7 @@ __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ
 #pragma unroll 4
     for (int idx = tid; idx < (BP << LNY); idx += NT) {
         const int b = idx >> LNY, p = idx & (NY - 1);
-        stq(s + p * PITCH + b, b < nvalid ? ldgq(src + idx) : cq_zero<T>());
+        stq(s + p * PITCH + b, b < nvalid ? ldsq(src + idx) : cq_zero<T>());
     }
     __syncthreads();
     InvPasses<T, LNY, POL, 1, SC.n, BP, PITCH, NT>::run(s, tw, tid);
@@ -362,7 +379,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     const size_t cstride = (size_t)nq * g.nz * g.Ny;
     CQ<T>* base = W2 + (size_t)ql * g.nz * g.Ny + py0;
     const int Ny = g.Ny;
-    auto ld = [&](int b, int z) { const int c = b / TY, ty = b - c * TY; return ldq(base + c * cstride + (size_t)z * Ny + ty); };
+    auto ld = [&](int b, int z) { const int c = b / TY, ty = b - c * TY; return ldsq(base + c * cstride + (size_t)z * Ny + ty); };
     pass_first<T, LNZ, POL, B, B, NT, true>(s, tw.p[0], tid, ld);
     __syncthreads();
     FwdPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
@@ -502,7 +519,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     for (int t = tid; t < TOT; t += NT) {
         const int b = t % RP, k = t / RP;
         const CQ<T>* d = in + (size_t)k * plane + 2 * b;
-        const CQ<T> Q0 = ldgq(d), Q1 = ldgq(d + 1);
+        const CQ<T> Q0 = ldsq(d), Q1 = ldsq(d + 1);
         V xkr, xmr, xki, xmi;
         xkr.x = Q0.re.x; xkr.y = Q1.re.x; xmr.x = Q0.re.y; xmr.y = Q1.re.y;
         xki.x = Q0.im.x; xki.y = Q1.im.x; xmi.x = Q0.im.y; xmi.y = Q1.im.y;
