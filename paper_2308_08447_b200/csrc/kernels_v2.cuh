@@ -194,16 +194,28 @@ __device__ __forceinline__ void pass_first(CQ<T>* s, const CQ<T>* __restrict__ t
     constexpr bool HOIST = (LS > 0) && ITER > 1 && (LF ? (NT % BL == 0 && (NT / BL) % S == 0) : (NT % S == 0));
     CQ<T> w[R];
     if (HOIST) load_tw<LR, LS>(w, tab, LF ? ((tid / BL) & (S - 1)) : (tid & (S - 1)));
-#pragma unroll(ITER <= 2 ? ITER : 1)
+    // software pipeline (short loops): the (global) inputs of butterfly k+1 are requested before butterfly k is computed
+    constexpr int H = R > 1 ? R / 2 : 1;
+    CQ<T> nxt[H];
+    auto fetch = [&](int k) {
+        const int t = tid + k * NT;
+        if (TOT % NT == 0 || t < TOT) {
+            const int i = LF ? ((t / BL) & (S - 1)) : (t & (S - 1)), b = LF ? (t % BL) : (t >> LS);
+#pragma unroll
+            for (int r = 0; r < H; ++r) nxt[r] = ld(b, i + r * S);
+        }
+    };
+    if (ITER <= 4) fetch(0);
+#pragma unroll(ITER <= 4 ? ITER : 1)
     for (int k = 0; k < ITER; ++k) {
         const int t = tid + k * NT;
         if (TOT % NT != 0 && t >= TOT) break;
         const int i = LF ? ((t / BL) & (S - 1)) : (t & (S - 1)), b = LF ? (t % BL) : (t >> LS);
         CQ<T> a[R];
-        if (R > 1) {
+        if (ITER > 4) fetch(k);                    // long loops: plain load-use order (fewer live registers)
 #pragma unroll
-            for (int r = 0; r < R / 2; ++r) a[r] = ld(b, i + r * S);
-        } else a[0] = ld(b, i);
+        for (int r = 0; r < H; ++r) a[r] = nxt[r];
+        if (ITER <= 4 && k + 1 < ITER) fetch(k + 1);
         dftR<LR, false, true>(a);
         if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, false>(a, w); }
         CQ<T>* d = s + i * PITCH + b;
@@ -519,7 +531,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     for (int t = tid; t < TOT; t += NT) {
         const int b = t % RP, k = t / RP;
         const CQ<T>* d = in + (size_t)k * plane + 2 * b;
-        const CQ<T> Q0 = ldsq(d), Q1 = ldsq(d + 1);
+        const CQ<T> Q0 = RP >= 4 ? ldsq(d) : ldgq(d), Q1 = RP >= 4 ? ldsq(d + 1) : ldgq(d + 1);
         V xkr, xmr, xki, xmi;
         xkr.x = Q0.re.x; xkr.y = Q1.re.x; xmr.x = Q0.re.y; xmr.y = Q1.re.y;
         xki.x = Q0.im.x; xki.y = Q1.im.x; xmi.x = Q0.im.y; xmi.y = Q1.im.y;
