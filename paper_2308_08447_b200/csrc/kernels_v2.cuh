@@ -376,13 +376,19 @@ template <typename T, int LNZ, int LRF, int KT> struct MulPoints<T, LNZ, LRF, KT
 
 // Nz >= 16 (at least two passes).  Tile = one pair plane ql x TY consecutive py x all z x 3 components:
 // shared s[Nz][3 TY] quads, lines fastest everywhere (a warp's accesses are consecutive quads: conflict free).
-template <typename T, int LNZ, int POL, int TY, int NT, int MINB>
+//
+// FILM = true (TY == 1): the same routine run along y on the x-stage workspace of a one-cell-thick mesh
+// (scope row a3': y FFT . multiply . y IFFT in one kernel, in place on W1v[3][hq][ny]; call it with g.nz = ny,
+// g.Nz = Ny, g.Ny = 1, nq = hq).  The transform axis is y, so the components that change sign on a mirrored
+// frequency are xy and yz: the three lines are taken in the order (x, z, y) and the stored spectrum is permuted
+// to match at plan time (k_pack_film_v), which turns "odd in z" into "odd in y" without touching this code.
+template <typename T, int LNZ, int POL, int TY, int NT, int MINB, bool FILM = false>
 __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K, TwSet<T> tw)
 {
     constexpr int NZ = 1 << LNZ, B = 3 * TY;
     constexpr Sched SC = make_sched(LNZ, POL);
     constexpr int NP = SC.n, LRF = SC.lr[NP - 1], RF = 1 << LRF;
-    static_assert(NP >= 2 && NT % TY == 0, "k_z_v: needs >= 2 passes");
+    static_assert(NP >= 2 && NT % TY == 0 && (!FILM || TY == 1), "k_z_v: needs >= 2 passes");
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     const int tid = threadIdx.x;
     const int tilesY = g.Ny / TY;
@@ -391,7 +397,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     const size_t cstride = (size_t)nq * g.nz * g.Ny;
     CQ<T>* base = W2 + (size_t)ql * g.nz * g.Ny + py0;
     const int Ny = g.Ny;
-    auto ld = [&](int b, int z) { const int c = b / TY, ty = b - c * TY; return ldsq(base + c * cstride + (size_t)z * Ny + ty); };
+    auto ld = [&](int b, int z) { const int c = FILM ? (b == 0 ? 0 : 3 - b) : b / TY, ty = FILM ? 0 : b - c * TY; return ldsq(base + c * cstride + (size_t)z * Ny + ty); };
     pass_first<T, LNZ, POL, B, B, NT, true>(s, tw.p[0], tid, ld);
     __syncthreads();
     FwdPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
@@ -423,7 +429,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     }
     __syncthreads();
     InvPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
-    auto st = [&](int b, int z, CQ<T> v) { const int c = b / TY, ty = b - c * TY; stq(base + c * cstride + (size_t)z * Ny + ty, v); };
+    auto st = [&](int b, int z, CQ<T> v) { const int c = FILM ? (b == 0 ? 0 : 3 - b) : b / TY, ty = FILM ? 0 : b - c * TY; stq(base + c * cstride + (size_t)z * Ny + ty, v); };
     pass_last<T, LNZ, POL, B, B, NT, true>(s, tw.p[0], tid, st);
 }
 

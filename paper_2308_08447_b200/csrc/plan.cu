@@ -294,6 +294,12 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         v2::GeoV gv;
         gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz;
         p->cf.g = gv; p->cd.g = gv;
+        {   // one-cell-thick mesh: y FFT . multiply . y IFFT fused in one kernel, in place on W1 (scope row a3')
+            const bool film = v2::film_supported(nz, g.Nz, g.lNy, p->esz, kMaxSmem) && !getenv("DEMAG_NO_FILM");
+            v2::GeoV gf = gv;
+            gf.nz = ny; gf.Nz = g.Ny; gf.Ny = 1; gf.kpz = g.kpy;
+            p->cf.film = p->cd.film = film; p->cf.gfilm = p->cd.gfilm = gf;
+        }
         p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
         const size_t qsz = 4 * p->esz;                      // one quad
         const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;
@@ -306,6 +312,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         p->w1_bytes = (size_t)3 * gv.hq * g.nz * g.ny * qsz;
         p->w2_bytes = (size_t)p->nq_auto * per_q;
         p->k_bytes = (size_t)gv.hq * g.kpz * g.Ny * 12 * p->esz;
+        if (p->cf.film) { p->w2_bytes = 256; p->k_bytes = (size_t)gv.hq * g.kpy * 12 * p->esz; }
     }
     auto alloc_all = [&]() -> demag_status {
         if (precision == DEMAG_FP32) { demag_status s = set_func_attrs<float>(); if (s) return s; }
@@ -321,7 +328,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         }
         if (p->v2) {
             const int LL[3] = {g.lLc, g.lNy, g.lNz};
-            const int POL[3] = {v2::x_pol(g.lLc), v2::y_pol(g.lNy), v2::z_pol(g.lNz)};
+            const int POL[3] = {v2::x_pol(g.lLc), p->cf.film ? v2::film_pol(g.lNy) : v2::y_pol(g.lNy), v2::z_pol(g.lNz)};
             cudaError_t verr = cudaSuccess;
             if (precision == DEMAG_FP32) {
                 for (int a = 0; a < 3; ++a) {
@@ -334,6 +341,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
                 v2::y_fwd<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::y_inv<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::z_mul<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                if (p->cf.film) { v2::y_film<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr); }
             } else {
                 for (int a = 0; a < 3; ++a) {
                     CUDA_TRY(v2::build_axis_tables<double>(LL[a], POL[a], a == 0 ? nx : 0, &p->td[a], a == 0 ? &p->cd.twpost : nullptr));
@@ -345,6 +353,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
                 v2::y_fwd<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::y_inv<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::z_mul<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                if (p->cd.film) { v2::y_film<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr); }
             }
             {   // y position -> frequency map of the y schedule, for the plan-time pack
                 const v2::Sched sc = v2::make_sched(g.lNy, v2::y_pol(g.lNy));
@@ -416,6 +425,7 @@ demag_status demag_set_slab(demag_plan_t p, int kx_per_slab)
 int demag_launches_per_apply(demag_plan_t p)
 {
     if (!p) return 0;
+    if (p->v2 && p->cf.film) return 3 + (p->embed ? 2 : 0);
     const int nslab = p->v2 ? (p->cf.g.hq + p->nq_slab - 1) / p->nq_slab : (p->g.hx + p->nkx_slab - 1) / p->nkx_slab;
     return 2 + 3 * nslab + (p->embed ? 2 : 0);
 }
@@ -519,7 +529,14 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
             // each odd axis contributes a factor i (X = i Im X): two odd axes -> -1.  Eq. (1)'s minus sign and
             // the inverse-transform normalisation 1/(Nx Ny Nz) are folded in here (R3).
             const double scale = (nodd == 2 ? -1.0 : 1.0) * (-1.0) / ((double)g.Nx * g.Ny * g.Nz);
-            if (p->v2) {    // pair layout; the real split of the x transform hands over 2 X[k]: fold the 1/2 here
+            if (p->v2 && p->cf.film) {
+                const v2::GeoV& gv = p->cf.g;
+                const size_t n = (size_t)gv.hq * g.kpy;
+                const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
+                if (p->prec == DEMAG_FP32) v2::k_pack_film_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, 0.5 * scale);
+                else v2::k_pack_film_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, 0.5 * scale);
+            }
+            else if (p->v2) {    // pair layout; the real split of the x transform hands over 2 X[k]: fold the 1/2 here
                 const v2::GeoV& gv = p->cf.g;
                 const size_t n = (size_t)gv.hq * g.kpz * g.Ny;
                 const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
@@ -600,7 +617,8 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
         const typename v2::kchunks<T>::V* Kv = (const typename v2::kchunks<T>::V*)p->K;
         cudaError_t verr = cudaSuccess;
         STAGE(0, (v2::x_fwd<T>(1, cx, st, M, V1, &verr)));
-        for (int q0 = 0; q0 < cx.g.hq; q0 += p->nq_slab) {
+        if (cx.film) STAGE(2, (v2::y_film<T>(1, cx, st, V1, Kv, &verr)));
+        else for (int q0 = 0; q0 < cx.g.hq; q0 += p->nq_slab) {
             const int nq = std::min(p->nq_slab, cx.g.hq - q0);
             STAGE(1, (v2::y_fwd<T>(1, cx, st, q0, nq, V1, V2, &verr)));
             STAGE(2, (v2::z_mul<T>(1, cx, st, q0, nq, V2, Kv, &verr)));

@@ -147,9 +147,36 @@ __global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv
     }
 }
 
+// One-cell-thick meshes (k_z_v FILM): A = [ky'][kx] (kpz = 1).  Kf[q][ky'][chunk], y packed by symmetry (the kernel
+// applies the mirror sign itself), components stored in the slots of the (x, z, y) line order:
+// xx->xx, yy->zz, zz->yy, xy->xz, xz->xy, yz->yz.
+template <typename T>
+__global__ void k_pack_film_v(const double* __restrict__ A, T* __restrict__ Kf, int comp, int Lc, int hq, int kpy, double scale)
+{
+    const size_t n = (size_t)hq * kpy;
+    const int hx = Lc + 1;
+    constexpr int U = 16 / (int)sizeof(T), NCH = 12 / U;
+    const int slot = comp == 1 ? 2 : comp == 2 ? 1 : comp == 3 ? 4 : comp == 4 ? 3 : comp;
+    const int j = sizeof(T) == 4 ? slot / 2 : slot, off = sizeof(T) == 4 ? (slot % 2) * 2 : 0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int ky = (int)(i % kpy), q = (int)(i / kpy);
+        const double* row = A + (size_t)ky * hx;
+        T* d = Kf + (i * NCH + j) * U + off;
+        d[0] = (T)(scale * row[q]);
+        d[1] = (T)(scale * row[Lc - q]);
+    }
+}
+inline bool film_supported(int nz, int Nz, int lNy, size_t esz, int max_smem)
+{
+    return nz == 1 && Nz == 1 && lNy >= 4 && lNy <= 12 && ((size_t)3 << lNy) * 4 * esz <= (size_t)max_smem;
+}
+inline int film_pol(int lNy) { return lNy == 4 ? 0 : 1; }
+
 // ---- launchers ---------------------------------------------------------------------------------------------
 template <typename T> struct Ctx {
     GeoV g;
+    GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
+    bool film;
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;
     const CQ<T>* twpost;
@@ -238,6 +265,24 @@ bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2
     case 2: if (mode) k_z1_v<T, 2><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
     case 3: if (mode) k_z1_v<T, 3><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
         V2_CASE_Z(4) V2_CASE_Z(5) V2_CASE_Z(6) V2_CASE_Z(7) V2_CASE_Z(8) V2_CASE_Z(9) V2_CASE_Z(10) V2_CASE_Z(11)
+    default: return false;
+    }
+}
+
+// fused y stage of a one-cell-thick mesh: k_z_v<FILM> along y, in place on W1v
+#define V2_CASE_FILM(L, POL_, NT_)                                                                                  \
+    case L: {                                                                                                        \
+        constexpr int smem = (3 << L) * (int)sizeof(CQ<T>);                                                          \
+        if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, POL_, 1, NT_, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+        else k_z_v<T, L, POL_, 1, NT_, 1, true><<<(unsigned)c.g.hq, NT_, smem, st>>>(c.gfilm, 0, c.g.hq, W1, K, c.twy); \
+        return true;                                                                                                 \
+    }
+template <typename T>
+bool y_film(int mode, const Ctx<T>& c, cudaStream_t st, CQ<T>* W1, const typename kchunks<T>::V* K, cudaError_t* err)
+{
+    switch (c.lNy) {
+        V2_CASE_FILM(4, 0, 32) V2_CASE_FILM(5, 1, 32) V2_CASE_FILM(6, 1, 32) V2_CASE_FILM(7, 1, 32) V2_CASE_FILM(8, 1, 64)
+        V2_CASE_FILM(9, 1, 64) V2_CASE_FILM(10, 1, 128) V2_CASE_FILM(11, 1, 256) V2_CASE_FILM(12, 1, 512)
     default: return false;
     }
 }
