@@ -170,7 +170,7 @@ inline bool film_supported(int nz, int Nz, int lNy, size_t esz, int max_smem)
 {
     return nz == 1 && Nz == 1 && lNy >= 4 && lNy <= 12 && ((size_t)3 << lNy) * 4 * esz <= (size_t)max_smem;
 }
-inline int film_pol(int lNy) { return lNy == 4 ? 0 : 1; }
+inline int film_pol(int lNy) { return lNy == 4 ? 0 : (lNy == 8 || lNy == 11) ? 2 : 1; }   // 2048 = 16 . 16 . 8
 
 // ---- launchers ---------------------------------------------------------------------------------------------
 template <typename T> struct Ctx {
@@ -281,8 +281,8 @@ template <typename T>
 bool y_film(int mode, const Ctx<T>& c, cudaStream_t st, CQ<T>* W1, const typename kchunks<T>::V* K, cudaError_t* err)
 {
     switch (c.lNy) {
-        V2_CASE_FILM(4, 0, 32) V2_CASE_FILM(5, 1, 32) V2_CASE_FILM(6, 1, 32) V2_CASE_FILM(7, 1, 32) V2_CASE_FILM(8, 1, 64)
-        V2_CASE_FILM(9, 1, 64) V2_CASE_FILM(10, 1, 128) V2_CASE_FILM(11, 1, 256) V2_CASE_FILM(12, 1, 512)
+        V2_CASE_FILM(4, 0, 32) V2_CASE_FILM(5, 1, 32) V2_CASE_FILM(6, 1, 32) V2_CASE_FILM(7, 1, 32) V2_CASE_FILM(8, 2, 64)
+        V2_CASE_FILM(9, 1, 64) V2_CASE_FILM(10, 1, 128) V2_CASE_FILM(11, 2, 256) V2_CASE_FILM(12, 1, 512)
     default: return false;
     }
 }
