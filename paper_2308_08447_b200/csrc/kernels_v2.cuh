@@ -98,7 +98,26 @@ __device__ __forceinline__ void apply_tw(CQ<T>* a, const CQ<T>* w)
     for (int m = 1; m < (1 << LR); ++m) a[m] = ctw<INV>(a[m], w[m]);
 }
 
-// ---- one in-place pass over a shared-memory tile s[p][PITCH], lines fastest ---------------------------------
+// ---- tile addressing ------------------------------------------------------------------------------------
+// PITCH > 0: point p of line b sits at s[p * PITCH + b].
+// PITCH < 0: skewed tile, s[p * |PITCH| + (p >> 3) + b]: besides "lines fastest" and "consecutive points", threads
+//            that walk the butterflies of a stride-1 radix-8 pass (points 8 i + r) also fall into distinct banks, so
+//            the y kernels can run their last forward / first inverse pass straight against global memory.
+//            (Strides are multiples of 8 or 1 in the POL 1 schedules, so every leg offset stays an immediate.)
+template <int PITCH> __device__ __forceinline__ int tile_addr(int p, int b)
+{
+    return PITCH > 0 ? p * PITCH + b : p * (-PITCH) + (p >> 3) + b;
+}
+template <int PITCH, int S> __host__ __device__ constexpr int tile_step()
+{
+    return PITCH > 0 ? S * PITCH : (S >= 8 ? S * (-PITCH) + S / 8 : S * (-PITCH));
+}
+template <int PITCH> __host__ __device__ constexpr int tile_quads(int L, int BL)
+{
+    return PITCH > 0 ? L * PITCH : L * (-PITCH) + L / 8 + BL;
+}
+
+// ---- one in-place pass over a shared-memory tile, lines fastest ---------------------------------------------
 // pass J of schedule SC on lines of length 2^LL; BL lines (quads) per tile; NT threads.
 template <typename T, int LL, int POL, int J, bool INV, int BL, int PITCH, int NT>
 __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab, int tid)
@@ -118,10 +137,11 @@ __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab,
         const int b = t % BL, i = t / BL;
         const int lo = i & (S - 1);
         const int p0 = ((i >> LS) << (LS + LR)) + lo;
-        CQ<T>* d = s + p0 * PITCH + b;
+        static_assert(PITCH > 0 || S >= 8 || (S == 1 && R <= 8), "skewed tile: strides must be multiples of 8, or 1");
+        CQ<T>* d = s + tile_addr<PITCH>(p0, b);
         CQ<T> a[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * S * PITCH);
+        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * tile_step<PITCH, S>());
         if (!INV) {
             dftR<LR, false, false>(a);
             if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, lo); apply_tw<LR, false>(a, w); }
@@ -130,7 +150,7 @@ __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab,
             dftR<LR, true, false>(a);
         }
 #pragma unroll
-        for (int r = 0; r < R; ++r) stq(d + r * S * PITCH, a[r]);
+        for (int r = 0; r < R; ++r) stq(d + r * tile_step<PITCH, S>(), a[r]);
     }
 }
 // forward passes J..J1-1 (each followed by a barrier) / inverse passes J-1 down to J0
@@ -218,9 +238,9 @@ __device__ __forceinline__ void pass_first(CQ<T>* s, const CQ<T>* __restrict__ t
         if (ITER <= 4 && k + 1 < ITER) fetch(k + 1);
         dftR<LR, false, true>(a);
         if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, false>(a, w); }
-        CQ<T>* d = s + i * PITCH + b;
+        CQ<T>* d = s + tile_addr<PITCH>(i, b);
 #pragma unroll
-        for (int r = 0; r < R; ++r) stq(d + r * S * PITCH, a[r]);
+        for (int r = 0; r < R; ++r) stq(d + r * tile_step<PITCH, S>(), a[r]);
     }
 }
 // last inverse pass (pass 0 backwards): outputs r < R/2 (the crop) go to st(line, point, value)
@@ -239,10 +259,10 @@ __device__ __forceinline__ void pass_last(const CQ<T>* s, const CQ<T>* __restric
         const int t = tid + k * NT;
         if (TOT % NT != 0 && t >= TOT) break;
         const int i = LF ? ((t / BL) & (S - 1)) : (t & (S - 1)), b = LF ? (t % BL) : (t >> LS);
-        const CQ<T>* d = s + i * PITCH + b;
+        const CQ<T>* d = s + tile_addr<PITCH>(i, b);
         CQ<T> a[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * S * PITCH);
+        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * tile_step<PITCH, S>());
         if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, true>(a, w); }
         dftR<LR, true, false>(a);
 #pragma unroll
@@ -258,13 +278,18 @@ __device__ __forceinline__ long long w1v_line_offset(const GeoV& g, int l, int q
     return (((long long)c * g.hq + q0 + ql) * g.nz + z) * g.ny;
 }
 
-// y forward FFT, zero padding synthesised (PAPER.md:309-315 yFFT): W1v -> W2v (position order)
+// W2v order of a y line ("position order"): with NP >= 2 passes the last forward pass (stride 1, radix R, butterfly i
+// = points R i .. R i + R - 1) stores its output r of butterfly i at  r * (Ny / R) + i  -- consecutive threads write
+// consecutive quads, straight from registers -- and the first inverse pass loads the same way.  The stored kernel
+// spectrum follows the same order (ypos2freq, v2_host.cuh: y_w2_pos_to_tile_pos).
+// y forward FFT, zero padding synthesised (PAPER.md:309-315 yFFT): W1v -> W2v
 template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
                                                CQ<T>* __restrict__ W2, TwSet<T> tw)
 {
-    constexpr int NY = 1 << LNY, PITCH = BP | 1;
     constexpr Sched SC = make_sched(LNY, POL);
+    constexpr int NP = SC.n;
+    constexpr int NY = 1 << LNY, PITCH = NP >= 2 ? -(BP | 1) : (BP | 1);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     __shared__ long long loff[BP];
     const int tid = threadIdx.x;
@@ -275,13 +300,32 @@ __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ
     auto ld = [&](int b, int p) { const long long o = loff[b]; return o >= 0 ? ldsq(W1 + o + p) : cq_zero<T>(); };
     pass_first<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, ld);
     __syncthreads();
-    FwdPasses<T, LNY, POL, 1, SC.n, BP, PITCH, NT>::run(s, tw, tid);
     CQ<T>* dst = W2 + (size_t)l0 * NY;
     const int nvalid = min(BP, nlines - l0);
+    if constexpr (NP >= 2) {
+        FwdPasses<T, LNY, POL, 1, NP - 1, BP, PITCH, NT>::run(s, tw, tid);
+        // last pass (stride 1, no twiddles): butterflies fastest, results straight to global
+        constexpr int LR = SC.lr[NP - 1], R = 1 << LR, LNB = LNY - LR, NBF = 1 << LNB, TOT = NBF * BP;
+        static_assert(SC.ls[NP - 1] == 0 && R <= 8, "last pass has stride 1");
+#pragma unroll 2
+        for (int t = tid; t < TOT; t += NT) {
+            const int i = t & (NBF - 1), b = t >> LNB;
+            const CQ<T>* d = s + tile_addr<PITCH>(i << LR, b);
+            CQ<T> a[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) a[r] = ldq(d + r * tile_step<PITCH, 1>());
+            dftR<LR, false, false>(a);
+            if (b < nvalid) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) stq(dst + ((size_t)b << LNY) + (r << LNB) + i, a[r]);
+            }
+        }
+    } else {
 #pragma unroll 4
-    for (int idx = tid; idx < (nvalid << LNY); idx += NT) {
-        const int b = idx >> LNY, p = idx & (NY - 1);
-        stq(dst + idx, ldq(s + p * PITCH + b));
+        for (int idx = tid; idx < (nvalid << LNY); idx += NT) {
+            const int b = idx >> LNY, p = idx & (NY - 1);
+            stq(dst + idx, ldq(s + tile_addr<PITCH>(p, b)));
+        }
     }
 }
 
@@ -290,8 +334,9 @@ template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
                                                CQ<T>* __restrict__ W1, TwSet<T> tw)
 {
-    constexpr int NY = 1 << LNY, PITCH = BP | 1;
     constexpr Sched SC = make_sched(LNY, POL);
+    constexpr int NP = SC.n;
+    constexpr int NY = 1 << LNY, PITCH = NP >= 2 ? -(BP | 1) : (BP | 1);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     __shared__ long long loff[BP];
     const int tid = threadIdx.x;
@@ -300,13 +345,30 @@ __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ
     if (tid < BP) loff[tid] = (l0 + tid < nlines) ? w1v_line_offset(g, l0 + tid, q0, nq) : -1;
     const CQ<T>* src = W2 + (size_t)l0 * NY;
     const int nvalid = min(BP, nlines - l0);
+    if constexpr (NP >= 2) {
+        // first inverse pass (stride 1, no twiddles): inputs straight from global, butterflies fastest
+        constexpr int LR = SC.lr[NP - 1], R = 1 << LR, LNB = LNY - LR, NBF = 1 << LNB, TOT = NBF * BP;
+#pragma unroll 2
+        for (int t = tid; t < TOT; t += NT) {
+            const int i = t & (NBF - 1), b = t >> LNB;
+            CQ<T> a[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) a[r] = b < nvalid ? ldsq(src + ((size_t)b << LNY) + (r << LNB) + i) : cq_zero<T>();
+            dftR<LR, true, false>(a);
+            CQ<T>* d = s + tile_addr<PITCH>(i << LR, b);
+#pragma unroll
+            for (int r = 0; r < R; ++r) stq(d + r * tile_step<PITCH, 1>(), a[r]);
+        }
+        __syncthreads();
+        InvPasses<T, LNY, POL, 1, NP - 1, BP, PITCH, NT>::run(s, tw, tid);
+    } else {
 #pragma unroll 4
-    for (int idx = tid; idx < (BP << LNY); idx += NT) {
-        const int b = idx >> LNY, p = idx & (NY - 1);
-        stq(s + p * PITCH + b, b < nvalid ? ldsq(src + idx) : cq_zero<T>());
+        for (int idx = tid; idx < (BP << LNY); idx += NT) {
+            const int b = idx >> LNY, p = idx & (NY - 1);
+            stq(s + tile_addr<PITCH>(p, b), b < nvalid ? ldsq(src + idx) : cq_zero<T>());
+        }
+        __syncthreads();
     }
-    __syncthreads();
-    InvPasses<T, LNY, POL, 1, SC.n, BP, PITCH, NT>::run(s, tw, tid);
     auto st = [&](int b, int p, CQ<T> v) { const long long o = loff[b]; if (o >= 0) stq(W1 + o + p, v); };
     pass_last<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, st);
 }

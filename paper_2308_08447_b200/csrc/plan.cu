@@ -358,7 +358,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
             {   // y position -> frequency map of the y schedule, for the plan-time pack
                 const v2::Sched sc = v2::make_sched(g.lNy, v2::y_pol(g.lNy));
                 std::vector<int> h((size_t)g.Ny);
-                for (int q = 0; q < g.Ny; ++q) h[q] = v2::sched_freq_of_pos(sc, q);
+                for (int q = 0; q < g.Ny; ++q) h[q] = v2::sched_freq_of_pos(sc, v2::y_w2_pos_to_tile_pos(g.lNy, v2::y_pol(g.lNy), q));
                 CUDA_TRY(cudaMalloc(&p->ypos2freq, sizeof(int) * (size_t)g.Ny));
                 CUDA_TRY(cudaMemcpy(p->ypos2freq, h.data(), sizeof(int) * (size_t)g.Ny, cudaMemcpyHostToDevice));
                 p->tw_bytes += sizeof(int) * (size_t)g.Ny;

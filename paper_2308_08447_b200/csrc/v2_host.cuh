@@ -36,6 +36,20 @@ template <> struct ZCfg<9>  { static constexpr int POL = 1, TY = 4,  NT = 128, M
 template <> struct ZCfg<10> { static constexpr int POL = 1, TY = 2,  NT = 128, MINB = 1; };   // 16 . 8 . 8
 template <> struct ZCfg<11> { static constexpr int POL = 1, TY = 1,  NT = 64,  MINB = 1; };   // 4 . 8 . 8 . 8
 
+// quads of the y tile (skewed when the schedule has >= 2 passes, kernels_v2.cuh "tile addressing")
+constexpr int y_tile_quads(int LNY, int POL, int BP)
+{
+    return make_sched(LNY, POL).n >= 2 ? (1 << LNY) * (BP | 1) + (1 << LNY) / 8 + BP : (1 << LNY) * (BP | 1);
+}
+// W2v position p' of a y line -> in-place (digit-reversed) tile position: with >= 2 passes the last pass scatters
+// output r of butterfly i to r * (Ny / R) + i
+inline int y_w2_pos_to_tile_pos(int LNY, int POL, int pw)
+{
+    const Sched sc = make_sched(LNY, POL);
+    if (sc.n < 2) return pw;
+    const int lr = sc.lr[sc.n - 1], lnb = LNY - lr;
+    return ((pw & ((1 << lnb) - 1)) << lr) + (pw >> lnb);
+}
 constexpr int kXMin = 4, kXMax = 12, kYMin = 4, kYMax = 13, kZMin = 2, kZMax = 11;
 
 inline int x_rp(int lLc)
@@ -66,7 +80,7 @@ inline bool supported(int nx, int ny, int nz, int Nx, int Ny, int Nz, int lLc, i
     if (lNz < 4 && Ny < 32) return false;
     // shared memory of the y tile (the largest): Ny * (BP|1) quads
     const int bp = lNy <= 9 ? 8 : lNy == 10 ? 4 : lNy == 11 ? 2 : 1;
-    if ((size_t)Ny * (bp | 1) * 4 * esz > (size_t)max_smem) return false;
+    if ((size_t)y_tile_quads(lNy, y_pol(lNy), bp) * 4 * esz > (size_t)max_smem) return false;
     if ((size_t)nx * (x_rp(lLc) | 1) * 4 * esz > (size_t)max_smem) return false;
     if ((size_t)Nz * 3 * z_ty(lNz) * 4 * esz > (size_t)max_smem && lNz >= 4) return false;
     return true;
@@ -221,7 +235,7 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
 #define V2_BODY_Y(L, KERN, A, B)                                                                                    \
     {                                                                                                                \
         using C = YCfg<L>;                                                                                           \
-        constexpr int smem = (1 << L) * (C::BP | 1) * (int)sizeof(CQ<T>);                                            \
+        constexpr int smem = y_tile_quads(L, C::POL, C::BP) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::BP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
         else KERN<T, L, C::POL, C::BP, C::NT><<<(unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st>>>(c.g, q0, nq, A, B, c.twy); \
         return true;                                                                                                 \
