@@ -99,23 +99,29 @@ __device__ __forceinline__ void apply_tw(CQ<T>* a, const CQ<T>* w)
 }
 
 // ---- tile addressing ------------------------------------------------------------------------------------
-// PITCH > 0: point p of line b sits at s[p * PITCH + b].
-// PITCH < 0: skewed tile, s[p * |PITCH| + (p >> 3) + b]: besides "lines fastest" and "consecutive points", threads
-//            that walk the butterflies of a stride-1 radix-8 pass (points 8 i + r) also fall into distinct banks, so
-//            the y kernels can run their last forward / first inverse pass straight against global memory.
-//            (Strides are multiples of 8 or 1 in the POL 1 schedules, so every leg offset stays an immediate.)
-template <int PITCH> __device__ __forceinline__ int tile_addr(int p, int b)
+// A tile parameter PE encodes (pitch, skew) = (PE & 0xffff, PE >> 16): point p of line b sits at
+//     s[p * pitch + (p >> 3) * skew + b].
+// skew = 0 is the plain point-major tile.  With a skew, threads that walk the butterflies of a stride-1 pass
+// (points R i + r, R >= 8) fall into distinct banks even when the tile holds fewer than 8 lines (long lines), and the
+// y kernels can run their last forward / first inverse pass butterflies-fastest straight against global memory.
+// Strides are multiples of 8, or 1 with radix >= 8, wherever a skewed tile is used, so every leg offset is an immediate.
+DM_HDC int tile_pe(int pitch, int skew) { return pitch + (skew << 16); }
+template <int PE> __device__ __forceinline__ int tile_addr(int p, int b)
 {
-    return PITCH > 0 ? p * PITCH + b : p * (-PITCH) + (p >> 3) + b;
+    return (PE >> 16) ? p * (PE & 0xffff) + (p >> 3) * (PE >> 16) + b : p * PE + b;
 }
-template <int PITCH, int S> __host__ __device__ constexpr int tile_step()
+template <int PE, int S> __host__ __device__ constexpr int tile_leg(int r)      // offset of leg r (point p0 + r S) from leg 0
 {
-    return PITCH > 0 ? S * PITCH : (S >= 8 ? S * (-PITCH) + S / 8 : S * (-PITCH));
+    return r * S * (PE & 0xffff) + ((r * S) >> 3) * (PE >> 16);
 }
-template <int PITCH> __host__ __device__ constexpr int tile_quads(int L, int BL)
+DM_HDC bool skew_ok(int LL, int POL)      // can a skewed tile be used with this schedule?
 {
-    return PITCH > 0 ? L * PITCH : L * (-PITCH) + L / 8 + BL;
+    const Sched sc = make_sched(LL, POL);
+    for (int j = 0; j < sc.n; ++j)
+        if (!(sc.ls[j] >= 3 || (sc.ls[j] == 0 && sc.lr[j] >= 3))) return false;
+    return true;
 }
+DM_HDC int tile_quads(int PE, int L, int BL) { return L * (PE & 0xffff) + ((PE >> 16) ? (L / 8) * (PE >> 16) + BL : 0); }
 
 // ---- one in-place pass over a shared-memory tile, lines fastest ---------------------------------------------
 // pass J of schedule SC on lines of length 2^LL; BL lines (quads) per tile; NT threads.
@@ -137,11 +143,11 @@ __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab,
         const int b = t % BL, i = t / BL;
         const int lo = i & (S - 1);
         const int p0 = ((i >> LS) << (LS + LR)) + lo;
-        static_assert(PITCH > 0 || S >= 8 || (S == 1 && R <= 8), "skewed tile: strides must be multiples of 8, or 1");
+        static_assert((PITCH >> 16) == 0 || S >= 8 || (S == 1 && R >= 8), "skewed tile: strides must be multiples of 8, or 1 with radix >= 8");
         CQ<T>* d = s + tile_addr<PITCH>(p0, b);
         CQ<T> a[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * tile_step<PITCH, S>());
+        for (int r = 0; r < R; ++r) a[r] = ldq(d + tile_leg<PITCH, S>(r));
         if (!INV) {
             dftR<LR, false, false>(a);
             if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, lo); apply_tw<LR, false>(a, w); }
@@ -150,7 +156,7 @@ __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab,
             dftR<LR, true, false>(a);
         }
 #pragma unroll
-        for (int r = 0; r < R; ++r) stq(d + r * tile_step<PITCH, S>(), a[r]);
+        for (int r = 0; r < R; ++r) stq(d + tile_leg<PITCH, S>(r), a[r]);
     }
 }
 // forward passes J..J1-1 (each followed by a barrier) / inverse passes J-1 down to J0
@@ -240,7 +246,7 @@ __device__ __forceinline__ void pass_first(CQ<T>* s, const CQ<T>* __restrict__ t
         if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, false>(a, w); }
         CQ<T>* d = s + tile_addr<PITCH>(i, b);
 #pragma unroll
-        for (int r = 0; r < R; ++r) stq(d + r * tile_step<PITCH, S>(), a[r]);
+        for (int r = 0; r < R; ++r) stq(d + tile_leg<PITCH, S>(r), a[r]);
     }
 }
 // last inverse pass (pass 0 backwards): outputs r < R/2 (the crop) go to st(line, point, value)
@@ -262,7 +268,7 @@ __device__ __forceinline__ void pass_last(const CQ<T>* s, const CQ<T>* __restric
         const CQ<T>* d = s + tile_addr<PITCH>(i, b);
         CQ<T> a[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) a[r] = ldq(d + r * tile_step<PITCH, S>());
+        for (int r = 0; r < R; ++r) a[r] = ldq(d + tile_leg<PITCH, S>(r));
         if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, true>(a, w); }
         dftR<LR, true, false>(a);
 #pragma unroll
@@ -289,7 +295,7 @@ __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ
 {
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
-    constexpr int NY = 1 << LNY, PITCH = NP >= 2 ? -(BP | 1) : (BP | 1);
+    constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     __shared__ long long loff[BP];
     const int tid = threadIdx.x;
@@ -306,14 +312,14 @@ __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ
         FwdPasses<T, LNY, POL, 1, NP - 1, BP, PITCH, NT>::run(s, tw, tid);
         // last pass (stride 1, no twiddles): butterflies fastest, results straight to global
         constexpr int LR = SC.lr[NP - 1], R = 1 << LR, LNB = LNY - LR, NBF = 1 << LNB, TOT = NBF * BP;
-        static_assert(SC.ls[NP - 1] == 0 && R <= 8, "last pass has stride 1");
+        static_assert(SC.ls[NP - 1] == 0 && R >= 8, "last pass: stride 1, radix >= 8");
 #pragma unroll 2
         for (int t = tid; t < TOT; t += NT) {
             const int i = t & (NBF - 1), b = t >> LNB;
             const CQ<T>* d = s + tile_addr<PITCH>(i << LR, b);
             CQ<T> a[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) a[r] = ldq(d + r * tile_step<PITCH, 1>());
+            for (int r = 0; r < R; ++r) a[r] = ldq(d + tile_leg<PITCH, 1>(r));
             dftR<LR, false, false>(a);
             if (b < nvalid) {
 #pragma unroll
@@ -336,7 +342,7 @@ __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ
 {
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
-    constexpr int NY = 1 << LNY, PITCH = NP >= 2 ? -(BP | 1) : (BP | 1);
+    constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     __shared__ long long loff[BP];
     const int tid = threadIdx.x;
@@ -357,7 +363,7 @@ __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ
             dftR<LR, true, false>(a);
             CQ<T>* d = s + tile_addr<PITCH>(i << LR, b);
 #pragma unroll
-            for (int r = 0; r < R; ++r) stq(d + r * tile_step<PITCH, 1>(), a[r]);
+            for (int r = 0; r < R; ++r) stq(d + tile_leg<PITCH, 1>(r), a[r]);
         }
         __syncthreads();
         InvPasses<T, LNY, POL, 1, NP - 1, BP, PITCH, NT>::run(s, tw, tid);
@@ -451,6 +457,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     constexpr Sched SC = make_sched(LNZ, POL);
     constexpr int NP = SC.n, LRF = SC.lr[NP - 1], RF = 1 << LRF;
     static_assert(NP >= 2 && NT % TY == 0 && (!FILM || TY == 1), "k_z_v: needs >= 2 passes");
+    constexpr int PE = tile_pe(B, (TY <= 2 && skew_ok(LNZ, POL)) ? TY : 0);     // narrow tiles: skewed (bank conflicts)
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     const int tid = threadIdx.x;
     const int tilesY = g.Ny / TY;
@@ -460,9 +467,9 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     CQ<T>* base = W2 + (size_t)ql * g.nz * g.Ny + py0;
     const int Ny = g.Ny;
     auto ld = [&](int b, int z) { const int c = FILM ? (b == 0 ? 0 : 3 - b) : b / TY, ty = FILM ? 0 : b - c * TY; return ldsq(base + c * cstride + (size_t)z * Ny + ty); };
-    pass_first<T, LNZ, POL, B, B, NT, true>(s, tw.p[0], tid, ld);
+    pass_first<T, LNZ, POL, B, PE, NT, true>(s, tw.p[0], tid, ld);
     __syncthreads();
-    FwdPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
+    FwdPasses<T, LNZ, POL, 1, NP - 1, B, PE, NT>::run(s, tw, tid);
     {   // fused: last forward pass . multiply . first inverse pass; item = (butterfly i, column ty), 3 components
         constexpr int NBF = NZ >> LRF, TOT = NBF * TY, ITER = (TOT + NT - 1) / NT;
         const typename kchunks<T>::V* Kq = K + ((size_t)(q0 + ql) * tilesY + pyt) * g.kpz * (kchunks<T>::N * TY);   // KT == TY
@@ -476,7 +483,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
 #pragma unroll
             for (int cc = 0; cc < 3; ++cc) {
 #pragma unroll
-                for (int m = 0; m < RF; ++m) a[cc][m] = ldq(s + (p0 + m) * B + cc * TY + ty);
+                for (int m = 0; m < RF; ++m) a[cc][m] = ldq(s + tile_addr<PE>(p0, cc * TY + ty) + tile_leg<PE, 1>(m));
                 dftR<LRF, false, false>(a[cc]);
             }
             const int f0 = freq_of_pos_rt<LNZ, POL>(p0);
@@ -485,14 +492,14 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
             for (int cc = 0; cc < 3; ++cc) {
                 dftR<LRF, true, false>(a[cc]);
 #pragma unroll
-                for (int m = 0; m < RF; ++m) stq(s + (p0 + m) * B + cc * TY + ty, a[cc][m]);
+                for (int m = 0; m < RF; ++m) stq(s + tile_addr<PE>(p0, cc * TY + ty) + tile_leg<PE, 1>(m), a[cc][m]);
             }
         }
     }
     __syncthreads();
-    InvPasses<T, LNZ, POL, 1, NP - 1, B, B, NT>::run(s, tw, tid);
+    InvPasses<T, LNZ, POL, 1, NP - 1, B, PE, NT>::run(s, tw, tid);
     auto st = [&](int b, int z, CQ<T> v) { const int c = FILM ? (b == 0 ? 0 : 3 - b) : b / TY, ty = FILM ? 0 : b - c * TY; stq(base + c * cstride + (size_t)z * Ny + ty, v); };
-    pass_last<T, LNZ, POL, B, B, NT, true>(s, tw.p[0], tid, st);
+    pass_last<T, LNZ, POL, B, PE, NT, true>(s, tw.p[0], tid, st);
 }
 
 // Nz <= 8: the whole z transform of a column is one butterfly per component in registers; no shared memory.
@@ -538,7 +545,7 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
     using V = typename vec2<T>::type;
-    constexpr int LC = 1 << LLC, PITCH = RP | 1;
+    constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0);
     constexpr Sched SC = make_sched(LLC, POL);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     const int tid = threadIdx.x;
@@ -562,8 +569,8 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
 #pragma unroll 2
     for (int t = tid; t < TOT; t += NT) {
         const int b = t % RP, k = t / RP;
-        const CQ<T> Zk = ldq(s + pos_of_freq_rt<LLC, POL>(k) * PITCH + b);
-        const CQ<T> Zm = ldq(s + pos_of_freq_rt<LLC, POL>((LC - k) & (LC - 1)) * PITCH + b);
+        const CQ<T> Zk = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>(k), b));
+        const CQ<T> Zm = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>((LC - k) & (LC - 1)), b));
         const CQ<T> w = ldgq(twpost + k);
         CQ<T> D; D.re = vsub(Zk.re, Zm.re); D.im = vadd(Zk.im, Zm.im);
         const V A = vadd(Zk.re, Zm.re), Bm = vsub(Zk.im, Zm.im);
@@ -584,7 +591,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
     using V = typename vec2<T>::type;
-    constexpr int LC = 1 << LLC, PITCH = RP | 1;
+    constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0);
     constexpr Sched SC = make_sched(LLC, POL);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     const int tid = threadIdx.x;
@@ -609,8 +616,8 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
         CQ<T> Zk, Zm;
         Zk.re = vsub(Ar, u.im); Zk.im = vadd(Ai, u.re);
         Zm.re = vadd(Ar, u.im); Zm.im = vsub(u.re, Ai);
-        stq(s + pos_of_freq_rt<LLC, POL>(k) * PITCH + b, Zk);
-        if (k != 0 && 2 * k != LC) stq(s + pos_of_freq_rt<LLC, POL>(LC - k) * PITCH + b, Zm);
+        stq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>(k), b), Zk);
+        if (k != 0 && 2 * k != LC) stq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>(LC - k), b), Zm);
     }
     __syncthreads();
     InvPasses<T, LLC, POL, 1, SC.n, RP, PITCH, NT>::run(s, tw, tid);

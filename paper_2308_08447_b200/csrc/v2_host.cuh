@@ -39,8 +39,10 @@ template <> struct ZCfg<11> { static constexpr int POL = 1, TY = 1,  NT = 64,  M
 // quads of the y tile (skewed when the schedule has >= 2 passes, kernels_v2.cuh "tile addressing")
 constexpr int y_tile_quads(int LNY, int POL, int BP)
 {
-    return make_sched(LNY, POL).n >= 2 ? (1 << LNY) * (BP | 1) + (1 << LNY) / 8 + BP : (1 << LNY) * (BP | 1);
+    return tile_quads(tile_pe(BP | 1, make_sched(LNY, POL).n >= 2 ? 1 : 0), 1 << LNY, BP);
 }
+constexpr int x_tile_quads(int LLC, int POL, int RP) { return tile_quads(tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0), 1 << LLC, RP); }
+constexpr int z_tile_quads(int LNZ, int POL, int TY) { return tile_quads(tile_pe(3 * TY, (TY <= 2 && skew_ok(LNZ, POL)) ? TY : 0), 1 << LNZ, 3 * TY); }
 // W2v position p' of a y line -> in-place (digit-reversed) tile position: with >= 2 passes the last pass scatters
 // output r of butterfly i to r * (Ny / R) + i
 inline int y_w2_pos_to_tile_pos(int LNY, int POL, int pw)
@@ -81,8 +83,8 @@ inline bool supported(int nx, int ny, int nz, int Nx, int Ny, int Nz, int lLc, i
     // shared memory of the y tile (the largest): Ny * (BP|1) quads
     const int bp = lNy <= 9 ? 8 : lNy == 10 ? 4 : lNy == 11 ? 2 : 1;
     if ((size_t)y_tile_quads(lNy, y_pol(lNy), bp) * 4 * esz > (size_t)max_smem) return false;
-    if ((size_t)nx * (x_rp(lLc) | 1) * 4 * esz > (size_t)max_smem) return false;
-    if ((size_t)Nz * 3 * z_ty(lNz) * 4 * esz > (size_t)max_smem && lNz >= 4) return false;
+    if ((size_t)x_tile_quads(lLc, x_pol(lLc), x_rp(lLc)) * 4 * esz > (size_t)max_smem) return false;
+    if (lNz >= 4 && (size_t)z_tile_quads(lNz, z_pol(lNz), z_ty(lNz)) * 4 * esz > (size_t)max_smem) return false;
     return true;
 }
 
@@ -180,11 +182,11 @@ __global__ void k_pack_film_v(const double* __restrict__ A, T* __restrict__ Kf, 
         d[1] = (T)(scale * row[Lc - q]);
     }
 }
+inline int film_pol(int lNy) { return lNy == 4 ? 0 : (lNy == 8 || lNy == 11) ? 2 : 1; }   // 2048 = 16 . 16 . 8
 inline bool film_supported(int nz, int Nz, int lNy, size_t esz, int max_smem)
 {
-    return nz == 1 && Nz == 1 && lNy >= 4 && lNy <= 12 && ((size_t)3 << lNy) * 4 * esz <= (size_t)max_smem;
+    return nz == 1 && Nz == 1 && lNy >= 4 && lNy <= 12 && (size_t)z_tile_quads(lNy, film_pol(lNy), 1) * 4 * esz <= (size_t)max_smem;
 }
-inline int film_pol(int lNy) { return lNy == 4 ? 0 : (lNy == 8 || lNy == 11) ? 2 : 1; }   // 2048 = 16 . 16 . 8
 
 // ---- launchers ---------------------------------------------------------------------------------------------
 template <typename T> struct Ctx {
@@ -199,7 +201,7 @@ template <typename T> struct Ctx {
 #define V2_CASE_X(L, KERN, ...)                                                                                     \
     case L: {                                                                                                        \
         using C = XCfg<L>;                                                                                           \
-        constexpr int smem = (1 << L) * (C::RP | 1) * (int)sizeof(CQ<T>);                                            \
+        constexpr int smem = x_tile_quads(L, C::POL, C::RP) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::RP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
         else KERN<T, L, C::POL, C::RP, C::NT><<<3u * c.g.nz * (c.g.ny / (2 * C::RP)), C::NT, smem, st>>>(__VA_ARGS__); \
         return true;                                                                                                 \
@@ -266,7 +268,7 @@ bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<
 #define V2_CASE_Z(L)                                                                                                \
     case L: {                                                                                                        \
         using C = ZCfg<L>;                                                                                           \
-        constexpr int smem = (1 << L) * 3 * C::TY * (int)sizeof(CQ<T>);                                              \
+        constexpr int smem = z_tile_quads(L, C::POL, C::TY) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
         else k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB><<<(unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st>>>(c.g, q0, nq, W2, K, c.twz); \
         return true;                                                                                                 \
@@ -286,7 +288,7 @@ bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2
 // fused y stage of a one-cell-thick mesh: k_z_v<FILM> along y, in place on W1v
 #define V2_CASE_FILM(L, POL_, NT_)                                                                                  \
     case L: {                                                                                                        \
-        constexpr int smem = (3 << L) * (int)sizeof(CQ<T>);                                                          \
+        constexpr int smem = z_tile_quads(L, POL_, 1) * (int)sizeof(CQ<T>);                                          \
         if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, POL_, 1, NT_, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
         else k_z_v<T, L, POL_, 1, NT_, 1, true><<<(unsigned)c.g.hq, NT_, smem, st>>>(c.gfilm, 0, c.g.hq, W1, K, c.twy); \
         return true;                                                                                                 \
