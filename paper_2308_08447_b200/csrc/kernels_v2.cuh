@@ -3,7 +3,7 @@
 // (x R2C -> y FFT -> z FFT . kernel multiplication . z IFFT -> y IFFT -> x C2R), different
 // data layout of the private workspaces:
 //
-//   W1v [3][hq][nz][ny] quads   one quad = x-frequencies (k, Lc-k) of one (y,z): the pair the Hermitian split of
+//   W1v [3][nz][hq][ny] quads   one quad = x-frequencies (k, Lc-k) of one (y,z): the pair the Hermitian split of
 //                               the real transform produces / consumes together (hq = Lc/2 + 1, Lc = Nx/2 = nx)
 //   W2v [3][nq][nz][Ny] quads   slab of nq pairs; y in the digit-reversed "position order" the forward passes
 //                               leave behind (the stored kernel spectrum uses the same order: nothing is permuted)
@@ -538,6 +538,21 @@ __global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2,
 //   2 X[k] = A - i w^k D,  2 X[Lc-k] = conj(A + i w^k D),  A = Z[k] + conj Z[Lc-k],  D = Z[k] - conj Z[Lc-k],
 // w = exp(-2 pi i / 2Lc).  The factor 2 is folded into the stored kernel spectrum.
 
+// Frequency handled by item j (0 <= j <= Lc/2) of the split / merge loops.  With 8 row pairs per tile consecutive
+// threads are consecutive row pairs and k = j.  With fewer (long rows) consecutive threads are consecutive j, and the
+// digit-reversed tile positions of consecutive k all fall into one bank; there j walks the tile POSITIONS whose top
+// frequency digit is 0..3 (k < Lc/2) instead, so that the loads of Z[k] (and of Z[Lc-k], whose position runs
+// backwards) are contiguous (not for single-pair tiles: there the scattered order of the global side costs more,
+// C4 measured): j < Lc/2 -> position 8 (j >> 2) + (j & 3), k = the frequency stored there; j = Lc/2 -> k = Lc/2.
+template <int LLC, int POL, int RP> __device__ __forceinline__ int split_k(int j)
+{
+    constexpr Sched SC = make_sched(LLC, POL);
+    constexpr bool REMAP = RP < 8 && RP > 1 && SC.n >= 2 && SC.lr[SC.n - 1] == 3 && SC.ls[SC.n - 1] == 0;
+    if (!REMAP) return j;
+    if (j >= (1 << (LLC - 1))) return 1 << (LLC - 1);
+    return freq_of_pos_rt<LLC, POL>(((j >> 2) << 3) + (j & 3));
+}
+
 // x R2C FFT fused with the zero padding and the transposition to y-contiguous storage
 // (PAPER.md:35, :296-300 xFFT_R2C; :343 "xy transposition ... to avoid strided y FFTs"):  M -> W1v
 template <typename T, int LLC, int POL, int RP, int NT>
@@ -568,7 +583,7 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
     constexpr int TOT = (LC / 2 + 1) * RP;
 #pragma unroll 2
     for (int t = tid; t < TOT; t += NT) {
-        const int b = t % RP, k = t / RP;
+        const int b = t % RP, k = split_k<LLC, POL, RP>(t / RP);
         const CQ<T> Zk = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>(k), b));
         const CQ<T> Zm = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>((LC - k) & (LC - 1)), b));
         const CQ<T> w = ldgq(twpost + k);
@@ -604,7 +619,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     constexpr int TOT = (LC / 2 + 1) * RP;
 #pragma unroll 2
     for (int t = tid; t < TOT; t += NT) {
-        const int b = t % RP, k = t / RP;
+        const int b = t % RP, k = split_k<LLC, POL, RP>(t / RP);
         const CQ<T>* d = in + (size_t)k * plane + 2 * b;
         const CQ<T> Q0 = RP >= 4 ? ldsq(d) : ldgq(d), Q1 = RP >= 4 ? ldsq(d + 1) : ldgq(d + 1);
         V xkr, xmr, xki, xmi;
