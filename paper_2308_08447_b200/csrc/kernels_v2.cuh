@@ -105,14 +105,21 @@ __device__ __forceinline__ void apply_tw(CQ<T>* a, const CQ<T>* w)
 // (points R i + r, R >= 8) fall into distinct banks even when the tile holds fewer than 8 lines (long lines), and the
 // y kernels can run their last forward / first inverse pass butterflies-fastest straight against global memory.
 // Strides are multiples of 8, or 1 with radix >= 8, wherever a skewed tile is used, so every leg offset is an immediate.
-DM_HDC int tile_pe(int pitch, int skew) { return pitch + (skew << 16); }
+DM_HDC int tile_pe(int pitch, int skew, bool digit_sum = false) { return pitch + (skew << 16) + (digit_sum ? (1 << 30) : 0); }
+// skew term of point p: (p >> 3), or with the digit-sum flag (p >> 3) + (p >> 6) + (p >> 9) + (p >> 12): the bank then
+// depends on the SUM of the base-8 digits of p, so positions that differ in any single digit -- in particular the
+// digit-reversed positions of consecutive frequencies (the split / merge loops of the x stage) -- never collide.
+DM_HDC int tile_skew_term(int PE, int p) { return (PE >> 30) ? (p >> 3) + (p >> 6) + (p >> 9) + (p >> 12) : (p >> 3); }
 template <int PE> __device__ __forceinline__ int tile_addr(int p, int b)
 {
-    return (PE >> 16) ? p * (PE & 0xffff) + (p >> 3) * (PE >> 16) + b : p * PE + b;
+    constexpr int P = PE & 0xffff, SK = (PE >> 16) & 0x3fff;
+    return SK ? p * P + tile_skew_term(PE, p) * SK + b : p * P + b;
 }
-template <int PE, int S> __host__ __device__ constexpr int tile_leg(int r)      // offset of leg r (point p0 + r S) from leg 0
+// offset of leg r (point p0 + r S) from leg 0: p0 has zero bits wherever r S has set bits (in-place passes), so every
+// shifted term separates and the offset is a compile-time constant
+template <int PE, int S> __host__ __device__ constexpr int tile_leg(int r)
 {
-    return r * S * (PE & 0xffff) + ((r * S) >> 3) * (PE >> 16);
+    return r * S * (PE & 0xffff) + tile_skew_term(PE, r * S) * ((PE >> 16) & 0x3fff);
 }
 DM_HDC bool skew_ok(int LL, int POL)      // can a skewed tile be used with this schedule?
 {
@@ -121,7 +128,10 @@ DM_HDC bool skew_ok(int LL, int POL)      // can a skewed tile be used with this
         if (!(sc.ls[j] >= 3 || (sc.ls[j] == 0 && sc.lr[j] >= 3))) return false;
     return true;
 }
-DM_HDC int tile_quads(int PE, int L, int BL) { return L * (PE & 0xffff) + ((PE >> 16) ? (L / 8) * (PE >> 16) + BL : 0); }
+DM_HDC int tile_quads(int PE, int L, int BL)
+{
+    return L * (PE & 0xffff) + (((PE >> 16) & 0x3fff) ? tile_skew_term(PE, L) * ((PE >> 16) & 0x3fff) + BL : 0);
+}
 
 // ---- one in-place pass over a shared-memory tile, lines fastest ---------------------------------------------
 // pass J of schedule SC on lines of length 2^LL; BL lines (quads) per tile; NT threads.
@@ -143,7 +153,6 @@ __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab,
         const int b = t % BL, i = t / BL;
         const int lo = i & (S - 1);
         const int p0 = ((i >> LS) << (LS + LR)) + lo;
-        static_assert((PITCH >> 16) == 0 || S >= 8 || (S == 1 && R >= 8), "skewed tile: strides must be multiples of 8, or 1 with radix >= 8");
         CQ<T>* d = s + tile_addr<PITCH>(p0, b);
         CQ<T> a[R];
 #pragma unroll
@@ -538,21 +547,6 @@ __global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2,
 //   2 X[k] = A - i w^k D,  2 X[Lc-k] = conj(A + i w^k D),  A = Z[k] + conj Z[Lc-k],  D = Z[k] - conj Z[Lc-k],
 // w = exp(-2 pi i / 2Lc).  The factor 2 is folded into the stored kernel spectrum.
 
-// Frequency handled by item j (0 <= j <= Lc/2) of the split / merge loops.  With 8 row pairs per tile consecutive
-// threads are consecutive row pairs and k = j.  With fewer (long rows) consecutive threads are consecutive j, and the
-// digit-reversed tile positions of consecutive k all fall into one bank; there j walks the tile POSITIONS whose top
-// frequency digit is 0..3 (k < Lc/2) instead, so that the loads of Z[k] (and of Z[Lc-k], whose position runs
-// backwards) are contiguous (not for single-pair tiles: there the scattered order of the global side costs more,
-// C4 measured): j < Lc/2 -> position 8 (j >> 2) + (j & 3), k = the frequency stored there; j = Lc/2 -> k = Lc/2.
-template <int LLC, int POL, int RP> __device__ __forceinline__ int split_k(int j)
-{
-    constexpr Sched SC = make_sched(LLC, POL);
-    constexpr bool REMAP = RP < 8 && RP > 1 && SC.n >= 2 && SC.lr[SC.n - 1] == 3 && SC.ls[SC.n - 1] == 0;
-    if (!REMAP) return j;
-    if (j >= (1 << (LLC - 1))) return 1 << (LLC - 1);
-    return freq_of_pos_rt<LLC, POL>(((j >> 2) << 3) + (j & 3));
-}
-
 // x R2C FFT fused with the zero padding and the transposition to y-contiguous storage
 // (PAPER.md:35, :296-300 xFFT_R2C; :343 "xy transposition ... to avoid strided y FFTs"):  M -> W1v
 template <typename T, int LLC, int POL, int RP, int NT>
@@ -560,7 +554,7 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
     using V = typename vec2<T>::type;
-    constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0);
+    constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true);
     constexpr Sched SC = make_sched(LLC, POL);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     const int tid = threadIdx.x;
@@ -583,7 +577,7 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
     constexpr int TOT = (LC / 2 + 1) * RP;
 #pragma unroll 2
     for (int t = tid; t < TOT; t += NT) {
-        const int b = t % RP, k = split_k<LLC, POL, RP>(t / RP);
+        const int b = t % RP, k = t / RP;
         const CQ<T> Zk = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>(k), b));
         const CQ<T> Zm = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>((LC - k) & (LC - 1)), b));
         const CQ<T> w = ldgq(twpost + k);
@@ -606,7 +600,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
     using V = typename vec2<T>::type;
-    constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0);
+    constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true);
     constexpr Sched SC = make_sched(LLC, POL);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     const int tid = threadIdx.x;
@@ -619,7 +613,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     constexpr int TOT = (LC / 2 + 1) * RP;
 #pragma unroll 2
     for (int t = tid; t < TOT; t += NT) {
-        const int b = t % RP, k = split_k<LLC, POL, RP>(t / RP);
+        const int b = t % RP, k = t / RP;
         const CQ<T>* d = in + (size_t)k * plane + 2 * b;
         const CQ<T> Q0 = RP >= 4 ? ldsq(d) : ldgq(d), Q1 = RP >= 4 ? ldsq(d + 1) : ldgq(d + 1);
         V xkr, xmr, xki, xmi;

@@ -41,7 +41,7 @@ constexpr int y_tile_quads(int LNY, int POL, int BP)
 {
     return tile_quads(tile_pe(BP | 1, make_sched(LNY, POL).n >= 2 ? 1 : 0), 1 << LNY, BP);
 }
-constexpr int x_tile_quads(int LLC, int POL, int RP) { return tile_quads(tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0), 1 << LLC, RP); }
+constexpr int x_tile_quads(int LLC, int POL, int RP) { return tile_quads(tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true), 1 << LLC, RP); }
 constexpr int z_tile_quads(int LNZ, int POL, int TY) { return tile_quads(tile_pe(3 * TY, (TY <= 2 && skew_ok(LNZ, POL)) ? TY : 0), 1 << LNZ, 3 * TY); }
 // W2v position p' of a y line -> in-place (digit-reversed) tile position: with >= 2 passes the last pass scatters
 // output r of butterfly i to r * (Ny / R) + i
