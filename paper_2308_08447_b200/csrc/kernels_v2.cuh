@@ -84,10 +84,24 @@ __device__ __forceinline__ CQ<double> ldsq(const CQ<double>* p)
     return r;
 }
 
-// twiddles of one butterfly: w^(lo m), m = 1..R-1, from the pass table [m-1][lo]
+// twiddles of one butterfly: w^(lo m), m = 1..R-1, from the pass table [m-1][lo].
+// Long strides (S >= 64): only w^lo is loaded and the powers are formed by multiplication (depth <= 4, i.e. a few
+// ulp, far inside the tolerances): the full table of a long pass ((R-1) S quads, 57 KB for a 4096-point line) does not
+// stay in L1 next to the tile and was measured to triple the L2 read traffic of the long-line kernels (C4).
 template <int LR, int LS, typename T>
 __device__ __forceinline__ void load_tw(CQ<T>* w, const CQ<T>* __restrict__ tab, int lo)
 {
+    if (LS >= 6 && LR >= 2) {
+        w[1] = ldgq(tab + lo);
+        w[2] = cmul(w[1], w[1]); w[3] = cmul(w[2], w[1]);
+        if (LR >= 3) { w[4] = cmul(w[2], w[2]); w[5] = cmul(w[4], w[1]); w[6] = cmul(w[3], w[3]); w[7] = cmul(w[4], w[3]); }
+        if (LR >= 4) {
+            w[8] = cmul(w[4], w[4]);
+#pragma unroll
+            for (int m = 1; m < 8; ++m) w[8 + m] = cmul(w[8], w[m]);
+        }
+        return;
+    }
 #pragma unroll
     for (int m = 1; m < (1 << LR); ++m) w[m] = ldgq(tab + ((m - 1) << LS) + lo);
 }
