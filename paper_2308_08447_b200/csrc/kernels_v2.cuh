@@ -561,6 +561,14 @@ __global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2,
 //   2 X[k] = A - i w^k D,  2 X[Lc-k] = conj(A + i w^k D),  A = Z[k] + conj Z[Lc-k],  D = Z[k] - conj Z[Lc-k],
 // w = exp(-2 pi i / 2Lc).  The factor 2 is folded into the stored kernel spectrum.
 
+// w^k of the real-transform split, k = 0..Lc/2.  Long rows: w^k = w^(k & ~63) w^(k & 63) from 33 + 64 entries of the
+// table (they stay in L1) instead of one read of a 33 KB table per tile.
+template <int LLC, typename T> __device__ __forceinline__ CQ<T> split_tw(const CQ<T>* __restrict__ twpost, int k)
+{
+    if (LLC < 10) return ldgq(twpost + k);
+    return cmul(ldgq(twpost + (k & ~63)), ldgq(twpost + (k & 63)));
+}
+
 // x R2C FFT fused with the zero padding and the transposition to y-contiguous storage
 // (PAPER.md:35, :296-300 xFFT_R2C; :343 "xy transposition ... to avoid strided y FFTs"):  M -> W1v
 template <typename T, int LLC, int POL, int RP, int NT>
@@ -594,7 +602,7 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
         const int b = t % RP, k = t / RP;
         const CQ<T> Zk = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>(k), b));
         const CQ<T> Zm = ldq(s + tile_addr<PITCH>(pos_of_freq_rt<LLC, POL>((LC - k) & (LC - 1)), b));
-        const CQ<T> w = ldgq(twpost + k);
+        const CQ<T> w = split_tw<LLC>(twpost, k);
         CQ<T> D; D.re = vsub(Zk.re, Zm.re); D.im = vadd(Zk.im, Zm.im);
         const V A = vadd(Zk.re, Zm.re), Bm = vsub(Zk.im, Zm.im);
         const CQ<T> u = cmul(D, w);
@@ -635,7 +643,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
         xki.x = Q0.im.x; xki.y = Q1.im.x; xmi.x = Q0.im.y; xmi.y = Q1.im.y;
         const V Ar = vadd(xkr, xmr), Ai = vsub(xki, xmi);
         CQ<T> D; D.re = vsub(xkr, xmr); D.im = vadd(xki, xmi);
-        const CQ<T> u = cmulc(D, ldgq(twpost + k));
+        const CQ<T> u = cmulc(D, split_tw<LLC>(twpost, k));
         CQ<T> Zk, Zm;
         Zk.re = vsub(Ar, u.im); Zk.im = vadd(Ai, u.re);
         Zm.re = vadd(Ar, u.im); Zm.im = vsub(u.re, Ai);
