@@ -225,6 +225,7 @@ template <int LR, bool INV, bool HALF_IN, typename T> DM_HD void dftR(CQ<T>* a)
 //   POL 1: one leading radix-16 pass when LL % 3 == 1, leading radix 4 when LL % 3 == 2
 //   POL 2: as many radix-16 as the remainder allows: LL%3==1 -> 16,8,..; LL%3==2 -> 16,16,8,.. (LL >= 8)
 //   POL 3: radix 8 passes, remainder, radix 4 LAST (LL >= 4)
+//   POL 5: radix 16 passes, remainder LAST
 struct Sched {
     int n;          // number of passes
     int lr[6];      // log2 radix of each pass
@@ -236,6 +237,9 @@ DM_HDC Sched make_sched(int LL, int POL)
     int rem = LL;
     if (POL == 0) {
         while (rem >= 3) { s.lr[s.n++] = 3; rem -= 3; }
+        if (rem) s.lr[s.n++] = rem;
+    } else if (POL == 5) {          // radix 16 passes, remainder LAST (long x rows: fewest sweeps)
+        while (rem >= 4) { s.lr[s.n++] = 4; rem -= 4; }
         if (rem) s.lr[s.n++] = rem;
     } else if (POL == 3) {          // radix 8 passes, remainder, and a radix-4 LAST pass (small fused z stage)
         rem -= 2;

@@ -16,7 +16,7 @@ template <> struct XCfg<8>  { static constexpr int POL = 2, RP = 8, NT = 128; };
 template <> struct XCfg<9>  { static constexpr int POL = 1, RP = 8, NT = 256; };
 template <> struct XCfg<10> { static constexpr int POL = 1, RP = 4, NT = 256; };
 template <> struct XCfg<11> { static constexpr int POL = 1, RP = 2, NT = 256; };
-template <> struct XCfg<12> { static constexpr int POL = 1, RP = 1, NT = 256; };
+template <> struct XCfg<12> { static constexpr int POL = 5, RP = 1, NT = 256; };   // 16 . 16 . 16
 // y stage (K2v / K4v): radix policy, line pairs per tile, threads
 template <int LNY> struct YCfg { static constexpr int POL = 1, BP = 8, NT = 64; };
 template <> struct YCfg<8>  { static constexpr int POL = 1, BP = 8, NT = 128; };
@@ -58,7 +58,7 @@ inline int x_rp(int lLc)
 {
     switch (lLc) { case 10: return XCfg<10>::RP; case 11: return XCfg<11>::RP; case 12: return XCfg<12>::RP; default: return 8; }
 }
-inline int x_pol(int lLc) { return lLc == 8 ? XCfg<8>::POL : 1; }
+inline int x_pol(int lLc) { return lLc == 8 ? XCfg<8>::POL : lLc == 12 ? XCfg<12>::POL : 1; }
 inline int y_pol(int) { return 1; }
 inline int z_pol(int lNz) { return lNz == 4 ? ZCfg<4>::POL : 1; }
 inline int z_ty(int lNz)
