@@ -15,6 +15,8 @@ Citations are ``PAPER.md:<line>`` (arXiv 2308.08447) or a DESIGN.md reading (R<n
     energy              E = -(mu0/2) V_cell sum M.H (R12)                            [NumPy]
     macrocell_average   Eq. (9) (R13)                              [NumPy]
     macrocell_scatter   "applied equally to all spins" (PAPER.md:133; R14)           [NumPy]
+    dipole_table        point-dipole tensor that turns Eq. (8) into Eq. (1)   [NumPy]
+    dipole_field_eq8    Eq. (8) written out, O(n^2)                [NumPy]
 
 All of them are pinned in tests/test_oracle_pins.py; none is "parity unpinned".
 """
@@ -248,3 +250,42 @@ def macrocell_scatter(H, c) -> np.ndarray:
     """the cell field is applied equally to all spins of the cell (R14)."""
     cx, cy, cz = map(int, c)
     return np.repeat(np.repeat(np.repeat(np.asarray(H), cz, axis=1), cy, axis=2), cx, axis=3)
+
+
+def dipole_table(L, a) -> np.ndarray:
+    """Point-dipole tensor on a simple cubic lattice of constant a over the non-negative offsets, [6][Lz][Ly][Lx]:
+    the kernel that puts the dipole-dipole field of Eq. (8) ("can be re-arranged into the form of
+    Equation (1)") into the form H = -sum_j N(i-j) M_j with M_j = mu_B mu_S S^_j / a^3:
+        N_ab(r) = (a^3 / 4 pi) (delta_ab / r^3 - 3 r_a r_b / r^5),   N(0) = 0 (the sum of Eq. (8) runs over j != i)."""
+    Lx, Ly, Lz = map(int, L)
+    z, y, x = np.meshgrid(np.arange(Lz) * a, np.arange(Ly) * a, np.arange(Lx) * a, indexing="ij")
+    r2 = x * x + y * y + z * z
+    r2[0, 0, 0] = 1.0
+    ir3 = r2 ** -1.5
+    ir5 = r2 ** -2.5
+    f = a ** 3 / (4.0 * np.pi)
+    T = np.stack([f * (ir3 - 3 * x * x * ir5), f * (ir3 - 3 * y * y * ir5), f * (ir3 - 3 * z * z * ir5),
+                  f * (-3 * x * y * ir5), f * (-3 * x * z * ir5), f * (-3 * y * z * ir5)])
+    T[:, 0, 0, 0] = 0.0
+    return T
+
+
+def dipole_field_eq8(S, mu_s, a) -> np.ndarray:
+    """Eq. (8) written out, O(n^2), small lattices only:
+        H_i = (mu_B / 4 pi) sum_{j != i} [3 (S_j . r^_ij) r^_ij - S_j] / r_ij^3,   S_j = mu_S S^_j,
+    r_ij the vector from spin i to spin j.  S: unit spins [3][Lz][Ly][Lx]; result in A/m, same layout."""
+    S = np.asarray(S, dtype=np.float64)
+    _, Lz, Ly, Lx = S.shape
+    z, y, x = np.meshgrid(np.arange(Lz) * a, np.arange(Ly) * a, np.arange(Lx) * a, indexing="ij")
+    pos = np.stack([x.ravel(), y.ravel(), z.ravel()], axis=1)
+    Sv = S.reshape(3, -1).T * mu_s
+    H = np.zeros_like(Sv)
+    for i in range(pos.shape[0]):
+        d = pos - pos[i]
+        r = np.sqrt((d * d).sum(axis=1))
+        r[i] = 1.0
+        rh = d / r[:, None]
+        t = (3.0 * (Sv * rh).sum(axis=1)[:, None] * rh - Sv) / (r ** 3)[:, None]
+        t[i] = 0.0
+        H[i] = MU_B / (4.0 * np.pi) * t.sum(axis=0)
+    return H.T.reshape(3, Lz, Ly, Lx)

@@ -172,6 +172,27 @@ def test_general_mesh_builder_table_energy_atomistic(torch, B, oracle):
         assert np.abs(Hs.cpu().numpy() - Href).max() / np.abs(Mref).max() <= 1e-11
 
 
+# --------------------------------------------------------------------------------- dipole-dipole (Eq. (8))
+@pytest.mark.parametrize("L", [(16, 16, 4), (12, 10, 3), (32, 16, 8)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_dipole_dipole_field_through_set_kernel(torch, B, oracle, L, prec):
+    """NEXT row 2: the atomistic dipole-dipole field of Eq. (8) "re-arranged into the form of
+    Equation (1)": same engine, caller-supplied point-dipole tensor (N(0) = 0), one cell per spin.  Reference =
+    Eq. (8) written out pair by pair on the small lattices, the direct sum of Eq. (1) with that tensor on the larger."""
+    from paper_2308_08447_b200 import workloads as W
+    a, mu_s = 0.3e-9, 2.0
+    Ms = oracle.MU_B * mu_s / a ** 3
+    S = W.random_spins_numpy(L, 21 + sum(L))
+    M = (S.astype(np.float64) * Ms).astype(np.float32)
+    T = oracle.dipole_table(L, a)
+    if np.prod(L) <= 1100:
+        ref = oracle.dipole_field_eq8(M.astype(np.float64) / Ms, mu_s, a)
+    else:
+        ref = oracle.direct_sum(T, M.astype(np.float64))
+    H = run_gpu(torch, B, L, (a, a, a), T, M, prec)
+    assert np.abs(H - ref).max() / Ms <= (TOL32 if prec == 0 else TOL64)
+
+
 # --------------------------------------------------------------------------------- tensor builder
 @pytest.mark.parametrize("n,h", [((64, 32, 4), (2e-9, 2e-9, 1e-9)), ((128, 128, 1), (2e-9, 2e-9, 1e-9)),
                                  ((32, 32, 32), (3e-9, 3e-9, 3e-9)), ((256, 8, 2), (1e-9, 1.5e-9, 0.5e-9))])

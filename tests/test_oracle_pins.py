@@ -312,3 +312,24 @@ def test_macrocell_average_and_scatter(oracle):
     Hs = oracle.macrocell_scatter(M, (4, 2, 2))
     assert Hs.shape == S.shape and np.array_equal(Hs[:, 3, 1, 5], M[:, 1, 0, 1])
     assert np.allclose(oracle.macrocell_average(Hs, (4, 2, 2), 1.0, 1.0) * 16 / oracle.MU_B, M * 16, rtol=1e-13)
+
+
+def test_dipole_tensor_rearranges_eq8_into_eq1(oracle):
+    """"Equation (8) can be re-arranged into the form of Equation (1)".  The rearrangement
+    (oracle.dipole_table + the direct sum of Eq. (1)) against Eq. (8) written out pair by pair; plus what the
+    mathematics fixes for the tensor: zero trace (Laplace), zero self term, the parity of R1, and the far-field limit
+    of the cell-averaged (Newell) tensor of a cube of edge a."""
+    from paper_2308_08447_b200 import workloads as W
+    L, a, mu_s = (6, 5, 3), 0.3e-9, 2.0
+    S = W.random_spins_numpy(L, 5).astype(np.float64)
+    T = oracle.dipole_table(L, a)
+    M = S * (oracle.MU_B * mu_s / a ** 3)
+    H1 = oracle.direct_sum(T, M)
+    H8 = oracle.dipole_field_eq8(S, mu_s, a)
+    assert np.abs(H1 - H8).max() <= 1e-12 * np.abs(H8).max()
+    assert np.abs(T[0] + T[1] + T[2]).max() <= 1e-18 + 1e-15 * np.abs(T).max()
+    assert np.all(T[:, 0, 0, 0] == 0)
+    assert np.all(T[3, :, 0, :] == 0) and np.all(T[3, :, :, 0] == 0)          # xy vanishes on its mirror planes
+    far = oracle.N_at((9 * a, 7 * a, 5 * a), (a, a, a))
+    Tf = oracle.dipole_table((10, 8, 6), a)[:, 5, 7, 9]
+    assert np.abs(far - Tf).max() <= 2e-3 * np.abs(Tf).max()                  # cube -> point dipole, O((a/r)^4)
