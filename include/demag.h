@@ -42,7 +42,8 @@ typedef struct demag_plan_s* demag_plan_t;            /* opaque; owned by the li
 typedef enum {
     DEMAG_OK = 0,
     DEMAG_ERR_INVALID_ARG = 1,   /* NULL / misaligned / aliased pointer, non-positive size          */
-    DEMAG_ERR_UNSUPPORTED = 2,   /* size > 4096, periodic size not a power of two, built-in tensor + PBC */
+    DEMAG_ERR_UNSUPPORTED = 2,   /* size > 4096, periodic size not a power of two, built-in tensor + PBC,
+                                    fp64 with nz > 2048 (an 8192-point fp64 z line exceeds shared memory)   */
     DEMAG_ERR_ALLOC = 3,         /* cudaMalloc / malloc failed                                       */
     DEMAG_ERR_CUDA = 4,          /* a CUDA runtime call or launch failed (see demag_last_error)      */
     DEMAG_ERR_NO_KERNEL = 5      /* demag_apply before demag_set_kernel                              */

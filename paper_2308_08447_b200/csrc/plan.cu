@@ -290,6 +290,12 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         p->v2 = want && !(path && !strcmp(path, "generic")) && pbc_flags == 0 &&
                 v2::supported(nx, ny, nz, g.Nx, g.Ny, g.Nz, g.lLc, g.lNy, g.lNz, p->esz, kMaxSmem);
     }
+    if (!p->v2 && (p->smem1 > kMaxSmem || p->smem2 > kMaxSmem || p->smem3 > kMaxSmem)) {
+        const int worst = std::max(p->smem1, std::max(p->smem2, p->smem3));
+        delete p;
+        return fail(DEMAG_ERR_UNSUPPORTED, "a transform line of this plan needs %d bytes of shared memory (limit %d): "
+                    "8192-point z lines are fp32 only", worst, kMaxSmem);
+    }
     if (p->v2) {
         v2::GeoV gv;
         gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz;

@@ -87,6 +87,29 @@ def test_shapes_against_oracle(torch, B, oracle, n, prec):
     assert err <= (TOL32 if prec == 0 else TOL64), err
 
 
+@pytest.mark.parametrize("n", [(16, 16, 2048), (4, 4, 4096), (4096, 4, 1), (2, 4096, 2)])
+def test_maximum_axis_lengths(torch, B, oracle, n):
+    """The longest transforms the library accepts (n_a = 4096 -> N_a = 8192) on every axis, incl. the z lengths beyond
+    the fast family's range (size-generic kernels); full field against the NumPy-FFT cross-check O-C, which is itself
+    checked against Eq. (1) at sampled cells."""
+    from paper_2308_08447_b200 import workloads as W
+    h, Ms = (2e-9, 3e-9, 1e-9), 8e5
+    M = rand_M(n, Ms, 900 + sum(n))
+    T = oracle.tensor_table(n, h)
+    ref = oracle.fft_conv(T, M.astype(np.float64))
+    cells = W.sample_cells(n, 32, 3)
+    Hs = oracle.direct_sum_sampled(T, M.astype(np.float64), cells)
+    assert np.abs(ref.reshape(3, -1)[:, cells].T - Hs).max() / Ms < 1e-12
+    for prec in (0, 1):
+        if prec == 1 and n[2] == 4096:           # an 8192-point fp64 z line does not fit in shared memory: refused
+            with pytest.raises(B.DemagError) as e:
+                B.demag_plan_create(*n, *h, 0, 1)
+            assert e.value.status == 2
+            continue
+        H = run_gpu(torch, B, n, h, T, M, prec)
+        assert np.abs(H - ref).max() / Ms <= (TOL32 if prec == 0 else TOL64)
+
+
 @pytest.mark.parametrize("slab", [1, 3, 7])
 def test_slab_size_does_not_change_result(torch, B, oracle, slab):
     n, h = (32, 16, 8), (2e-9, 2e-9, 2e-9)
