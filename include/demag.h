@@ -66,7 +66,9 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz,
  *   N6_host != NULL: host array double[6][nz][ny][nx]: N_c at the non-negative cell offsets
  *                    (dx,dy,dz); negative offsets follow by parity (diagonal even; xy odd in x,y;
  *                    xz odd in x,z; yz odd in y,z).  On a PBC axis the n_a entries are the periodic
- *                    kernel at offsets 0..n_a-1 (no parity folding on that axis).
+ *                    kernel at offsets 0..n_a-1 (no parity folding on that axis); a periodic kernel obeys
+ *                    K(n_a - d) = parity * K(d) there, and only that symmetric part of the table is used
+ *                    (the stored spectrum is real).
  * The spectrum is computed in fp64, the factor -1/(Nx Ny Nz) is folded in (R3), and it is
  * rounded once to fp32 (kept fp64 for a DEMAG_FP64 plan).  Synchronous (plan-time call). */
 demag_status demag_set_kernel(demag_plan_t plan, const double* N6_host);

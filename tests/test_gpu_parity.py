@@ -195,6 +195,78 @@ def test_general_mesh_builder_table_energy_atomistic(torch, B, oracle):
         assert np.abs(Hs.cpu().numpy() - Href).max() / np.abs(Mref).max() <= 1e-11
 
 
+# --------------------------------------------------------------------------------- periodic axes (caller's kernel)
+def _periodic_table(oracle, n, h, pbc, images=2):
+    """Caller-side periodic kernel ("modified convolution kernel"; R11): the open-boundary tensor
+    summed over `images` periodic images on each side along the periodic axes, at offsets 0 <= d_a < n_a."""
+    nx, ny, nz = n
+    T = np.zeros((6, nz, ny, nx))
+    rng = [range(-images, images + 1) if p else range(1) for p in pbc]
+    for dz in range(nz):
+        for dy in range(ny):
+            for dx in range(nx):
+                acc = np.zeros(6)
+                for mx in rng[0]:
+                    for my in rng[1]:
+                        for mz in rng[2]:
+                            acc += oracle.N_at(((dx + mx * nx) * h[0], (dy + my * ny) * h[1], (dz + mz * nz) * h[2]), h)
+                T[:, dz, dy, dx] = acc
+    # a periodic kernel obeys K(n_a - d) = parity * K(d) on its periodic axes (include/demag.h); the truncated image sum
+    # does so only up to its last images: symmetrise it
+    for a, ax in ((0, 3), (1, 2), (2, 1)):
+        if pbc[a]:
+            idx = (-np.arange(n[a])) % n[a]
+            par = oracle.PARITY[:, a].reshape(6, 1, 1, 1)
+            T = 0.5 * (T + par * np.take(T, idx, axis=ax))
+    return T
+
+
+def _periodic_direct(oracle, T, M, pbc):
+    """H_i = -sum_j K(i - j) M_j with the offset wrapped on periodic axes and reflected (parity of R1) on open ones."""
+    PAR, COMP = oracle.PARITY, oracle.COMP
+    _, nz, ny, nx = M.shape
+    n = (nx, ny, nz)
+    H = np.zeros_like(M)
+    cells = [(x, y, z) for z in range(nz) for y in range(ny) for x in range(nx)]
+    for (ix, iy, iz) in cells:
+        for (jx, jy, jz) in cells:
+            d = [ix - jx, iy - jy, iz - jz]
+            sg = np.ones(6)
+            for a in range(3):
+                if pbc[a]:
+                    d[a] %= n[a]
+                elif d[a] < 0:
+                    d[a] = -d[a]; sg = sg * PAR[:, a]
+            k = T[:, d[2], d[1], d[0]] * sg
+            for a in range(3):
+                H[a, iz, iy, ix] -= sum(k[COMP[a, b]] * M[b, jz, jy, jx] for b in range(3))
+    return H
+
+
+@pytest.mark.parametrize("n,pbc", [((8, 4, 2), (True, False, False)), ((4, 8, 2), (False, True, False)),
+                                   ((8, 8, 1), (True, True, False)), ((4, 2, 8), (False, False, True))])
+def test_periodic_axes_with_callers_kernel(torch, B, oracle, n, pbc):
+    """pbc_flags: a periodic axis is not padded and the caller's table is taken as the periodic kernel on
+    it.  Reference = the wrapped direct sum written out here, cross-checked with the oracle's naive-DFT convolution on
+    the unpadded axis."""
+    h, Ms = (2e-9, 3e-9, 1e-9), 8e5
+    T = _periodic_table(oracle, n, h, pbc)
+    M = rand_M(n, Ms, 40 + sum(n)).astype(np.float64)
+    ref = _periodic_direct(oracle, T, M, pbc)
+    P = tuple(na if (p or na == 1) else 2 * na for na, p in zip(n, pbc))
+    assert np.abs(oracle.naive_dft_conv(T, M, P) - ref).max() / Ms < 1e-12
+    flags = sum(f for f, p in zip((B.DEMAG_PBC_X, B.DEMAG_PBC_Y, B.DEMAG_PBC_Z), pbc) if p)
+    for prec, tol in ((0, TOL32), (1, TOL64)):
+        dt = torch.float32 if prec == 0 else torch.float64
+        with B.Plan(n, h, flags, prec) as p:
+            p.set_kernel(T)
+            Md = torch.from_numpy(M).to("cuda", dt); Hd = torch.empty_like(Md)
+            p.apply(Md, Hd); torch.cuda.synchronize()
+            Mq = Md.cpu().numpy().astype(np.float64)
+            refq = ref if prec == 1 else _periodic_direct(oracle, T, Mq, pbc)
+            assert np.abs(Hd.cpu().numpy().astype(np.float64) - refq).max() / Ms <= tol
+
+
 # --------------------------------------------------------------------------------- dipole-dipole (Eq. (8))
 @pytest.mark.parametrize("L", [(16, 16, 4), (12, 10, 3), (32, 16, 8)])
 @pytest.mark.parametrize("prec", [0, 1])
