@@ -78,6 +78,11 @@ demag_status demag_set_kernel(demag_plan_t plan, const double* N6_host);
  * M is not modified; H is overwritten.  DEMAG_ERR_NO_KERNEL before demag_set_kernel. */
 demag_status demag_apply(demag_plan_t plan, const void* M_dev, void* H_dev, void* cuda_stream);
 
+/* H_eff += -N * M: the same convolution, ADDED into an existing effective-field array (the demagnetizing
+ * field is one contribution to H_eff) inside the last kernel, so the integrator needs no extra pass over H.
+ * Same arguments, layout and errors as demag_apply; Heff_dev is read and written. */
+demag_status demag_apply_add(demag_plan_t plan, const void* M_dev, void* Heff_dev, void* cuda_stream);
+
 /* Demagnetizing energy  E = -(mu0/2) hx hy hz sum_i M_i . H_i  [J] (R12), accumulated in
  * fp64 and written to the device scalar *E_dev (double).  Asynchronous on the stream. */
 demag_status demag_energy(demag_plan_t plan, const void* M_dev, const void* H_dev,

@@ -21,7 +21,7 @@ STATUS = {0: "DEMAG_OK", 1: "DEMAG_ERR_INVALID_ARG", 2: "DEMAG_ERR_UNSUPPORTED",
 
 EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy", "demag_apply_atomistic",
            "demag_get_kernel_real", "demag_workspace_bytes", "demag_set_slab", "demag_launches_per_apply",
-           "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path"]
+           "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path", "demag_apply_add"]
 
 
 class DemagError(RuntimeError):
@@ -45,6 +45,7 @@ def lib():
         L.demag_plan_create.argtypes = [ctypes.POINTER(vp), i, i, i, d, d, d, u, i]
         L.demag_set_kernel.argtypes = [vp, vp]
         L.demag_apply.argtypes = [vp, vp, vp, vp]
+        L.demag_apply_add.argtypes = [vp, vp, vp, vp]
         L.demag_energy.argtypes = [vp, vp, vp, vp, vp]
         L.demag_apply_profiled.argtypes = [vp, vp, vp, vp, vp, vp]
         L.demag_apply_atomistic.argtypes = [vp, vp, vp, i, i, i, d, d, i, vp]
@@ -94,6 +95,10 @@ def demag_set_kernel(plan, N6_host=None):
 
 def demag_apply(plan, M, H, stream=None):
     _check(lib().demag_apply(plan, M.data_ptr(), H.data_ptr(), _stream(stream)))
+
+
+def demag_apply_add(plan, M, Heff, stream=None):
+    _check(lib().demag_apply_add(plan, M.data_ptr(), Heff.data_ptr(), _stream(stream)))
 
 
 def demag_apply_profiled(plan, M, H, stream=None):
@@ -154,6 +159,9 @@ class Plan:
 
     def apply(self, M, H, stream=None):
         demag_apply(self.handle, M, H, stream)
+
+    def apply_add(self, M, Heff, stream=None):
+        demag_apply_add(self.handle, M, Heff, stream)
 
     def apply_profiled(self, M, H, stream=None):
         return demag_apply_profiled(self.handle, M, H, stream)

@@ -21,6 +21,7 @@ struct Geo {
     int hx;                // Nx/2 + 1 (1 if Nx == 1)
     int lLc, lNy, lNz;     // log2(Nx/2), log2(Ny), log2(Nz)
     int kpy, kpz, kpitch;  // packed kernel extents along y, z and the row pitch (elements)
+    int acc;               // x C2R: 0 = overwrite H, 1 = add into H (demag_apply_add)
 };
 
 
@@ -77,10 +78,10 @@ __global__ void k_x_copy_fwd(size_t n, const T* __restrict__ M, typename cx_of<T
         W1[i] = cmake<C>(M[i], (T)0);
 }
 template <typename T>
-__global__ void k_x_copy_inv(size_t n, const typename cx_of<T>::type* __restrict__ W1, T* __restrict__ H)
+__global__ void k_x_copy_inv(size_t n, const typename cx_of<T>::type* __restrict__ W1, T* __restrict__ H, int acc)
 {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
-        H[i] = W1[i].x;
+        H[i] = acc ? H[i] + W1[i].x : W1[i].x;
 }
 
 // ------------------------------------------------------------------------------------------ K5
@@ -119,7 +120,10 @@ __global__ void __launch_bounds__(512) k_x_c2r(Geo g, int R, int pitch, const ty
     const size_t rowbase = ((size_t)cz * g.ny + y0) * g.nx;
     for (int idx = tid; idx < R * nout; idx += nthr) {
         const int b = idx >> lno, m = idx & (nout - 1);
-        *reinterpret_cast<C*>(H + rowbase + (size_t)b * g.nx + 2 * m) = s[taddr<SWZ, RB>(m * pitch + b)];
+        C v = s[taddr<SWZ, RB>(m * pitch + b)];
+        C* d = reinterpret_cast<C*>(H + rowbase + (size_t)b * g.nx + 2 * m);
+        if (g.acc) { const C o = *d; v.x += o.x; v.y += o.y; }
+        *d = v;
     }
 }
 

@@ -141,7 +141,12 @@ __global__ void __launch_bounds__(512) k_x_c2r_f(Geo g, int R, int pitch, const 
     fft_mid<T, true>(s, g.lLc, R, pitch, twx, 1, tid, nthr);
     T* rows = H + ((size_t)cz * g.ny + y0) * g.nx;
     const int nx = g.nx;
-    auto stf = [&](int b, int m, C v) { *reinterpret_cast<C*>(rows + (size_t)b * nx + 2 * m) = v; };
+    const int acc = g.acc;
+    auto stf = [&](int b, int m, C v) {
+        C* d = reinterpret_cast<C*>(rows + (size_t)b * nx + 2 * m);
+        if (acc) { const C o = *d; v.x += o.x; v.y += o.y; }
+        *d = v;
+    };
     pass_last_inv<T>(s, g.lLc, R, pitch, twx, 1, tid, nthr, g.Nx != g.nx, stf);
 }
 

@@ -29,6 +29,7 @@ struct GeoV {
     int Lc;              // complex length of the packed real x transform = nx (Nx = 2 nx)
     int hq;              // number of (k, Lc-k) pairs = Lc/2 + 1
     int kpz;             // Nz/2 + 1
+    int acc;             // x C2R: 0 = overwrite H, 1 = add into H (demag_apply_add)
 };
 
 template <typename T> struct TwSet { const CQ<T>* p[6]; };   // per-pass twiddle tables (NULL for stride-1 passes)
@@ -652,12 +653,14 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     }
     __syncthreads();
     InvPasses<T, LLC, POL, 1, SC.n, RP, PITCH, NT>::run(s, tw, tid);
-    const int nx = g.nx;
+    const int nx = g.nx, acc = g.acc;
     T* rows = H + ((size_t)cz * g.ny + y0) * nx;
     auto st = [&](int b, int m, CQ<T> v) {
         V r0, r1; r0.x = v.re.x; r0.y = v.im.x; r1.x = v.re.y; r1.y = v.im.y;
-        *reinterpret_cast<V*>(rows + (size_t)(2 * b) * nx + 2 * m) = r0;
-        *reinterpret_cast<V*>(rows + (size_t)(2 * b + 1) * nx + 2 * m) = r1;
+        V* d0 = reinterpret_cast<V*>(rows + (size_t)(2 * b) * nx + 2 * m);
+        V* d1 = reinterpret_cast<V*>(rows + (size_t)(2 * b + 1) * nx + 2 * m);
+        if (acc) { const V o0 = *d0, o1 = *d1; r0.x += o0.x; r0.y += o0.y; r1.x += o1.x; r1.y += o1.y; }
+        *d0 = r0; *d1 = r1;
     };
     pass_last<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, st);
 }

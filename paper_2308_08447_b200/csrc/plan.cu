@@ -298,7 +298,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
     }
     if (p->v2) {
         v2::GeoV gv;
-        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz;
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0;
         p->cf.g = gv; p->cd.g = gv;
         {   // one-cell-thick mesh: y FFT . multiply . y IFFT fused in one kernel, in place on W1 (scope row a3')
             const bool film = v2::film_supported(nz, g.Nz, g.lNy, p->esz, kMaxSmem) && !getenv("DEMAG_NO_FILM");
@@ -610,10 +610,11 @@ template <> const v2::Ctx<float>& v2_ctx<float>(const demag_plan_s* p) { return 
 template <> const v2::Ctx<double>& v2_ctx<double>(const demag_plan_s* p) { return p->cd; }
 
 template <typename T>
-demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr)
+demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr, int acc = 0)
 {
     using C = typename cx_of<T>::type;
     const Geo& g = p->g;
+    Geo ga = g; ga.acc = acc;                       // the x C2R kernels add into H when asked (demag_apply_add)
     C* W1 = (C*)p->W1; C* W2 = (C*)p->W2;
     const C* twx = (const C*)p->tw[0]; const C* twy = (const C*)p->tw[1]; const C* twz = (const C*)p->tw[2];
     const size_t nc = (size_t)g.nx * g.ny * g.nz;
@@ -630,7 +631,7 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
             STAGE(2, (v2::z_mul<T>(1, cx, st, q0, nq, V2, Kv, &verr)));
             STAGE(3, (v2::y_inv<T>(1, cx, st, q0, nq, V2, V1, &verr)));
         }
-        STAGE(4, (v2::x_inv<T>(1, cx, st, V1, H, &verr)));
+        STAGE(4, (v2::x_inv<T>(1, cx, st, V1, H, &verr, acc)));
         CUDA_TRY(cudaGetLastError());
         return DEMAG_OK;
     }
@@ -662,11 +663,11 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
     }
     if (g.Nx == 1) {
         const unsigned grid = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)p->sm_count * 16);
-        STAGE(4, (k_x_copy_inv<T><<<grid, 256, 0, st>>>(3 * nc, W1, H)));
+        STAGE(4, (k_x_copy_inv<T><<<grid, 256, 0, st>>>(3 * nc, W1, H, acc)));
     } else {
-        if (p->fast1) STAGE(4, (k_x_c2r_f<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, W1, H, twx)));
-        else if (p->pitch1 == 1) STAGE(4, (k_x_c2r<T, true><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, W1, H, twx)));
-        else STAGE(4, (k_x_c2r<T, false><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(g, p->R1, p->pitch1, W1, H, twx)));
+        if (p->fast1) STAGE(4, (k_x_c2r_f<T><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(ga, p->R1, p->pitch1, W1, H, twx)));
+        else if (p->pitch1 == 1) STAGE(4, (k_x_c2r<T, true><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(ga, p->R1, p->pitch1, W1, H, twx)));
+        else STAGE(4, (k_x_c2r<T, false><<<3u * g.nz * (g.ny / p->R1), p->thr1, p->smem1, st>>>(ga, p->R1, p->pitch1, W1, H, twx)));
     }
     CUDA_TRY(cudaGetLastError());
     return DEMAG_OK;
@@ -683,25 +684,25 @@ __global__ void __launch_bounds__(256) k_embed(int onx, int ony, int onz, int nx
     for (int x = blockIdx.x * 256 + threadIdx.x; x < nx; x += gridDim.x * 256) dst[x] = (in && x < onx) ? src[x] : (T)0;
 }
 template <typename T>
-__global__ void __launch_bounds__(256) k_crop(int onx, int ony, int onz, int nx, int ny, int nz, const T* __restrict__ Hp, T* __restrict__ H)
+__global__ void __launch_bounds__(256) k_crop(int onx, int ony, int onz, int nx, int ny, int nz, const T* __restrict__ Hp, T* __restrict__ H, int acc)
 {
     const int y = blockIdx.y, cz = blockIdx.z, c = cz / onz, z = cz - c * onz;
     const T* src = Hp + (((size_t)c * nz + z) * ny + y) * nx;
     T* dst = H + (((size_t)c * onz + z) * ony + y) * onx;
-    for (int x = blockIdx.x * 256 + threadIdx.x; x < onx; x += gridDim.x * 256) dst[x] = src[x];
+    for (int x = blockIdx.x * 256 + threadIdx.x; x < onx; x += gridDim.x * 256) dst[x] = acc ? dst[x] + src[x] : src[x];
 }
 // demag_apply on the caller's mesh
 template <typename T>
-demag_status apply_outer(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr)
+demag_status apply_outer(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr, int acc = 0)
 {
-    if (!p->embed) return apply_impl<T>(p, M, H, st, tm);
+    if (!p->embed) return apply_impl<T>(p, M, H, st, tm, acc);
     const Geo& g = p->g;
     k_embed<T><<<dim3((unsigned)((g.nx + 255) / 256), (unsigned)g.ny, (unsigned)(3 * g.nz)), 256, 0, st>>>(
         p->on[0], p->on[1], p->on[2], g.nx, g.ny, g.nz, M, (T*)p->Mp);
     demag_status s = apply_impl<T>(p, (const T*)p->Mp, (T*)p->Hp, st, tm);
     if (s) return s;
     k_crop<T><<<dim3((unsigned)((p->on[0] + 255) / 256), (unsigned)p->on[1], (unsigned)(3 * p->on[2])), 256, 0, st>>>(
-        p->on[0], p->on[1], p->on[2], g.nx, g.ny, g.nz, (const T*)p->Hp, H);
+        p->on[0], p->on[1], p->on[2], g.nx, g.ny, g.nz, (const T*)p->Hp, H, acc);
     CUDA_TRY(cudaGetLastError());
     return DEMAG_OK;
 }
@@ -729,6 +730,19 @@ extern "C" demag_status demag_apply(demag_plan_t p, const void* M_dev, void* H_d
     cudaStream_t st = (cudaStream_t)cuda_stream;
     return p->prec == DEMAG_FP32 ? apply_outer<float>(p, (const float*)M_dev, (float*)H_dev, st)
                                  : apply_outer<double>(p, (const double*)M_dev, (double*)H_dev, st);
+}
+
+extern "C" demag_status demag_apply_add(demag_plan_t p, const void* M_dev, void* Heff_dev, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    const size_t bytes = (size_t)3 * p->on[0] * p->on[1] * p->on[2] * p->esz;
+    demag_status s = check_apply_args(p, M_dev, Heff_dev, bytes);
+    if (s) return s;
+    if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return p->prec == DEMAG_FP32 ? apply_outer<float>(p, (const float*)M_dev, (float*)Heff_dev, st, nullptr, 1)
+                                 : apply_outer<double>(p, (const double*)M_dev, (double*)Heff_dev, st, nullptr, 1);
 }
 
 extern "C" demag_status demag_apply_profiled(demag_plan_t p, const void* M_dev, void* H_dev, void* cuda_stream,

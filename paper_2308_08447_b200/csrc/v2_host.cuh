@@ -221,14 +221,15 @@ bool x_fwd(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cu
     }
 }
 template <typename T>
-bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cudaError_t* err)
+bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cudaError_t* err, int acc = 0)
 {
+    GeoV ga = c.g; ga.acc = acc;
     switch (c.lLc) {
-        V2_CASE_X(4, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(5, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
-        V2_CASE_X(6, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(7, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
-        V2_CASE_X(8, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(9, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
-        V2_CASE_X(10, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost) V2_CASE_X(11, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
-        V2_CASE_X(12, k_x_c2r_v, c.g, W1, H, c.twx, c.twpost)
+        V2_CASE_X(4, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(5, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
+        V2_CASE_X(6, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(7, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
+        V2_CASE_X(8, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(9, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
+        V2_CASE_X(10, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(11, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
+        V2_CASE_X(12, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
     default: return false;
     }
 }

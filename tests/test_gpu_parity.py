@@ -288,6 +288,30 @@ def test_dipole_dipole_field_through_set_kernel(torch, B, oracle, L, prec):
     assert np.abs(H - ref).max() / Ms <= (TOL32 if prec == 0 else TOL64)
 
 
+# --------------------------------------------------------------------------------- accumulate into H_eff
+@pytest.mark.parametrize("n", [(32, 16, 8), (64, 32, 1), (12, 10, 3), (1, 8, 4), (4, 4, 2)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_apply_add_accumulates_into_heff(torch, B, oracle, n, prec):
+    """demag_apply_add: H_eff <- H_eff + H_d in the last kernel (both kernel families, film, embedded and 1-cell-wide
+    meshes): equal to demag_apply's field added to the same start array, to rounding."""
+    h, Ms = (2e-9, 3e-9, 1e-9), 8e5
+    dt = torch.float32 if prec == 0 else torch.float64
+    M = rand_M(n, Ms, 70 + sum(n))
+    T = oracle.tensor_table(n, h)
+    with B.Plan(n, h, 0, prec) as p:
+        p.set_kernel(T)
+        Md = torch.from_numpy(M).to("cuda", dt)
+        Hd = torch.empty_like(Md)
+        H0 = torch.randn_like(Md) * Ms
+        Heff = H0.clone()
+        p.apply(Md, Hd); p.apply_add(Md, Heff); torch.cuda.synchronize()
+        want = (H0.double() + Hd.double()).cpu().numpy()
+        got = Heff.double().cpu().numpy()
+        assert np.abs(got - want).max() / Ms <= (4e-7 if prec == 0 else 1e-15)
+        ref = oracle.direct_sum(T, M.astype(np.float64))
+        assert np.abs(got - H0.double().cpu().numpy() - ref).max() / Ms <= (TOL32 if prec == 0 else TOL64)
+
+
 # --------------------------------------------------------------------------------- tensor builder
 @pytest.mark.parametrize("n,h", [((64, 32, 4), (2e-9, 2e-9, 1e-9)), ((128, 128, 1), (2e-9, 2e-9, 1e-9)),
                                  ((32, 32, 32), (3e-9, 3e-9, 3e-9)), ((256, 8, 2), (1e-9, 1.5e-9, 0.5e-9))])
