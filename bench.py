@@ -437,7 +437,7 @@ def run_ours(args, cfg, fp64):
         line["cufft"] = cufft
     if atom:
         line["spins_per_s_G"] = world * units * args.steps / (ms_total * 1e-3) / 1e9
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json.txt")
     try:
         tr = json.load(open(traffic_file)).get(args.config, {}).get(STAGE_NAMES[dom])
         if tr:
