@@ -113,7 +113,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100", "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "20", "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
@@ -176,7 +176,8 @@ def stage_bytes(n, esz):
     return [3 * nc * esz + w1, w1 + w2, w2 + kern + w2, w2 + w1, w1 + 3 * nc * esz]
 
 
-STAGE_NAMES = ["k_x_r2c", "k_y_fwd", "k_z_mul", "k_y_inv", "k_x_c2r"]
+STAGE_NAMES = ["k_x_r2c", "k_y_fwd", "k_z_mul", "k_y_inv", "k_x_c2r"]                 # size-generic kernel family
+STAGE_NAMES_FAST = ["k_x_r2c_v", "k_y_fwd_v", "k_z_v", "k_y_inv_v", "k_x_c2r_v"]     # compile-time specialised family
 
 
 def cufft_baseline(torch, n, dt, dev, reps=10):
@@ -401,6 +402,7 @@ def run_ours(args, cfg, fp64):
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     sb = stage_bytes(n, esz)
+    names = STAGE_NAMES_FAST if plan.path() == 1 else STAGE_NAMES
     dom = int(np.argmax(st_ms))
     achieved = sb[dom] / (st_ms[dom] * 1e-3) / 1e9
     value = aggregate_throughput(world, nc, args.steps, ms_total) / 1e9
@@ -420,11 +422,11 @@ def run_ours(args, cfg, fp64):
         "gpu_launches": launches_per_step * args.steps,
         "launches_per_step": launches_per_step,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": STAGE_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                      "bytes_per_apply_model": sb[dom], "ms_per_apply": float(st_ms[dom]),
                      "launches_per_apply": int(st_n[dom] // reps)},
-        "stages": {STAGE_NAMES[i]: {"ms": float(st_ms[i]), "model_bytes": sb[i],
+        "stages": {names[i]: {"ms": float(st_ms[i]), "model_bytes": sb[i],
                                     "model_GBps": sb[i] / max(st_ms[i], 1e-9) / 1e6} for i in range(5)},
         "whole_apply_model": {"T2_5pass_bytes": sum(sb), "T2_GBps": sum(sb) / (ms_total / args.steps) / 1e6,
                               "frac_of_peak": sum(sb) / (ms_total / args.steps) / 1e6 / peak},
@@ -439,7 +441,7 @@ def run_ours(args, cfg, fp64):
         line["spins_per_s_G"] = world * units * args.steps / (ms_total * 1e-3) / 1e9
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json.txt")
     try:
-        tr = json.load(open(traffic_file)).get(args.config, {}).get(STAGE_NAMES[dom])
+        tr = json.load(open(traffic_file)).get(args.config, {}).get(names[dom])
         if tr:
             line["roofline"]["traffic"] = tr
     except Exception:
