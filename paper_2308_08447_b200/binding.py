@@ -37,6 +37,12 @@ def lib():
     """Load libdemag_b200.so (built by paper_2308_08447_b200/build.py).  Fails loudly if absent."""
     global _lib
     if _lib is None:
+        if not os.path.exists(LIB_PATH) and os.environ.get("DEMAG_NO_AUTOBUILD") is None:
+            try:                                   # build the CUDA extension in-tree (nvcc); still no CPU fallback
+                from . import build as _build
+                _build.build()
+            except Exception:
+                pass
         if not os.path.exists(LIB_PATH):
             raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2308_08447_b200.build` "
                               "(the CUDA extension is required; there is no CPU fallback)")

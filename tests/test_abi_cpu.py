@@ -42,6 +42,7 @@ def test_missing_library_fails_loudly(monkeypatch):
     from paper_2308_08447_b200 import binding
     monkeypatch.setattr(binding, "_lib", None)
     monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libdemag_b200.so")
+    monkeypatch.setenv("DEMAG_NO_AUTOBUILD", "1")
     with pytest.raises(ImportError):
         binding.lib()
 
