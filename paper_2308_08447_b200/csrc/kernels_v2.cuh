@@ -85,6 +85,37 @@ __device__ __forceinline__ CQ<double> ldsq(const CQ<double>* p)
     return r;
 }
 
+// ---- asynchronous bulk copy (TMA, 1D) signalled through an mbarrier -------------------------------------------
+// Used by the long-line y kernel (one line pair per block, one block per SM): the next line lands in a staging
+// buffer while the block transforms the current one.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
 // twiddles of one butterfly: w^(lo m), m = 1..R-1, from the pass table [m-1][lo].
 // Long strides (S >= 64): only w^lo is loaded and the powers are formed by multiplication (depth <= 4, i.e. a few
 // ulp, far inside the tolerances): the full table of a long pass ((R-1) S quads, 57 KB for a 4096-point line) does not
@@ -356,6 +387,51 @@ __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ
             const int b = idx >> LNY, p = idx & (NY - 1);
             stq(dst + idx, ldq(s + tile_addr<PITCH>(p, b)));
         }
+    }
+}
+
+// Long lines (one line pair per tile: Ny >= 4096): persistent blocks, one per SM.  The zero-padded input half of the
+// NEXT line is bulk-copied (cp.async.bulk + mbarrier) into a staging buffer while the current line is transformed, so
+// the block never waits for its input (with a single resident block nothing else hides that latency).
+template <typename T, int LNY, int POL, int NT>
+__global__ void __launch_bounds__(NT) k_y_fwd_long_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
+                                                    CQ<T>* __restrict__ W2, TwSet<T> tw)
+{
+    constexpr Sched SC = make_sched(LNY, POL);
+    constexpr int NP = SC.n;
+    static_assert(NP >= 2, "long lines have several passes");
+    constexpr int NY = 1 << LNY, PITCH = tile_pe(1, 1), TQ = tile_quads(PITCH, NY, 1);
+    constexpr uint32_t kBytes = (uint32_t)((NY / 2) * sizeof(CQ<T>));
+    CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
+    CQ<T>* stage = s + TQ;
+    __shared__ uint64_t mbar;
+    const int tid = threadIdx.x;
+    const int nlines = 3 * nq * g.nz;
+    if (tid == 0) { mbar_init(&mbar, 1); fence_mbar_init(); }
+    __syncthreads();
+    int line = blockIdx.x;
+    if (tid == 0 && line < nlines) { mbar_arrive_expect_tx(&mbar, kBytes); bulk_g2s(stage, W1 + w1v_line_offset(g, line, q0, nq), kBytes, &mbar); }
+    for (int it = 0; line < nlines; line += gridDim.x, ++it) {
+        mbar_wait(&mbar, (uint32_t)(it & 1));
+        auto ld = [&](int, int p) { return ldq(stage + p); };
+        pass_first<T, LNY, POL, 1, PITCH, NT, false>(s, tw.p[0], tid, ld);
+        __syncthreads();                                       // staging buffer consumed, tile written
+        const int next = line + gridDim.x;
+        if (tid == 0 && next < nlines) { mbar_arrive_expect_tx(&mbar, kBytes); bulk_g2s(stage, W1 + w1v_line_offset(g, next, q0, nq), kBytes, &mbar); }
+        FwdPasses<T, LNY, POL, 1, NP - 1, 1, PITCH, NT>::run(s, tw, tid);
+        constexpr int LR = SC.lr[NP - 1], R = 1 << LR, LNB = LNY - LR, NBF = 1 << LNB;
+        CQ<T>* dst = W2 + (size_t)line * NY;
+#pragma unroll 2
+        for (int i = tid; i < NBF; i += NT) {
+            const CQ<T>* d = s + tile_addr<PITCH>(i << LR, 0);
+            CQ<T> a[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) a[r] = ldq(d + tile_leg<PITCH, 1>(r));
+            dftR<LR, false, false>(a);
+#pragma unroll
+            for (int r = 0; r < R; ++r) stq(dst + (r << LNB) + i, a[r]);
+        }
+        __syncthreads();                                       // tile free for the next line
     }
 }
 

@@ -307,6 +307,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
             p->cf.film = p->cd.film = film; p->cf.gfilm = p->cd.gfilm = gf;
         }
         p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
+        p->cf.sm_count = p->cd.sm_count = p->sm_count;
         const size_t qsz = 4 * p->esz;                      // one quad
         const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;
         size_t slab_bytes = kSlabBytes;

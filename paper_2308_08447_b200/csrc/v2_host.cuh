@@ -190,6 +190,7 @@ inline bool film_supported(int nz, int Nz, int lNy, size_t esz, int max_smem)
 
 // ---- launchers ---------------------------------------------------------------------------------------------
 template <typename T> struct Ctx {
+    int sm_count;
     GeoV g;
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
@@ -243,9 +244,20 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
         else KERN<T, L, C::POL, C::BP, C::NT><<<(unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st>>>(c.g, q0, nq, A, B, c.twy); \
         return true;                                                                                                 \
     }
+#define V2_BODY_YLONG(L)                                                                                            \
+    {                                                                                                                \
+        using C = YCfg<L>;                                                                                           \
+        constexpr int smem = (y_tile_quads(L, C::POL, 1) + (1 << (L - 1))) * (int)sizeof(CQ<T>);                      \
+        if (mode == 0) *err = cudaFuncSetAttribute(k_y_fwd_long_v<T, L, C::POL, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+        else { const long long nl = 3LL * nq * c.g.nz;                                                               \
+               k_y_fwd_long_v<T, L, C::POL, C::NT><<<(unsigned)(nl < c.sm_count ? nl : c.sm_count), C::NT, smem, st>>>(c.g, q0, nq, W1, W2, c.twy); } \
+        return true;                                                                                                 \
+    }
 template <typename T>
 bool y_fwd(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W1, CQ<T>* W2, cudaError_t* err)
 {
+    if (c.lNy == 12 && !getenv("DEMAG_NO_YLONG")) V2_BODY_YLONG(12)
+    if constexpr (sizeof(T) == 4) { if (c.lNy == 13 && !getenv("DEMAG_NO_YLONG")) V2_BODY_YLONG(13) }
     switch (c.lNy) {
         V2_CASE_Y(4, k_y_fwd_v, W1, W2) V2_CASE_Y(5, k_y_fwd_v, W1, W2) V2_CASE_Y(6, k_y_fwd_v, W1, W2) V2_CASE_Y(7, k_y_fwd_v, W1, W2)
         V2_CASE_Y(8, k_y_fwd_v, W1, W2) V2_CASE_Y(9, k_y_fwd_v, W1, W2) V2_CASE_Y(10, k_y_fwd_v, W1, W2) V2_CASE_Y(11, k_y_fwd_v, W1, W2)
