@@ -127,6 +127,72 @@ int demag_launches_per_apply(demag_plan_t plan);
  * (used by the tests to cover both families in both precisions). */
 int demag_path(demag_plan_t plan);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * Several GPUs, one process (rank) per GPU: the paper's multi-GPU convolution (Fig. 1; Appendix A,
+ * PAPER.md:261-341), DESIGN.md 8.
+ *
+ * Partitioning.  The paper splits M / H along x and needs four transfers per convolution (M->In, S1->S2, S2->S1,
+ * Out->H).  Here M and H are split along Y -- rank r owns the rows [y0_r, y0_r + ny_r) of every
+ * (component, z) plane, arrays [3][nz][ny_r][nx] -- so the x transforms are local and only the two spectrum
+ * transfers remain (12 n_c (G-1)/G^2 reals per rank instead of the paper's 18).  The y and z stages and
+ * the stored kernel use the paper's x partitioning of the half spectrum ("for the y and z FFT steps the
+ * x dimension partitioning is used"; K^(g)): rank s owns the frequency pairs (k, nx-k),
+ * k in [q0_s, q0_s + nq_s), of 0 <= k <= nx/2.  Both splits give every rank `per` units and the last rank the
+ * remainder, see demag_shard_range.
+ * The transfers are not copies: the x R2C kernel stores every spectrum element directly into the workspace of the
+ * rank that owns its pair, and the y inverse kernel stores every cropped element into the workspace of the rank
+ * that owns its row (peer device pointers, NVLink), so the exchange overlaps the transforms tile by tile.
+ *
+ * Protocol per convolution, on every rank, all on one stream:
+ *     demag_apply_sharded(plan, 0, M_loc, NULL, stream);     x R2C            (writes peers' W1in)
+ *     <barrier over all ranks, ordered on the stream>
+ *     demag_apply_sharded(plan, 1, NULL, NULL, stream);      y FFT, z FFT . multiply . z IFFT, y IFFT (writes peers' W1out)
+ *     <barrier over all ranks, ordered on the stream>
+ *     demag_apply_sharded(plan, 2, NULL, H_loc, stream);     x C2R
+ * The barrier is the caller's (the Python binding enqueues an NCCL all-reduce of one element on the same stream).  No
+ * barrier is needed between two convolutions.
+ *
+ * Restrictions (DEMAG_ERR_UNSUPPORTED otherwise): the fast kernel family only -- power-of-two mesh sizes, nz >= 2,
+ * no periodic axis, sizes in the instantiated range (demag_path() == 1) -- world <= 16, and at least 16 rows
+ * (8 for nx >= 1024 ... see demag_shard_range's align) and one frequency pair per rank. */
+
+/* Host-only arithmetic of the partition: units [begin, begin + count) of n belong to `rank` of `world`; every rank
+ * gets per = floor(n / world / align) * align units and the last one the remainder.  DEMAG_ERR_UNSUPPORTED if
+ * per == 0, DEMAG_ERR_INVALID_ARG for bad arguments.  Needs no GPU. */
+demag_status demag_shard_range(int n, int world, int rank, int align, int* begin, int* count);
+
+/* As demag_plan_create, for rank `rank` of `world`; (nx, ny, nz) is the WHOLE mesh.  Allocates this rank's W1in,
+ * W1out, its slab of the y/z workspace and, at demag_set_kernel (which takes the whole real-space table or NULL, as on
+ * one GPU), only its part K^(rank) of the spectrum.  world == 1 is allowed (and equals demag_plan_create's result). */
+demag_status demag_plan_create_sharded(demag_plan_t* out, int nx, int ny, int nz, double hx, double hy, double hz,
+                                       unsigned pbc_flags, int precision, int rank, int world);
+
+/* This rank's ranges (any pointer may be NULL): rows [y0, y0 + ny_loc), frequency pairs [q0, q0 + nq_loc). */
+demag_status demag_shard_info(demag_plan_t plan, int* rank, int* world, int* y0, int* ny_loc, int* q0, int* nq_loc);
+
+/* This rank's two exchange buffers (device pointers owned by the plan) and their sizes in bytes. */
+demag_status demag_shard_buffers(demag_plan_t plan, void** w1in_dev, size_t* w1in_bytes, void** w1out_dev, size_t* w1out_bytes);
+
+/* Wiring the ranks together.  Either exchange CUDA IPC handles between the processes:
+ *   demag_shard_ipc_export writes 128 bytes (two cudaIpcMemHandle_t: W1in, W1out) to handles_host;
+ *   demag_shard_ipc_connect takes world * 128 bytes, rank-major (an all-gather of the exports), opens every other
+ *   rank's buffers (peer access over NVLink) and installs them;
+ * or, when the buffers of all ranks are already addressable from this device (one process driving several plans),
+ *   demag_shard_set_peers installs world pointers to the W1in and world pointers to the W1out buffers (host arrays
+ *   of device pointers, entry `rank` must be the plan's own buffer).
+ * DEMAG_ERR_INVALID_ARG for a plan that is not sharded; DEMAG_ERR_CUDA if a handle cannot be opened. */
+demag_status demag_shard_ipc_export(demag_plan_t plan, void* handles_host);
+demag_status demag_shard_ipc_connect(demag_plan_t plan, const void* all_handles_host);
+demag_status demag_shard_set_peers(demag_plan_t plan, void* const* w1in_of_rank, void* const* w1out_of_rank);
+
+/* One phase (0, 1, 2: see the protocol above) of the partitioned convolution.  M_loc_dev (phase 0) and H_loc_dev
+ * (phase 2) are this rank's rows, [3][nz][ny_loc][nx] in the plan's precision, 16-byte aligned; the other pointer
+ * arguments are ignored.  Asynchronous on the stream, never allocates or synchronises.
+ * DEMAG_ERR_NO_KERNEL before demag_set_kernel, DEMAG_ERR_INVALID_ARG before the peers are installed, for a bad phase
+ * or a plan that is not sharded.  demag_apply / demag_apply_add / demag_apply_atomistic on a sharded plan with
+ * world > 1 return DEMAG_ERR_INVALID_ARG; demag_energy returns this rank's partial sum over its rows. */
+demag_status demag_apply_sharded(demag_plan_t plan, int phase, const void* M_loc_dev, void* H_loc_dev, void* cuda_stream);
+
 /* Last error message of the calling thread ("" if none). */
 const char* demag_last_error(void);
 

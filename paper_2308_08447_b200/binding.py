@@ -21,7 +21,9 @@ STATUS = {0: "DEMAG_OK", 1: "DEMAG_ERR_INVALID_ARG", 2: "DEMAG_ERR_UNSUPPORTED",
 
 EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy", "demag_apply_atomistic",
            "demag_get_kernel_real", "demag_workspace_bytes", "demag_set_slab", "demag_launches_per_apply",
-           "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path", "demag_apply_add"]
+           "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path", "demag_apply_add",
+           "demag_shard_range", "demag_plan_create_sharded", "demag_shard_info", "demag_shard_buffers",
+           "demag_shard_ipc_export", "demag_shard_ipc_connect", "demag_shard_set_peers", "demag_apply_sharded"]
 
 
 class DemagError(RuntimeError):
@@ -65,6 +67,14 @@ def lib():
         L.demag_path.restype = i
         L.demag_last_error.restype = ctypes.c_char_p
         L.demag_plan_destroy.argtypes = [vp]
+        L.demag_shard_range.argtypes = [i, i, i, i, vp, vp]
+        L.demag_plan_create_sharded.argtypes = [ctypes.POINTER(vp), i, i, i, d, d, d, u, i, i, i]
+        L.demag_shard_info.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.demag_shard_buffers.argtypes = [vp, vp, vp, vp, vp]
+        L.demag_shard_ipc_export.argtypes = [vp, vp]
+        L.demag_shard_ipc_connect.argtypes = [vp, vp]
+        L.demag_shard_set_peers.argtypes = [vp, vp, vp]
+        L.demag_apply_sharded.argtypes = [vp, i, vp, vp, vp]
         for name in EXPORTS:
             if name not in ("demag_workspace_bytes", "demag_launches_per_apply", "demag_last_error"):
                 getattr(L, name).restype = i
@@ -150,6 +160,140 @@ def demag_path(plan) -> int:
 
 def demag_plan_destroy(plan):
     _check(lib().demag_plan_destroy(plan))
+
+
+# ---- several GPUs (include/demag.h "Several GPUs"): one rank per process ------------------------------------
+IPC_BYTES = 128
+
+
+def demag_shard_range(n, world, rank, align=1):
+    """-> (begin, count) of `rank`'s units; host arithmetic only."""
+    b, c = ctypes.c_int(), ctypes.c_int()
+    _check(lib().demag_shard_range(int(n), int(world), int(rank), int(align), ctypes.addressof(b), ctypes.addressof(c)))
+    return b.value, c.value
+
+
+def demag_plan_create_sharded(nx, ny, nz, hx, hy, hz, pbc_flags, precision, rank, world) -> int:
+    h = ctypes.c_void_p()
+    _check(lib().demag_plan_create_sharded(ctypes.byref(h), int(nx), int(ny), int(nz), float(hx), float(hy), float(hz),
+                                           int(pbc_flags), int(precision), int(rank), int(world)))
+    return h.value
+
+
+def demag_shard_info(plan) -> dict:
+    v = [ctypes.c_int() for _ in range(6)]
+    _check(lib().demag_shard_info(plan, *[ctypes.addressof(x) for x in v]))
+    return dict(zip(("rank", "world", "y0", "ny_loc", "q0", "nq_loc"), (x.value for x in v)))
+
+
+def demag_shard_buffers(plan):
+    """-> (w1in_ptr, w1in_bytes, w1out_ptr, w1out_bytes)"""
+    a, b = ctypes.c_void_p(), ctypes.c_void_p()
+    na, nb = ctypes.c_size_t(), ctypes.c_size_t()
+    _check(lib().demag_shard_buffers(plan, ctypes.addressof(a), ctypes.addressof(na), ctypes.addressof(b), ctypes.addressof(nb)))
+    return a.value, na.value, b.value, nb.value
+
+
+def demag_shard_ipc_export(plan) -> bytes:
+    buf = (ctypes.c_ubyte * IPC_BYTES)()
+    _check(lib().demag_shard_ipc_export(plan, ctypes.addressof(buf)))
+    return bytes(buf)
+
+
+def demag_shard_ipc_connect(plan, all_handles: bytes):
+    buf = (ctypes.c_ubyte * len(all_handles)).from_buffer_copy(all_handles)
+    _check(lib().demag_shard_ipc_connect(plan, ctypes.addressof(buf)))
+
+
+def demag_shard_set_peers(plan, w1in_of_rank, w1out_of_rank):
+    n = len(w1in_of_rank)
+    a = (ctypes.c_void_p * n)(*w1in_of_rank)
+    b = (ctypes.c_void_p * n)(*w1out_of_rank)
+    _check(lib().demag_shard_set_peers(plan, ctypes.addressof(a), ctypes.addressof(b)))
+
+
+def demag_apply_sharded(plan, phase, M_loc=None, H_loc=None, stream=None):
+    _check(lib().demag_apply_sharded(plan, int(phase), M_loc.data_ptr() if M_loc is not None else None,
+                                     H_loc.data_ptr() if H_loc is not None else None, _stream(stream)))
+
+
+def gather_handles(handle_bytes: bytes, group=None) -> bytes:
+    """All-gather of the ranks' IPC exports over torch.distributed (any backend), rank-major."""
+    import torch.distributed as dist
+    out = [None] * dist.get_world_size(group)
+    dist.all_gather_object(out, handle_bytes, group=group)
+    return b"".join(out)
+
+
+class ShardedPlan:
+    """One rank of the partitioned convolution.  `apply` runs the three phases with a barrier over the process
+    group between them; the barrier is an all-reduce of one element enqueued on the current stream (NCCL), so
+    the host never waits."""
+
+    def __init__(self, n, h, precision=DEMAG_FP32, rank=None, world=None, group=None, connect=True):
+        import torch
+        import torch.distributed as dist
+        self.group = group
+        if rank is None:
+            rank, world = dist.get_rank(group), dist.get_world_size(group)
+        self.n, self.h, self.precision, self.rank, self.world = tuple(n), tuple(h), precision, rank, world
+        self.handle = demag_plan_create_sharded(*n, *h, 0, precision, rank, world)
+        self.info = demag_shard_info(self.handle)
+        self._flag = None
+        if connect:
+            if world == 1:
+                a, _, b, _ = demag_shard_buffers(self.handle)
+                demag_shard_set_peers(self.handle, [a], [b])
+            else:
+                demag_shard_ipc_connect(self.handle, gather_handles(demag_shard_ipc_export(self.handle), group))
+                self._flag = torch.zeros(1, device="cuda")
+
+    def local_shape(self):
+        nx, ny, nz = self.n
+        return (3, nz, self.info["ny_loc"], nx)
+
+    def set_kernel(self, N6_host=None):
+        demag_set_kernel(self.handle, N6_host)
+        return self
+
+    def barrier(self):
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.all_reduce(self._flag, group=self.group)
+
+    def apply(self, M_loc, H_loc, stream=None):
+        demag_apply_sharded(self.handle, 0, M_loc, None, stream)
+        self.barrier()
+        demag_apply_sharded(self.handle, 1, None, None, stream)
+        self.barrier()
+        demag_apply_sharded(self.handle, 2, None, H_loc, stream)
+
+    def energy(self, M_loc, H_loc, E, stream=None):
+        """E <- the whole mesh's energy on every rank (partial sums all-reduced)."""
+        demag_energy(self.handle, M_loc, H_loc, E, stream)
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.all_reduce(E, group=self.group)
+
+    def workspace_bytes(self):
+        return demag_workspace_bytes(self.handle)
+
+    def close(self):
+        if self.handle:
+            demag_plan_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 class Plan:

@@ -38,6 +38,24 @@ template <typename T> struct alignas(4 * sizeof(T)) KQ {     // kernel spectrum 
     typename vec2<T>::type xx, yy, zz, xy, xz, yz;
 };
 
+// ---- partitioned workspaces (several GPUs; PAPER.md:31-35 and Fig. 1, :261-341) -------------------
+// With G ranks the spectrum W1v exists twice, each copy split a different way (the paper's S1 and S2 partitionings):
+//   W1in  on rank s: [3][nq_s][nz][ny]     all y of the pairs q this rank owns   (input of its y/z stage)
+//   W1out on rank r: [3][hq][nz][ny_r]     all pairs of the rows y this rank owns (input of its x C2R stage)
+// The kernel that PRODUCES a spectrum stores every element straight into the buffer of the rank that consumes it
+// (peer-mapped device pointers over NVLink), so the paper's Transfer_S1_to_S2 / Transfer_S2_to_S1 (:272-289) happen
+// inside the x R2C and y inverse kernels, tile by tile, and no pack / unpack copy exists.  Ranges are `per` units
+// per rank, the last rank takes the remainder (:33 "approximately, since ... may not integer-divide").
+constexpr int kMaxRanks = 16;
+template <typename T> struct ShardMap {
+    int G;                    // number of ranks
+    int per;                  // units per rank: pairs q (x R2C -> W1in), rows y (y inverse -> W1out)
+    int total;                // hq (x R2C), ny (y inverse)
+    int off;                  // this rank's first global row y (x R2C), first global pair q (y inverse)
+    int pitch;                // global ny (x R2C: row length of W1in), global hq (y inverse: pairs of W1out)
+    CQ<T>* base[kMaxRanks];   // W1in / W1out of every rank, as seen from this device
+};
+
 // ---- 128-bit quad access ----------------------------------------------------------------------------
 __device__ __forceinline__ CQ<float> ldq(const CQ<float>* p)
 {
@@ -436,9 +454,9 @@ __global__ void __launch_bounds__(NT) k_y_fwd_long_v(GeoV g, int q0, int nq, con
 }
 
 // y inverse FFT fused with the crop: W2v -> W1v
-template <typename T, int LNY, int POL, int BP, int NT>
-__global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
-                                               CQ<T>* __restrict__ W1, TwSet<T> tw)
+template <typename T, int LNY, int POL, int BP, int NT, bool SH>
+__device__ __forceinline__ void y_inv_body(const GeoV& g, int q0, int nq, const CQ<T>* __restrict__ W2,
+                                           CQ<T>* __restrict__ W1, const ShardMap<T>* map, const TwSet<T>& tw)
 {
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
@@ -448,7 +466,16 @@ __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ
     const int tid = threadIdx.x;
     const int nlines = 3 * nq * g.nz;
     const int l0 = blockIdx.x * BP;
-    if (tid < BP) loff[tid] = (l0 + tid < nlines) ? w1v_line_offset(g, l0 + tid, q0, nq) : -1;
+    if (tid < BP) {
+        long long o = -1;
+        if (l0 + tid < nlines) {
+            if constexpr (SH) {      // global line number ((c hq + q) nz + z) of the partitioned W1out
+                const int l = l0 + tid, z = l % g.nz, ck = l / g.nz, ql = ck % nq, c = ck / nq;
+                o = ((long long)c * map->pitch + map->off + q0 + ql) * g.nz + z;
+            } else o = w1v_line_offset(g, l0 + tid, q0, nq);
+        }
+        loff[tid] = o;
+    }
     const CQ<T>* src = W2 + (size_t)l0 * NY;
     const int nvalid = min(BP, nlines - l0);
     if constexpr (NP >= 2) {
@@ -475,8 +502,33 @@ __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ
         }
         __syncthreads();
     }
-    auto st = [&](int b, int p, CQ<T> v) { const long long o = loff[b]; if (o >= 0) stq(W1 + o + p, v); };
-    pass_last<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, st);
+    if constexpr (SH) {
+        // row y of line L belongs to rank r = y / per: its W1out holds [line][ny_r] (Transfer_S2_to_S1)
+        auto st = [&](int b, int p, CQ<T> v) {
+            const long long o = loff[b];
+            if (o < 0) return;
+            const int r = min(p / map->per, map->G - 1), y0 = r * map->per;
+            const int nyr = r == map->G - 1 ? map->total - y0 : map->per;
+            stq(map->base[r] + o * nyr + (p - y0), v);
+        };
+        pass_last<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, st);
+    } else {
+        auto st = [&](int b, int p, CQ<T> v) { const long long o = loff[b]; if (o >= 0) stq(W1 + o + p, v); };
+        pass_last<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, st);
+    }
+}
+template <typename T, int LNY, int POL, int BP, int NT>
+__global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
+                                               CQ<T>* __restrict__ W1, TwSet<T> tw)
+{
+    y_inv_body<T, LNY, POL, BP, NT, false>(g, q0, nq, W2, W1, nullptr, tw);
+}
+// the same with the crop scattered to the ranks that own the rows (several GPUs)
+template <typename T, int LNY, int POL, int BP, int NT>
+__global__ void __launch_bounds__(NT) k_y_inv_sh_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
+                                                  const __grid_constant__ ShardMap<T> map, TwSet<T> tw)
+{
+    y_inv_body<T, LNY, POL, BP, NT, true>(g, q0, nq, W2, nullptr, &map, tw);
 }
 
 // =========================================================================================== K3v: z stage
@@ -648,9 +700,9 @@ template <int LLC, typename T> __device__ __forceinline__ CQ<T> split_tw(const C
 
 // x R2C FFT fused with the zero padding and the transposition to y-contiguous storage
 // (PAPER.md:35, :296-300 xFFT_R2C; :343 "xy transposition ... to avoid strided y FFTs"):  M -> W1v
-template <typename T, int LLC, int POL, int RP, int NT>
-__global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
-                                               TwSet<T> tw, const CQ<T>* __restrict__ twpost)
+template <typename T, int LLC, int POL, int RP, int NT, bool SH>
+__device__ __forceinline__ void x_r2c_body(const GeoV& g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
+                                           const ShardMap<T>* map, const TwSet<T>& tw, const CQ<T>* __restrict__ twpost)
 {
     using V = typename vec2<T>::type;
     constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true);
@@ -672,7 +724,7 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
     FwdPasses<T, LLC, POL, 1, SC.n, RP, PITCH, NT>::run(s, tw, tid);
     const int c = cz / g.nz, z = cz - c * g.nz;
     const size_t plane = (size_t)g.nz * g.ny;
-    CQ<T>* out = W1 + ((size_t)c * g.hq * g.nz + z) * g.ny + y0;
+    CQ<T>* out = SH ? nullptr : W1 + ((size_t)c * g.hq * g.nz + z) * g.ny + y0;
     constexpr int TOT = (LC / 2 + 1) * RP;
 #pragma unroll 2
     for (int t = tid; t < TOT; t += NT) {
@@ -687,9 +739,27 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
         CQ<T> o0, o1;
         o0.re.x = xkr.x; o0.re.y = xmr.x; o0.im.x = xki.x; o0.im.y = xmi.x;
         o1.re.x = xkr.y; o1.re.y = xmr.y; o1.im.x = xki.y; o1.im.y = xmi.y;
-        CQ<T>* d = out + (size_t)k * plane + 2 * b;
+        CQ<T>* d;
+        if constexpr (SH) {      // pair k belongs to rank s = k / per: its W1in holds [c][nq_s][nz][ny] (Transfer_S1_to_S2)
+            const int sr = min(k / map->per, map->G - 1), k0 = sr * map->per;
+            const int nqs = sr == map->G - 1 ? map->total - k0 : map->per;
+            d = map->base[sr] + (((size_t)c * nqs + (k - k0)) * g.nz + z) * map->pitch + map->off + y0 + 2 * b;
+        } else d = out + (size_t)k * plane + 2 * b;
         stq(d, o0); stq(d + 1, o1);
     }
+}
+template <typename T, int LLC, int POL, int RP, int NT>
+__global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
+                                               TwSet<T> tw, const CQ<T>* __restrict__ twpost)
+{
+    x_r2c_body<T, LLC, POL, RP, NT, false>(g, M, W1, nullptr, tw, twpost);
+}
+// the same on this rank's rows only (g.ny = rows of this rank), every pair stored at the rank that owns it
+template <typename T, int LLC, int POL, int RP, int NT>
+__global__ void __launch_bounds__(NT) k_x_r2c_sh_v(GeoV g, const T* __restrict__ M, const __grid_constant__ ShardMap<T> map,
+                                                  TwSet<T> tw, const CQ<T>* __restrict__ twpost)
+{
+    x_r2c_body<T, LLC, POL, RP, NT, true>(g, M, nullptr, &map, tw, twpost);
 }
 
 // x C2R FFT fused with the crop; writes H:  W1v -> H

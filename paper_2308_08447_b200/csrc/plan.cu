@@ -82,6 +82,11 @@ struct demag_plan_s {
     int on[3] = {0, 0, 0};
     bool embed = false;
     void* Mp = nullptr; void* Hp = nullptr;
+    // several GPUs (demag_plan_create_sharded): W1 is W1in [3][nq_loc][nz][ny], W1out is [3][hq][nz][ny_loc]
+    bool sharded = false, peers_set = false;
+    int world = 1, rank = 0, y0 = 0, ny_loc = 0, q0 = 0, nq_loc = 0;
+    void* W1out = nullptr; size_t w1out_bytes = 0;
+    void* ipc_open[2 * v2::kMaxRanks] = {};
 };
 
 namespace {
@@ -236,8 +241,35 @@ extern "C" {
 
 const char* demag_last_error(void) { return g_err; }
 
+static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, double hx, double hy, double hz,
+                                     unsigned pbc_flags, int precision, int rank, int world, bool sharded);
+
 demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double hx, double hy, double hz,
                                unsigned pbc_flags, int precision)
+{
+    return plan_create_impl(out, nx, ny, nz, hx, hy, hz, pbc_flags, precision, 0, 1, false);
+}
+
+demag_status demag_plan_create_sharded(demag_plan_t* out, int nx, int ny, int nz, double hx, double hy, double hz,
+                                       unsigned pbc_flags, int precision, int rank, int world)
+{
+    return plan_create_impl(out, nx, ny, nz, hx, hy, hz, pbc_flags, precision, rank, world, true);
+}
+
+demag_status demag_shard_range(int n, int world, int rank, int align, int* begin, int* count)
+{
+    g_err[0] = 0;
+    if (n < 1 || world < 1 || rank < 0 || rank >= world || align < 1 || !begin || !count)
+        return fail(DEMAG_ERR_INVALID_ARG, "demag_shard_range: bad arguments (n %d, world %d, rank %d, align %d)", n, world, rank, align);
+    const int per = n / world / align * align;
+    if (per == 0) return fail(DEMAG_ERR_UNSUPPORTED, "%d units cannot be split over %d ranks in multiples of %d", n, world, align);
+    *begin = rank * per;
+    *count = rank == world - 1 ? n - rank * per : per;
+    return DEMAG_OK;
+}
+
+static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, double hx, double hy, double hz,
+                                     unsigned pbc_flags, int precision, int rank, int world, bool sharded)
 {
     g_err[0] = 0;
     if (!out) return fail(DEMAG_ERR_INVALID_ARG, "out is NULL");
@@ -252,8 +284,15 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         ((pbc_flags & DEMAG_PBC_Z) && !is_pow2(nz)))
         return fail(DEMAG_ERR_UNSUPPORTED, "a periodic axis cannot be padded: its size must be a power of two (got %d x %d x %d)", nx, ny, nz);
 
+    if (sharded) {
+        if (world < 1 || world > v2::kMaxRanks || rank < 0 || rank >= world)
+            return fail(DEMAG_ERR_INVALID_ARG, "bad rank %d / world %d (1 <= world <= %d)", rank, world, v2::kMaxRanks);
+        if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz) || nz < 2 || pbc_flags)
+            return fail(DEMAG_ERR_UNSUPPORTED, "a sharded plan needs power-of-two mesh sizes, nz >= 2 and no periodic axis");
+    }
     demag_plan_s* p = new (std::nothrow) demag_plan_s();
     if (!p) return fail(DEMAG_ERR_ALLOC, "out of host memory");
+    p->sharded = sharded; p->world = world; p->rank = rank;
     // General sizes (R10): the transforms need power-of-two lengths N_a >= 2 n_a - 1 for an exact linear
     // convolution, so the mesh is embedded, with zeros, in the mesh of the next powers of two.
     p->on[0] = nx; p->on[1] = ny; p->on[2] = nz;
@@ -296,9 +335,24 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         return fail(DEMAG_ERR_UNSUPPORTED, "a transform line of this plan needs %d bytes of shared memory (limit %d): "
                     "8192-point z lines are fp32 only", worst, kMaxSmem);
     }
+    if (sharded && !p->v2) {
+        delete p;
+        return fail(DEMAG_ERR_UNSUPPORTED, "a sharded plan needs the fast kernel family (sizes in its range; DEMAG_PATH=fast for fp64)");
+    }
     if (p->v2) {
         v2::GeoV gv;
         gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0;
+        p->cf.gx = gv; p->cd.gx = gv;
+        p->ny_loc = ny; p->nq_loc = gv.hq;
+        if (sharded) {
+            // rows of M / H (tiles of the x kernels: 2 RP rows) and frequency pairs of this rank
+            demag_status s1 = demag_shard_range(ny, world, rank, 2 * v2::x_rp(g.lLc), &p->y0, &p->ny_loc);
+            demag_status s2 = s1 ? s1 : demag_shard_range(gv.hq, world, rank, 1, &p->q0, &p->nq_loc);
+            if (s2) { delete p; return s2; }
+            p->cf.gx.ny = p->cd.gx.ny = p->ny_loc;
+            gv.hq = p->nq_loc;                              // the y / z stages see only this rank's pairs
+            p->cf.sharded = p->cd.sharded = true;
+        }
         p->cf.g = gv; p->cd.g = gv;
         {   // one-cell-thick mesh: y FFT . multiply . y IFFT fused in one kernel, in place on W1 (scope row a3')
             const bool film = v2::film_supported(nz, g.Nz, g.lNy, p->esz, kMaxSmem) && !getenv("DEMAG_NO_FILM");
@@ -317,6 +371,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
         if (n > gv.hq) n = gv.hq;
         p->nq_auto = p->nq_slab = (int)n;
         p->w1_bytes = (size_t)3 * gv.hq * g.nz * g.ny * qsz;
+        if (sharded) p->w1out_bytes = (size_t)3 * (nx / 2 + 1) * g.nz * p->ny_loc * qsz;
         p->w2_bytes = (size_t)p->nq_auto * per_q;
         p->k_bytes = (size_t)gv.hq * g.kpz * g.Ny * 12 * p->esz;
         if (p->cf.film) { p->w2_bytes = 256; p->k_bytes = (size_t)gv.hq * g.kpy * 12 * p->esz; }
@@ -349,6 +404,10 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
                 v2::y_inv<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::z_mul<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 if (p->cf.film) { v2::y_film<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr); }
+                if (sharded) {
+                    v2::x_fwd_sh<float>(0, p->cf, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                    v2::y_inv_sh<float>(0, p->cf, nullptr, 0, 0, nullptr, &verr); CUDA_TRY(verr);
+                }
             } else {
                 for (int a = 0; a < 3; ++a) {
                     CUDA_TRY(v2::build_axis_tables<double>(LL[a], POL[a], a == 0 ? nx : 0, &p->td[a], a == 0 ? &p->cd.twpost : nullptr));
@@ -361,6 +420,10 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
                 v2::y_inv<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::z_mul<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 if (p->cd.film) { v2::y_film<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr); }
+                if (sharded) {
+                    v2::x_fwd_sh<double>(0, p->cd, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                    v2::y_inv_sh<double>(0, p->cd, nullptr, 0, 0, nullptr, &verr); CUDA_TRY(verr);
+                }
             }
             {   // y position -> frequency map of the y schedule, for the plan-time pack
                 const v2::Sched sc = v2::make_sched(g.lNy, v2::y_pol(g.lNy));
@@ -378,6 +441,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
             p->macro_bytes += 2 * b;
         }
         CUDA_TRY(cudaMalloc(&p->W1, p->w1_bytes));
+        if (sharded) CUDA_TRY(cudaMalloc(&p->W1out, p->w1out_bytes));
         CUDA_TRY(cudaMalloc(&p->W2, p->w2_bytes));
         CUDA_TRY(cudaMalloc(&p->K, p->k_bytes));
         CUDA_TRY(cudaMemset(p->K, 0, p->k_bytes));
@@ -398,7 +462,8 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz, double
 demag_status demag_plan_destroy(demag_plan_t p)
 {
     if (!p) return DEMAG_OK;
-    cudaFree(p->W1); cudaFree(p->W2); cudaFree(p->K);
+    for (void* q : p->ipc_open) if (q) cudaIpcCloseMemHandle(q);
+    cudaFree(p->W1); cudaFree(p->W1out); cudaFree(p->W2); cudaFree(p->K);
     for (int a = 0; a < 3; ++a) cudaFree(p->tw[a]);
     cudaFree(p->Mc); cudaFree(p->Hc); cudaFree(p->Mp); cudaFree(p->Hp);
     for (int a = 0; a < 3; ++a) { cudaFree(p->tf[a].dev); cudaFree(p->td[a].dev); }
@@ -410,7 +475,7 @@ demag_status demag_plan_destroy(demag_plan_t p)
 size_t demag_workspace_bytes(demag_plan_t p)
 {
     if (!p) return 0;
-    return p->w1_bytes + p->w2_bytes + p->k_bytes + p->tw_bytes + p->macro_bytes;
+    return p->w1_bytes + p->w1out_bytes + p->w2_bytes + p->k_bytes + p->tw_bytes + p->macro_bytes;
 }
 
 demag_status demag_set_slab(demag_plan_t p, int kx_per_slab)
@@ -548,9 +613,9 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
                 const size_t n = (size_t)gv.hq * g.kpz * g.Ny;
                 const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
                 if (p->prec == DEMAG_FP32)
-                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale);
+                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale, p->q0);
                 else
-                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale);
+                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale, p->q0);
             }
             else if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
             else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
@@ -711,6 +776,7 @@ demag_status apply_outer(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Sta
 demag_status check_apply_args(demag_plan_s* p, const void* a, const void* b, size_t bytes)
 {
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (p->sharded && p->world > 1) return fail(DEMAG_ERR_INVALID_ARG, "plan is one rank of %d: use demag_apply_sharded", p->world);
     if (!a || !b) return fail(DEMAG_ERR_INVALID_ARG, "NULL device pointer");
     if (((uintptr_t)a & 15) || ((uintptr_t)b & 15)) return fail(DEMAG_ERR_INVALID_ARG, "device pointers must be 16-byte aligned");
     const char *pa = (const char*)a, *pb = (const char*)b;
@@ -744,6 +810,138 @@ extern "C" demag_status demag_apply_add(demag_plan_t p, const void* M_dev, void*
     cudaStream_t st = (cudaStream_t)cuda_stream;
     return p->prec == DEMAG_FP32 ? apply_outer<float>(p, (const float*)M_dev, (float*)Heff_dev, st, nullptr, 1)
                                  : apply_outer<double>(p, (const double*)M_dev, (double*)Heff_dev, st, nullptr, 1);
+}
+
+// ================================================================================ several GPUs
+extern "C" demag_status demag_shard_info(demag_plan_t p, int* rank, int* world, int* y0, int* ny_loc, int* q0, int* nq_loc)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->sharded) return fail(DEMAG_ERR_INVALID_ARG, "plan was not created by demag_plan_create_sharded");
+    if (rank) *rank = p->rank;
+    if (world) *world = p->world;
+    if (y0) *y0 = p->y0;
+    if (ny_loc) *ny_loc = p->ny_loc;
+    if (q0) *q0 = p->q0;
+    if (nq_loc) *nq_loc = p->nq_loc;
+    return DEMAG_OK;
+}
+
+extern "C" demag_status demag_shard_buffers(demag_plan_t p, void** w1in_dev, size_t* w1in_bytes, void** w1out_dev, size_t* w1out_bytes)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->sharded) return fail(DEMAG_ERR_INVALID_ARG, "plan was not created by demag_plan_create_sharded");
+    if (w1in_dev) *w1in_dev = p->W1;
+    if (w1in_bytes) *w1in_bytes = p->w1_bytes;
+    if (w1out_dev) *w1out_dev = p->W1out;
+    if (w1out_bytes) *w1out_bytes = p->w1out_bytes;
+    return DEMAG_OK;
+}
+
+namespace {
+template <typename T>
+void install_peers(demag_plan_s* p, v2::Ctx<T>& c, void* const* in, void* const* outp)
+{
+    const int hq = p->g.nx / 2 + 1;
+    int b0 = 0, cnt = 0;
+    // x R2C -> W1in of the pair's owner: pairs per rank, this rank's first row, row length = whole ny
+    demag_shard_range(hq, p->world, 0, 1, &b0, &cnt);
+    c.m_in.G = p->world; c.m_in.per = cnt; c.m_in.total = hq; c.m_in.off = p->y0; c.m_in.pitch = p->g.ny;
+    // y inverse -> W1out of the row's owner: rows per rank, this rank's first pair, pairs = whole hq
+    demag_shard_range(p->g.ny, p->world, 0, 2 * v2::x_rp(p->g.lLc), &b0, &cnt);
+    c.m_out.G = p->world; c.m_out.per = cnt; c.m_out.total = p->g.ny; c.m_out.off = p->q0; c.m_out.pitch = hq;
+    for (int r = 0; r < v2::kMaxRanks; ++r) {
+        c.m_in.base[r] = r < p->world ? (v2::CQ<T>*)in[r] : nullptr;
+        c.m_out.base[r] = r < p->world ? (v2::CQ<T>*)outp[r] : nullptr;
+    }
+}
+}  // namespace
+
+extern "C" demag_status demag_shard_set_peers(demag_plan_t p, void* const* w1in_of_rank, void* const* w1out_of_rank)
+{
+    g_err[0] = 0;
+    if (!p || !w1in_of_rank || !w1out_of_rank) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
+    if (!p->sharded) return fail(DEMAG_ERR_INVALID_ARG, "plan was not created by demag_plan_create_sharded");
+    for (int r = 0; r < p->world; ++r)
+        if (!w1in_of_rank[r] || !w1out_of_rank[r] || ((uintptr_t)w1in_of_rank[r] & 15) || ((uintptr_t)w1out_of_rank[r] & 15))
+            return fail(DEMAG_ERR_INVALID_ARG, "buffer of rank %d is NULL or not 16-byte aligned", r);
+    if (w1in_of_rank[p->rank] != p->W1 || w1out_of_rank[p->rank] != p->W1out)
+        return fail(DEMAG_ERR_INVALID_ARG, "entry %d must be this plan's own buffers (demag_shard_buffers)", p->rank);
+    if (p->prec == DEMAG_FP32) install_peers<float>(p, p->cf, w1in_of_rank, w1out_of_rank);
+    else install_peers<double>(p, p->cd, w1in_of_rank, w1out_of_rank);
+    p->peers_set = true;
+    return DEMAG_OK;
+}
+
+extern "C" demag_status demag_shard_ipc_export(demag_plan_t p, void* handles_host)
+{
+    g_err[0] = 0;
+    if (!p || !handles_host) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
+    if (!p->sharded) return fail(DEMAG_ERR_INVALID_ARG, "plan was not created by demag_plan_create_sharded");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "two 64-byte handles per rank");
+    cudaIpcMemHandle_t h[2];
+    CUDA_TRY(cudaIpcGetMemHandle(&h[0], p->W1));
+    CUDA_TRY(cudaIpcGetMemHandle(&h[1], p->W1out));
+    memcpy(handles_host, h, sizeof(h));
+    return DEMAG_OK;
+}
+
+extern "C" demag_status demag_shard_ipc_connect(demag_plan_t p, const void* all_handles_host)
+{
+    g_err[0] = 0;
+    if (!p || !all_handles_host) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
+    if (!p->sharded) return fail(DEMAG_ERR_INVALID_ARG, "plan was not created by demag_plan_create_sharded");
+    if (p->peers_set) return fail(DEMAG_ERR_INVALID_ARG, "peers are already installed");
+    void* in[v2::kMaxRanks]; void* outp[v2::kMaxRanks];
+    for (int r = 0; r < p->world; ++r) {
+        if (r == p->rank) { in[r] = p->W1; outp[r] = p->W1out; continue; }
+        cudaIpcMemHandle_t h[2];
+        memcpy(h, (const char*)all_handles_host + (size_t)r * sizeof(h), sizeof(h));
+        CUDA_TRY(cudaIpcOpenMemHandle(&p->ipc_open[2 * r], h[0], cudaIpcMemLazyEnablePeerAccess));
+        CUDA_TRY(cudaIpcOpenMemHandle(&p->ipc_open[2 * r + 1], h[1], cudaIpcMemLazyEnablePeerAccess));
+        in[r] = p->ipc_open[2 * r]; outp[r] = p->ipc_open[2 * r + 1];
+    }
+    return demag_shard_set_peers(p, in, outp);
+}
+
+namespace {
+template <typename T>
+demag_status apply_sharded_impl(demag_plan_s* p, int phase, const T* M, T* H, cudaStream_t st)
+{
+    const v2::Ctx<T>& cx = v2_ctx<T>(p);
+    cudaError_t verr = cudaSuccess;
+    if (phase == 0) v2::x_fwd_sh<T>(1, cx, st, M, &verr);                         // xFFT_R2C + Transfer_S1_to_S2
+    else if (phase == 1) {
+        v2::CQ<T>* V1 = (v2::CQ<T>*)p->W1; v2::CQ<T>* V2 = (v2::CQ<T>*)p->W2;
+        const typename v2::kchunks<T>::V* Kv = (const typename v2::kchunks<T>::V*)p->K;
+        for (int q0 = 0; q0 < cx.g.hq; q0 += p->nq_slab) {                        // this rank's pairs, slab by slab
+            const int nq = std::min(p->nq_slab, cx.g.hq - q0);
+            v2::y_fwd<T>(1, cx, st, q0, nq, V1, V2, &verr);
+            v2::z_mul<T>(1, cx, st, q0, nq, V2, Kv, &verr);
+            v2::y_inv_sh<T>(1, cx, st, q0, nq, V2, &verr);                        // yFFT inverse + Transfer_S2_to_S1
+        }
+    }
+    else v2::x_inv<T>(1, cx, st, (const v2::CQ<T>*)p->W1out, H, &verr, 0);        // xFFT_C2R
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}
+}  // namespace
+
+extern "C" demag_status demag_apply_sharded(demag_plan_t p, int phase, const void* M_loc_dev, void* H_loc_dev, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (!p->sharded) return fail(DEMAG_ERR_INVALID_ARG, "plan was not created by demag_plan_create_sharded");
+    if (phase < 0 || phase > 2) return fail(DEMAG_ERR_INVALID_ARG, "phase must be 0, 1 or 2");
+    if (!p->peers_set) return fail(DEMAG_ERR_INVALID_ARG, "peers not installed (demag_shard_ipc_connect / demag_shard_set_peers)");
+    if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
+    const void* io = phase == 0 ? M_loc_dev : phase == 2 ? H_loc_dev : (const void*)p->W1;
+    if (!io) return fail(DEMAG_ERR_INVALID_ARG, "NULL device pointer");
+    if ((uintptr_t)io & 15) return fail(DEMAG_ERR_INVALID_ARG, "device pointers must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return p->prec == DEMAG_FP32 ? apply_sharded_impl<float>(p, phase, (const float*)M_loc_dev, (float*)H_loc_dev, st)
+                                 : apply_sharded_impl<double>(p, phase, (const double*)M_loc_dev, (double*)H_loc_dev, st);
 }
 
 extern "C" demag_status demag_apply_profiled(demag_plan_t p, const void* M_dev, void* H_dev, void* cuda_stream,
@@ -781,7 +979,7 @@ extern "C" demag_status demag_energy(demag_plan_t p, const void* M_dev, const vo
     if (!p || !M_dev || !H_dev || !E_dev) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
     if ((uintptr_t)E_dev & 7) return fail(DEMAG_ERR_INVALID_ARG, "E_dev must be 8-byte aligned");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t n3 = (size_t)3 * p->on[0] * p->on[1] * p->on[2];
+    const size_t n3 = (size_t)3 * p->on[0] * (p->sharded ? p->ny_loc : p->on[1]) * p->on[2];   // sharded: this rank's rows
     const double mu0 = 4.0e-7 * 3.14159265358979323846;
     const double scale = -0.5 * mu0 * p->h[0] * p->h[1] * p->h[2];
     CUDA_TRY(cudaMemsetAsync(E_dev, 0, sizeof(double), st));

@@ -143,8 +143,9 @@ cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>*
 inline int z_kt(int lNz) { return lNz >= 4 ? z_ty(lNz) : 32; }
 template <typename T>
 __global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv, int comp, int Lc, int hq, int kpy, int kpz,
-                                int Ny, int KT, const int* __restrict__ ypos2freq, int par_y, double scale)
+                                int Ny, int KT, const int* __restrict__ ypos2freq, int par_y, double scale, int q0)
 {
+    // hq pairs starting at pair q0 (several GPUs: K^(g) holds only its own kx range; else q0 = 0)
     const size_t n = (size_t)hq * kpz * Ny;
     const int hx = Lc + 1;
     constexpr int U = 16 / (int)sizeof(T), NCH = 12 / U;          // values per 16-byte chunk, chunks per entry
@@ -158,8 +159,8 @@ __global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv
         const double* row = A + ((size_t)kz * kpy + kyp) * hx;
         const size_t tile_row = ((size_t)q * (Ny / KT) + py / KT) * kpz + kz;
         T* d = Kv + ((tile_row * NCH + j) * KT + py % KT) * U + off;
-        d[0] = (T)(sg * scale * row[q]);
-        d[1] = (T)(sg * scale * row[Lc - q]);
+        d[0] = (T)(sg * scale * row[q0 + q]);
+        d[1] = (T)(sg * scale * row[Lc - q0 - q]);
     }
 }
 
@@ -191,12 +192,15 @@ inline bool film_supported(int nz, int Nz, int lNy, size_t esz, int max_smem)
 // ---- launchers ---------------------------------------------------------------------------------------------
 template <typename T> struct Ctx {
     int sm_count;
-    GeoV g;
+    GeoV g;                     // y / z stages (several GPUs: hq = the pairs this rank owns)
+    GeoV gx;                    // x stages (several GPUs: ny = the rows this rank owns); = g on one GPU
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;
     const CQ<T>* twpost;
+    bool sharded = false;       // several GPUs: x R2C stores through m_in, y inverse through m_out (kernels_v2.cuh ShardMap)
+    ShardMap<T> m_in, m_out;
 };
 
 #define V2_CASE_X(L, KERN, ...)                                                                                     \
@@ -204,7 +208,7 @@ template <typename T> struct Ctx {
         using C = XCfg<L>;                                                                                           \
         constexpr int smem = x_tile_quads(L, C::POL, C::RP) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::RP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else KERN<T, L, C::POL, C::RP, C::NT><<<3u * c.g.nz * (c.g.ny / (2 * C::RP)), C::NT, smem, st>>>(__VA_ARGS__); \
+        else KERN<T, L, C::POL, C::RP, C::NT><<<3u * c.gx.nz * (c.gx.ny / (2 * C::RP)), C::NT, smem, st>>>(__VA_ARGS__); \
         return true;                                                                                                 \
     }
 
@@ -213,18 +217,31 @@ template <typename T>
 bool x_fwd(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cudaError_t* err)
 {
     switch (c.lLc) {
-        V2_CASE_X(4, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
-        V2_CASE_X(6, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
-        V2_CASE_X(8, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
-        V2_CASE_X(10, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
-        V2_CASE_X(12, k_x_r2c_v, c.g, M, W1, c.twx, c.twpost)
+        V2_CASE_X(4, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
+        V2_CASE_X(6, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
+        V2_CASE_X(8, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
+        V2_CASE_X(10, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
+        V2_CASE_X(12, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
+    default: return false;
+    }
+}
+// several GPUs: rows of this rank in, pairs stored at their owners (k_x_r2c_sh_v)
+template <typename T>
+bool x_fwd_sh(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, cudaError_t* err)
+{
+    switch (c.lLc) {
+        V2_CASE_X(4, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
+        V2_CASE_X(6, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
+        V2_CASE_X(8, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
+        V2_CASE_X(10, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
+        V2_CASE_X(12, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
     default: return false;
     }
 }
 template <typename T>
 bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cudaError_t* err, int acc = 0)
 {
-    GeoV ga = c.g; ga.acc = acc;
+    GeoV ga = c.gx; ga.acc = acc;
     switch (c.lLc) {
         V2_CASE_X(4, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(5, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
         V2_CASE_X(6, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(7, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
@@ -274,6 +291,26 @@ bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<
         V2_CASE_Y(8, k_y_inv_v, W2, W1) V2_CASE_Y(9, k_y_inv_v, W2, W1) V2_CASE_Y(10, k_y_inv_v, W2, W1) V2_CASE_Y(11, k_y_inv_v, W2, W1)
         V2_CASE_Y(12, k_y_inv_v, W2, W1)
     case 13: if constexpr (sizeof(T) == 4) V2_BODY_Y(13, k_y_inv_v, W2, W1) else return false;
+    default: return false;
+    }
+}
+
+// several GPUs: the cropped rows stored at the ranks that own them (k_y_inv_sh_v)
+#define V2_CASE_YSH(L)                                                                                              \
+    case L: {                                                                                                        \
+        using C = YCfg<L>;                                                                                           \
+        constexpr int smem = y_tile_quads(L, C::POL, C::BP) * (int)sizeof(CQ<T>);                                    \
+        if (mode == 0) *err = cudaFuncSetAttribute(k_y_inv_sh_v<T, L, C::POL, C::BP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+        else k_y_inv_sh_v<T, L, C::POL, C::BP, C::NT><<<(unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st>>>(c.g, q0, nq, W2, c.m_out, c.twy); \
+        return true;                                                                                                 \
+    }
+template <typename T>
+bool y_inv_sh(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W2, cudaError_t* err)
+{
+    switch (c.lNy) {
+        V2_CASE_YSH(4) V2_CASE_YSH(5) V2_CASE_YSH(6) V2_CASE_YSH(7) V2_CASE_YSH(8) V2_CASE_YSH(9) V2_CASE_YSH(10) V2_CASE_YSH(11)
+        V2_CASE_YSH(12)
+    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_YSH(13) } } return false;
     default: return false;
     }
 }
