@@ -39,6 +39,12 @@ def parse():
     ap.add_argument("--config", default="C3", help="C1..C5, suffix d = fp64 (e.g. C3d)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true")
+    ap.add_argument("--sharded", action="store_true",
+                    help="ONE convolution partitioned over the N ranks (strong scaling; include/demag.h 'Several GPUs') "
+                         "instead of the default N independent replicas")
+    ap.add_argument("--virtual-ranks", type=int, default=0,
+                    help="with --sharded on ONE GPU: emulate G ranks as G plans on this device, phase by phase, and "
+                         "report the per-rank device time of each phase (a compute-share model, no NVLink involved)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
 
@@ -454,6 +460,146 @@ def run_ours(args, cfg, fp64):
         dist.destroy_process_group()
 
 
+def run_virtual_ranks(args, cfg, fp64):
+    """G ranks as G sharded plans on ONE device, driven phase by phase (tests/test_gpu_sharded.py does the same for
+    parity): the device time of every rank's phase, i.e. the compute share a rank would have on its own GPU when the
+    peer stores cost nothing extra.  Not a multi-GPU measurement: the "peer" buffers are local HBM."""
+    import torch
+    from paper_2308_08447_b200 import binding as B
+    B.lib()
+    G = args.virtual_ranks
+    dev = torch.device("cuda", 0)
+    dt = torch.float64 if fp64 else torch.float32
+    n = cfg.n
+    nc = int(np.prod(n))
+    plans = [B.ShardedPlan(n, cfg.h, B.DEMAG_FP64 if fp64 else B.DEMAG_FP32, rank=r, world=G, connect=False) for r in range(G)]
+    bufs = [B.demag_shard_buffers(p.handle) for p in plans]
+    M_host = W.make_magnetisation(cfg)
+    Xs, Ys = [], []
+    for p in plans:
+        B.demag_shard_set_peers(p.handle, [b[0] for b in bufs], [b[2] for b in bufs])
+        p.set_kernel(None)
+        y0, nyl = p.info["y0"], p.info["ny_loc"]
+        Xs.append(torch.from_numpy(np.ascontiguousarray(M_host[:, :, y0:y0 + nyl, :])).to(dev, dt))
+        Ys.append(torch.empty_like(Xs[-1]))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ms = np.zeros((3, G))
+    reps = max(1, args.steps)
+    for it in range(reps + max(3, args.warmup)):
+        for ph in range(3):
+            for r, p in enumerate(plans):
+                flush.fill_(1)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); B.demag_apply_sharded(p.handle, ph, Xs[r], Ys[r]); b.record()
+                torch.cuda.synchronize()
+                if it >= max(3, args.warmup):
+                    ms[ph, r] += a.elapsed_time(b) / reps
+    per_rank = ms.sum(axis=0)
+    line = {"metric": "sharded_phase_ms_per_rank", "unit": "ms", "virtual_ranks": G, "n_gpus": 1, "steps": reps,
+            "dtype": "f64" if fp64 else "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, fp64), "mesh": list(n), "cells": nc,
+                       "note": "G plans on one device, phase by phase; peer buffers are local HBM (compute-share model)"},
+            "phase_ms_max_over_ranks": [float(v) for v in ms.max(axis=1)],
+            "phase_ms_mean_over_ranks": [float(v) for v in ms.mean(axis=1)],
+            "rank_ms_max": float(per_rank.max()), "rank_ms_sum": float(per_rank.sum()),
+            "exchange_bytes_per_rank": int(12 * nc * (G - 1) / G**2 * (8 if fp64 else 4)),
+            "rows_per_rank": [p.info["ny_loc"] for p in plans], "pairs_per_rank": [p.info["nq_loc"] for p in plans]}
+    for p in plans:
+        p.close()
+    print(json.dumps(line), flush=True)
+
+
+def run_sharded(args, cfg, fp64):
+    """One convolution of the workload split over all ranks (Fig. 1): rows of M / H along y, frequency
+    pairs along kx, the two spectrum exchanges written by the x R2C / y inverse kernels into peer memory, an NCCL
+    all-reduce of one element as the barrier between the three phases.  Timed as the default arm: CUDA events around K
+    steps, L2 flushed between steps, max over ranks; value = cells of the WHOLE mesh per second ("scaling": "strong")."""
+    import torch
+    import torch.distributed as dist
+    from paper_2308_08447_b200 import binding as B
+    B.lib()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    if cfg.kind == "atomistic" or cfg.n[2] == 1:
+        raise SystemExit("--sharded: mesh workloads with nz >= 2 only (C1, C3, C4)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    dt = torch.float64 if fp64 else torch.float32
+    n = cfg.n
+    nc = int(np.prod(n))
+    plan = B.ShardedPlan(n, cfg.h, B.DEMAG_FP64 if fp64 else B.DEMAG_FP32, rank=rank, world=world)
+    plan.set_kernel(None)
+    y0, nyl = plan.info["y0"], plan.info["ny_loc"]
+    M_host = np.ascontiguousarray(W.make_magnetisation(cfg)[:, :, y0:y0 + nyl, :])
+    X = torch.from_numpy(M_host).to(dev, dt)
+    Y = torch.empty_like(X)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        flush.fill_(1); plan.apply(X, Y)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for a, b in evs:
+        flush.fill_(1)
+        a.record(); plan.apply(X, Y); b.record()
+    barrier()
+    ms_total = sum(a.elapsed_time(b) for a, b in evs)
+    # end to end: this rank's rows host -> device, the convolution, this rank's field rows device -> host, every step
+    hin = torch.from_numpy(M_host).to(dt).pin_memory(); hout = torch.empty_like(hin).pin_memory()
+    def e2e_step():
+        X.copy_(hin, non_blocking=True); plan.apply(X, Y); hout.copy_(Y, non_blocking=True)
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    barrier()
+    t_e2e = time.perf_counter() - t0
+    assert torch.isfinite(hout).all() and float(hout.abs().max()) > 0, "e2e produced no field"
+    clocks = sampler.stop() if sampler else None
+    ms_total, t_e2e = allreduce_max([ms_total, t_e2e], dev, world)
+    launches = B.demag_launches_per_apply(plan.handle)
+    ws = plan.workspace_bytes()
+    plan.close()
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": nc * args.steps / (ms_total * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps,
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64" if fp64 else "f32",
+            "data": "synthetic",
+            "config": {"workload": workload_name(cfg, fp64), "mesh": list(n), "cells": nc,
+                       "l2": "flushed between timed steps (256 MB write outside each step's event pair)",
+                       "parallelism": f"one convolution sharded x{world}: rows of M/H along y, frequency pairs along kx; "
+                                      "exchanges stored into peer memory by the x R2C / y inverse kernels; "
+                                      "barrier = NCCL all-reduce of one element between the three phases",
+                       "kernel": "built-in Newell tensor (demag_set_kernel(NULL))", "kernel_family": "fast (kernels_v2.cuh)"},
+            "conv_per_s": args.steps / (ms_total * 1e-3),
+            "e2e": {"value": nc * args.steps / t_e2e / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": world * hin.numel() * hin.element_size(),
+                    "d2h_bytes_per_step": world * hout.numel() * hout.element_size()},
+            "gpu_launches": world * launches * args.steps, "launches_per_step": world * launches,
+            "clocks": clocks, "workspace_bytes_per_rank": ws,
+            "exchange_bytes_per_rank_per_step": int(12 * nc * (world - 1) / world**2 * (8 if fp64 else 4)),
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
     name = args.config
@@ -461,6 +607,10 @@ def main():
     cfg = W.CONFIGS[name[:2]]
     if args.impl == "reference":
         run_reference(args, cfg, fp64)
+    elif args.sharded and args.virtual_ranks > 0:
+        run_virtual_ranks(args, cfg, fp64)
+    elif args.sharded:
+        run_sharded(args, cfg, fp64)
     else:
         run_ours(args, cfg, fp64)
 
