@@ -17,6 +17,7 @@ Citations are ``PAPER.md:<line>`` (arXiv 2308.08447) or a DESIGN.md reading (R<n
     macrocell_scatter   "applied equally to all spins" (PAPER.md:133; R14)           [NumPy]
     dipole_table        point-dipole tensor that turns Eq. (8) into Eq. (1)   [NumPy]
     dipole_field_eq8    Eq. (8) written out, O(n^2)                [NumPy]
+    periodic_tensor_table  image-summed, symmetrised tensor on periodic axes (R11)   [NumPy loops over N_at]
 
 All of them are pinned in tests/test_oracle_pins.py; none is "parity unpinned".
 """
@@ -289,3 +290,31 @@ def dipole_field_eq8(S, mu_s, a) -> np.ndarray:
         t[i] = 0.0
         H[i] = MU_B / (4.0 * np.pi) * t.sum(axis=0)
     return H.T.reshape(3, Lz, Ly, Lx)
+
+
+def periodic_tensor_table(n, h, pbc, images) -> np.ndarray:
+    """Periodic tensor of reading R11 ("modified convolution kernel"; its reference [25] is absent), written as
+    the definition: on every periodic axis a the open-boundary tensor is summed over `images` images on each side,
+
+        S[d] = sum_{|m_a| <= images, a periodic} N((d + m o n) o h),        0 <= d_a < n_a,
+
+    then made symmetric under d_a -> n_a - d_a with the component's parity on that axis (a periodic kernel is; the
+    truncated sum only up to its last images):  T = sym_x sym_y sym_z S,  sym_a f(d_a) = (f(d_a) + parity_a f((n_a - d_a) mod n_a)) / 2.
+    Small meshes only (one N_at call per offset and image)."""
+    nx, ny, nz = map(int, n)
+    rng = [range(-images, images + 1) if p else range(1) for p in pbc]
+    T = np.zeros((6, nz, ny, nx))
+    for dz in range(nz):
+        for dy in range(ny):
+            for dx in range(nx):
+                acc = np.zeros(6)
+                for mx in rng[0]:
+                    for my in rng[1]:
+                        for mz in rng[2]:
+                            acc += N_at(((dx + mx * nx) * h[0], (dy + my * ny) * h[1], (dz + mz * nz) * h[2]), h)
+                T[:, dz, dy, dx] = acc
+    for a, ax in ((0, 3), (1, 2), (2, 1)):
+        if pbc[a]:
+            idx = (-np.arange((nx, ny, nz)[a])) % (nx, ny, nz)[a]
+            T = 0.5 * (T + PARITY[:, a].reshape(6, 1, 1, 1) * np.take(T, idx, axis=ax))
+    return T

@@ -333,3 +333,40 @@ def test_dipole_tensor_rearranges_eq8_into_eq1(oracle):
     far = oracle.N_at((9 * a, 7 * a, 5 * a), (a, a, a))
     Tf = oracle.dipole_table((10, 8, 6), a)[:, 5, 7, 9]
     assert np.abs(far - Tf).max() <= 2e-3 * np.abs(Tf).max()                  # cube -> point dipole, O((a/r)^4)
+
+
+def test_periodic_tensor_table_invariants_and_film_limit(oracle):
+    """oracle.periodic_tensor_table (reading R11).  Pins: (i) trace identity Nxx + Nyy + Nzz = delta(d) survives the image
+    sum (only the m = 0 image of d = 0 has r = 0); (ii) exact symmetry T(n - d) = parity T(d) on periodic axes, open axes
+    untouched; (iii) the symmetrised sum equals the image sum over m = -I-1 .. I with weight 1/2 on the two end images
+    for d > 0, the plain sum over |m| <= I for d = 0 (parity N(-x) = N(x)); (iv) physics: with x and y periodic, a uniformly z-magnetised mesh is a square plate of side
+    L = (2 I + 1) n h seen from its centre, whose demagnetizing factor is 1 - Omega / 2 pi -> 1 - (2 sqrt2 / pi) t / L for
+    a thin plate (solid angle of a square from a point t/2 above its centre): sum_d Tzz(d) tends to the infinite film's 1
+    at exactly that rate."""
+    h = (2e-9, 3e-9, 1e-9)
+    n, pbc, I = (4, 3, 2), (True, False, True), 2
+    T = oracle.periodic_tensor_table(n, h, pbc, I)
+    tr = T[0] + T[1] + T[2]
+    assert abs(tr[0, 0, 0] - 1) < 1e-12 and np.abs(tr.reshape(-1)[1:]).max() < 1e-12
+    for a, ax in ((0, 3), (2, 1)):
+        idx = (-np.arange(n[a])) % n[a]
+        assert np.abs(T - oracle.PARITY[:, a].reshape(6, 1, 1, 1) * np.take(T, idx, axis=ax)).max() < 1e-15
+    Topen = oracle.tensor_table((1, 3, 1), h)
+    assert np.abs(oracle.periodic_tensor_table((1, 3, 1), h, (False, False, False), 5) - Topen).max() == 0
+    W = np.zeros_like(T)
+    wt = lambda m, d: 1.0 if d == 0 else 0.5 if m in (-I - 1, I) else 1.0
+    for dz in range(n[2]):
+        for dy in range(n[1]):
+            for dx in range(n[0]):
+                for mx in range(-I - (dx > 0), I + 1):
+                    for mz in range(-I - (dz > 0), I + 1):
+                        W[:, dz, dy, dx] += wt(mx, dx) * wt(mz, dz) * oracle.N_at(((dx + mx * n[0]) * h[0], dy * h[1], (dz + mz * n[2]) * h[2]), h)
+    assert np.abs(W - T).max() < 1e-13
+    # (iv) the film limit, cube cells of edge t, mesh 2 x 2 x 1
+    t = 1e-9
+    for I in (6, 12):
+        Tf = oracle.periodic_tensor_table((2, 2, 1), (t, t, t), (True, True, False), I)
+        L = (2 * I + 1) * 2 * t
+        deficit = 1.0 - Tf[2].sum()
+        assert 0 < deficit < 0.1
+        assert abs(deficit / (2 * np.sqrt(2) / np.pi * t / L) - 1) < 0.05, (I, deficit, 2 * np.sqrt(2) / np.pi * t / L)
