@@ -62,7 +62,7 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz,
 /* Compute and store the transformed tensor ("convolution kernel ... computed in the initialization
  * stage"; stored packed by its y/z symmetries as real arrays).
  *   N6_host == NULL: built-in fp64 Newell builder on the GPU ("formulas in Ref. [23]";
- *                    DESIGN.md R1, R4).  DEMAG_ERR_UNSUPPORTED if any PBC flag is set.
+ *                    DESIGN.md R1, R4).  With PBC flags: the periodic tensor of demag_set_pbc_images.
  *   N6_host != NULL: host array double[6][nz][ny][nx]: N_c at the non-negative cell offsets
  *                    (dx,dy,dz); negative offsets follow by parity (diagonal even; xy odd in x,y;
  *                    xz odd in x,z; yz odd in y,z).  On a PBC axis the n_a entries are the periodic
@@ -72,6 +72,14 @@ demag_status demag_plan_create(demag_plan_t* out, int nx, int ny, int nz,
  * The spectrum is computed in fp64, the factor -1/(Nx Ny Nz) is folded in (R3), and it is
  * rounded once to fp32 (kept fp64 for a DEMAG_FP64 plan).  Synchronous (plan-time call). */
 demag_status demag_set_kernel(demag_plan_t plan, const double* N6_host);
+
+/* Built-in periodic tensor ("modified convolution kernel"; the paper's reference [25] is not available,
+ * DESIGN.md R11 states the reading): on every periodic axis a the open-boundary tensor is summed over `images` periodic
+ * images on each side, T(d) = sum_{|m_a| <= images} N((d_a + m_a n_a) h_a), and symmetrised under d_a -> n_a - d_a
+ * (indices mod n_a; a periodic kernel is symmetric up to the component's parity, the truncated sum only up to its
+ * last images), which for d_a > 0 amounts to weight 1/2 on the images m_a = -images-1 and m_a = images.  Default 10; 0..1000.  Takes effect at the
+ * next demag_set_kernel(plan, NULL) / demag_get_kernel_real.  Cost grows with (2 images + 2)^(periodic axes). */
+demag_status demag_set_pbc_images(demag_plan_t plan, int images);
 
 /* H = -N * M  (Eq. (1); execution order of Appendix A).
  * M_dev, H_dev: device arrays [3][nz][ny][nx] of the plan's precision.  Asynchronous on the stream.

@@ -23,7 +23,8 @@ EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy
            "demag_get_kernel_real", "demag_workspace_bytes", "demag_set_slab", "demag_launches_per_apply",
            "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path", "demag_apply_add",
            "demag_shard_range", "demag_plan_create_sharded", "demag_shard_info", "demag_shard_buffers",
-           "demag_shard_ipc_export", "demag_shard_ipc_connect", "demag_shard_set_peers", "demag_apply_sharded"]
+           "demag_shard_ipc_export", "demag_shard_ipc_connect", "demag_shard_set_peers", "demag_apply_sharded",
+           "demag_set_pbc_images"]
 
 
 class DemagError(RuntimeError):
@@ -67,6 +68,7 @@ def lib():
         L.demag_path.restype = i
         L.demag_last_error.restype = ctypes.c_char_p
         L.demag_plan_destroy.argtypes = [vp]
+        L.demag_set_pbc_images.argtypes = [vp, i]
         L.demag_shard_range.argtypes = [i, i, i, i, vp, vp]
         L.demag_plan_create_sharded.argtypes = [ctypes.POINTER(vp), i, i, i, d, d, d, u, i, i, i]
         L.demag_shard_info.argtypes = [vp, vp, vp, vp, vp, vp, vp]
@@ -148,6 +150,10 @@ def demag_workspace_bytes(plan) -> int:
 
 def demag_set_slab(plan, kx_per_slab: int):
     _check(lib().demag_set_slab(plan, int(kx_per_slab)))
+
+
+def demag_set_pbc_images(plan, images: int):
+    _check(lib().demag_set_pbc_images(plan, int(images)))
 
 
 def demag_launches_per_apply(plan) -> int:
@@ -336,6 +342,9 @@ class Plan:
 
     def set_slab(self, k):
         demag_set_slab(self.handle, k)
+
+    def set_pbc_images(self, images):
+        demag_set_pbc_images(self.handle, images)
 
     def close(self):
         if self.handle:

@@ -116,16 +116,9 @@ __device__ inline void series_N(double X, double Y, double Z, double hx, double 
 
 #define DEMAG_BUILDER_R_NEAR 24.0
 
-__global__ void __launch_bounds__(128) k_tensor_table(int nx, int ny, int nz, double hx, double hy, double hz,
-                                                      double* __restrict__ T)
+__device__ inline void tensor_at(double X, double Y, double Z, double hx, double hy, double hz, double* N6)
 {
-    const size_t nc = (size_t)nx * ny * nz;
-    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
-    if (i >= nc) return;
-    const int dx = (int)(i % nx), dy = (int)((i / nx) % ny), dz = (int)(i / ((size_t)nx * ny));
-    const double X = dx * hx, Y = dy * hy, Z = dz * hz;
     const double hm = fmax(hx, fmax(hy, hz));
-    double N6[6];
     if (sqrt(X * X + Y * Y + Z * Z) <= DEMAG_BUILDER_R_NEAR * hm) {
         N6[0] = nw_stencil<false>(X, Y, Z, hx, hy, hz);
         N6[1] = nw_stencil<false>(Y, X, Z, hy, hx, hz);
@@ -136,7 +129,52 @@ __global__ void __launch_bounds__(128) k_tensor_table(int nx, int ny, int nz, do
     } else {
         series_N(X, Y, Z, hx, hy, hz, N6);
     }
+}
+
+__global__ void __launch_bounds__(128) k_tensor_table(int nx, int ny, int nz, double hx, double hy, double hz,
+                                                      double* __restrict__ T)
+{
+    const size_t nc = (size_t)nx * ny * nz;
+    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (i >= nc) return;
+    const int dx = (int)(i % nx), dy = (int)((i / nx) % ny), dz = (int)(i / ((size_t)nx * ny));
+    double N6[6];
+    tensor_at(dx * hx, dy * hy, dz * hz, hx, hy, hz, N6);
     for (int c = 0; c < 6; ++c) T[c * nc + i] = N6[c];
+}
+
+// Periodic axes ("modified convolution kernel"; R11): the open-boundary tensor summed over
+// `img` periodic images on each side of every periodic axis a (period n_a h_a), and the result symmetrised,
+//   T(d) = sym_a [ sum_{|m_a| <= img} N((d_a + m_a n_a) h_a) ],   sym_a f(d_a) = ( f(d_a) + parity_a f(n_a - d_a) ) / 2,
+// (indices mod n_a, so d_a = 0 maps to itself) because a periodic kernel obeys K(n_a - d_a) = parity_a K(d_a) and the
+// truncated sum does so only up to its last images.  Since parity_a N(-x) = N(x), for d_a > 0 the symmetrised sum is the
+// image sum over m_a = -img-1 .. img with weight 1/2 on the two end images; for d_a = 0 it is the plain sum over
+// |m_a| <= img.  That is what the loops below evaluate.  img[a] < 0 marks an open axis (m_a = 0 only).
+__global__ void __launch_bounds__(128) k_tensor_table_pbc(int nx, int ny, int nz, double hx, double hy, double hz,
+                                                          int ix, int iy, int iz, double* __restrict__ T)
+{
+    const size_t nc = (size_t)nx * ny * nz;
+    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (i >= nc) return;
+    const int dx = (int)(i % nx), dy = (int)((i / nx) % ny), dz = (int)(i / ((size_t)nx * ny));
+    const bool ex = ix >= 0 && dx > 0, ey = iy >= 0 && dy > 0, ez = iz >= 0 && dz > 0;   // half-weight end images
+    const int x0 = ix < 0 ? 0 : -ix - (ex ? 1 : 0), x1 = ix < 0 ? 0 : ix;
+    const int y0 = iy < 0 ? 0 : -iy - (ey ? 1 : 0), y1 = iy < 0 ? 0 : iy;
+    const int z0 = iz < 0 ? 0 : -iz - (ez ? 1 : 0), z1 = iz < 0 ? 0 : iz;
+    double acc[6] = {0, 0, 0, 0, 0, 0};
+    for (int mz = z0; mz <= z1; ++mz) {
+        const double wz = (ez && (mz == z0 || mz == z1)) ? 0.5 : 1.0;
+        for (int my = y0; my <= y1; ++my) {
+            const double wy = wz * ((ey && (my == y0 || my == y1)) ? 0.5 : 1.0);
+            for (int mx = x0; mx <= x1; ++mx) {
+                const double w = wy * ((ex && (mx == x0 || mx == x1)) ? 0.5 : 1.0);
+                double N6[6];
+                tensor_at((dx + (double)mx * nx) * hx, (dy + (double)my * ny) * hy, (dz + (double)mz * nz) * hz, hx, hy, hz, N6);
+                for (int c = 0; c < 6; ++c) acc[c] += w * N6[c];
+            }
+        }
+    }
+    for (int c = 0; c < 6; ++c) T[c * nc + i] = acc[c];
 }
 
 // ---------------------------------------------------------------- spectrum of the extended tensor

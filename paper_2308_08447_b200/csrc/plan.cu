@@ -55,6 +55,7 @@ struct demag_plan_s {
     Geo g;
     double h[3];
     unsigned pbc;
+    int pbc_images = 10;   // built-in periodic tensor: images summed on each side of a periodic axis (demag_set_pbc_images)
     int prec;
     size_t esz;       // sizeof real
     int device;
@@ -504,6 +505,15 @@ int demag_launches_per_apply(demag_plan_t p)
 
 int demag_path(demag_plan_t p) { return p && p->v2 ? 1 : 0; }
 
+demag_status demag_set_pbc_images(demag_plan_t p, int images)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (images < 0 || images > 1000) return fail(DEMAG_ERR_INVALID_ARG, "images must be in 0..1000");
+    p->pbc_images = images;
+    return DEMAG_OK;
+}
+
 }  // extern "C"
 
 // ================================================================================ plan-time: kernel
@@ -516,6 +526,11 @@ demag_status build_table_dev(demag_plan_s* p, double** T_out)
     const size_t nc = (size_t)g.nx * g.ny * g.nz;
     double* T = nullptr;
     CUDA_TRY(cudaMalloc(&T, 6 * nc * sizeof(double)));
+    if (p->pbc) {
+        const int im = p->pbc_images;
+        k_tensor_table_pbc<<<(unsigned)((nc + 127) / 128), 128>>>(g.nx, g.ny, g.nz, p->h[0], p->h[1], p->h[2],
+            (p->pbc & DEMAG_PBC_X) ? im : -1, (p->pbc & DEMAG_PBC_Y) ? im : -1, (p->pbc & DEMAG_PBC_Z) ? im : -1, T);
+    } else
     k_tensor_table<<<(unsigned)((nc + 127) / 128), 128>>>(g.nx, g.ny, g.nz, p->h[0], p->h[1], p->h[2], T);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -555,7 +570,6 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
 {
     g_err[0] = 0;
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
-    if (!N6_host && p->pbc) return fail(DEMAG_ERR_UNSUPPORTED, "built-in tensor builder does not support PBC");
     const Geo& g = p->g;
     const size_t nc = (size_t)g.nx * g.ny * g.nz;
     static const int par[6][3] = {{1, 1, 1}, {1, 1, 1}, {1, 1, 1}, {-1, -1, 1}, {-1, 1, -1}, {1, -1, -1}};
@@ -635,7 +649,6 @@ extern "C" demag_status demag_get_kernel_real(demag_plan_t p, double* N6_host)
 {
     g_err[0] = 0;
     if (!p || !N6_host) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
-    if (p->pbc) return fail(DEMAG_ERR_UNSUPPORTED, "built-in tensor builder does not support PBC");
     double* T = nullptr;
     demag_status st = build_table_dev(p, &T);
     if (st) return st;
