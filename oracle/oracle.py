@@ -17,6 +17,7 @@ Citations are ``PAPER.md:<line>`` (arXiv 2308.08447) or a DESIGN.md reading (R<n
     macrocell_scatter   "applied equally to all spins" (PAPER.md:133; R14)           [NumPy]
     dipole_table        point-dipole tensor that turns Eq. (8) into Eq. (1)   [NumPy]
     dipole_field_eq8    Eq. (8) written out, O(n^2)                [NumPy]
+    poly_extrapolate    polynomial through previously computed fields, evaluated at a sub-step time (R19)  [NumPy]
     periodic_tensor_table  image-summed, symmetrised tensor on periodic axes (R11)   [NumPy loops over N_at]
 
 All of them are pinned in tests/test_oracle_pins.py; none is "parity unpinned".
@@ -318,3 +319,23 @@ def periodic_tensor_table(n, h, pbc, images) -> np.ndarray:
             idx = (-np.arange((nx, ny, nz)[a])) % (nx, ny, nz)[a]
             T = 0.5 * (T + PARITY[:, a].reshape(6, 1, 1, 1) * np.take(T, idx, axis=ax))
     return T
+
+
+def poly_extrapolate(H_hist, t_hist, t) -> np.ndarray:
+    """Demagnetizing field at a sub-step time t from previously computed fields ("polynomial extrapolation
+    of the demagnetizing field at sub-steps of the higher order evaluation method, using previously computed values ...
+    the RK4 method requires a quartic polynomial, whilst the RKF56 method requires a quintic polynomial"; reading R19):
+    the unique polynomial of degree p through the p+1 samples (t_k, H_k), every field entry on its own, in Lagrange form
+
+        H(t) = sum_k L_k(t) H_k,      L_k(t) = prod_{j != k} (t - t_j) / (t_k - t_j).
+
+    H_hist: sequence of p+1 equally shaped arrays; t_hist: p+1 distinct times."""
+    ts = [float(v) for v in t_hist]
+    out = np.zeros_like(np.asarray(H_hist[0], dtype=np.float64))
+    for k, Hk in enumerate(H_hist):
+        Lk = 1.0
+        for j, tj in enumerate(ts):
+            if j != k:
+                Lk *= (float(t) - tj) / (ts[k] - tj)
+        out += Lk * np.asarray(Hk, dtype=np.float64)
+    return out

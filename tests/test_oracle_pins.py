@@ -370,3 +370,26 @@ def test_periodic_tensor_table_invariants_and_film_limit(oracle):
         deficit = 1.0 - Tf[2].sum()
         assert 0 < deficit < 0.1
         assert abs(deficit / (2 * np.sqrt(2) / np.pi * t / L) - 1) < 0.05, (I, deficit, 2 * np.sqrt(2) / np.pi * t / L)
+
+
+def test_poly_extrapolate_reproduces_polynomials(oracle):
+    """oracle.poly_extrapolate (R19).  Pins: a field whose entries ARE polynomials in t of degree <= p is
+    reproduced exactly at any time from p+1 samples (quartic for RK4: 5 samples; quintic for RKF56: 6), and not from
+    p samples; at a sample time the sample itself comes back; the result equals NumPy's least-squares polynomial fit
+    of the same degree (which interpolates when the system is square)."""
+    rng = np.random.default_rng(7)
+    for p in (4, 5):
+        coef = rng.normal(size=(p + 1, 3, 2, 3, 4))
+        f = lambda t: sum(coef[d] * t ** d for d in range(p + 1))
+        ts = np.sort(rng.uniform(0.0, 1.0, p + 1))
+        H = [f(t) for t in ts]
+        for t in (1.3, 0.5 * (ts[0] + ts[1]), -0.2):
+            assert np.abs(oracle.poly_extrapolate(H, ts, t) - f(t)).max() <= 1e-9 * np.abs(f(t)).max()
+        assert np.abs(oracle.poly_extrapolate(H[1:], ts[1:], 1.3) - f(1.3)).max() > 1e-4      # one sample short: not exact
+        assert np.abs(oracle.poly_extrapolate(H, ts, ts[2]) - H[2]).max() <= 1e-12 * np.abs(H[2]).max()
+        flat = np.stack([h.reshape(-1) for h in H])
+        fit = np.polynomial.polynomial.polyfit(ts, flat, p)
+        ref = np.polynomial.polynomial.polyval(1.3, fit).reshape(H[0].shape)
+        assert np.abs(oracle.poly_extrapolate(H, ts, 1.3) - ref).max() <= 1e-7 * np.abs(ref).max()
+    one = oracle.poly_extrapolate([np.full((2, 2), 3.0)], [0.1], 9.0)                          # degree 0: constant
+    assert np.array_equal(one, np.full((2, 2), 3.0))
