@@ -91,6 +91,21 @@ demag_status demag_apply(demag_plan_t plan, const void* M_dev, void* H_dev, void
  * Same arguments, layout and errors as demag_apply; Heff_dev is read and written. */
 demag_status demag_apply_add(demag_plan_t plan, const void* M_dev, void* Heff_dev, void* cuda_stream);
 
+/* Polynomial extrapolation of the demagnetizing field at sub-steps of the time integrator ("polynomial
+ * extrapolation of the demagnetizing field at sub-steps of the higher order evaluation method, using previously computed
+ * values ... the RK4 method requires a quartic polynomial, whilst the RKF56 method requires a quintic polynomial";
+ * DESIGN.md R19): the polynomial of degree npts-1 through the npts previously computed fields, evaluated at time t,
+ *     H(t) = sum_k L_k(t) H_k,   L_k(t) = prod_{j != k} (t - t_j) / (t_k - t_j)        (every array entry on its own),
+ * written to H_out_dev (accumulate == 0) or added to it (accumulate != 0: H_out is then H_eff), in ONE streaming pass
+ * that replaces a whole convolution at that sub-step.
+ *   H_hist_dev:  host array of npts device pointers, each [3][nz][ny][nx] of the plan's precision (this rank's rows for a
+ *                sharded plan), 16-byte aligned, none overlapping H_out_dev;   1 <= npts <= 8 (quartic: 5, quintic: 6).
+ *   t_hist_host: host array of the npts distinct sample times; t: the time wanted (any unit, only ratios enter).
+ * The weights are evaluated on the host in extended precision; the device sums in the plan's precision with FMAs.
+ * Asynchronous on the stream; the host arrays are read before the call returns. */
+demag_status demag_extrapolate(demag_plan_t plan, int npts, const void* const* H_hist_dev, const double* t_hist_host,
+                               double t, void* H_out_dev, int accumulate, void* cuda_stream);
+
 /* Demagnetizing energy  E = -(mu0/2) hx hy hz sum_i M_i . H_i  [J] (R12), accumulated in
  * fp64 and written to the device scalar *E_dev (double).  Asynchronous on the stream. */
 demag_status demag_energy(demag_plan_t plan, const void* M_dev, const void* H_dev,

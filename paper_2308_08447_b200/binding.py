@@ -24,7 +24,7 @@ EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy
            "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path", "demag_apply_add",
            "demag_shard_range", "demag_plan_create_sharded", "demag_shard_info", "demag_shard_buffers",
            "demag_shard_ipc_export", "demag_shard_ipc_connect", "demag_shard_set_peers", "demag_apply_sharded",
-           "demag_set_pbc_images"]
+           "demag_set_pbc_images", "demag_extrapolate"]
 
 
 class DemagError(RuntimeError):
@@ -69,6 +69,7 @@ def lib():
         L.demag_last_error.restype = ctypes.c_char_p
         L.demag_plan_destroy.argtypes = [vp]
         L.demag_set_pbc_images.argtypes = [vp, i]
+        L.demag_extrapolate.argtypes = [vp, i, vp, vp, d, vp, i, vp]
         L.demag_shard_range.argtypes = [i, i, i, i, vp, vp]
         L.demag_plan_create_sharded.argtypes = [ctypes.POINTER(vp), i, i, i, d, d, d, u, i, i, i]
         L.demag_shard_info.argtypes = [vp, vp, vp, vp, vp, vp, vp]
@@ -126,6 +127,14 @@ def demag_apply_profiled(plan, M, H, stream=None):
     _check(lib().demag_apply_profiled(plan, M.data_ptr(), H.data_ptr(), _stream(stream),
                                       ctypes.addressof(ms), ctypes.addressof(cnt)))
     return list(ms), list(cnt)
+
+
+def demag_extrapolate(plan, H_hist, t_hist, t, H_out, accumulate=False, stream=None):
+    n = len(H_hist)
+    ptrs = (ctypes.c_void_p * n)(*[h.data_ptr() for h in H_hist])
+    ts = (ctypes.c_double * n)(*[float(v) for v in t_hist])
+    _check(lib().demag_extrapolate(plan, n, ctypes.addressof(ptrs), ctypes.addressof(ts), float(t), H_out.data_ptr(),
+                                   int(bool(accumulate)), _stream(stream)))
 
 
 def demag_energy(plan, M, H, E, stream=None):
@@ -324,6 +333,9 @@ class Plan:
 
     def energy(self, M, H, E, stream=None):
         demag_energy(self.handle, M, H, E, stream)
+
+    def extrapolate(self, H_hist, t_hist, t, H_out, accumulate=False, stream=None):
+        demag_extrapolate(self.handle, H_hist, t_hist, t, H_out, accumulate, stream)
 
     def apply_atomistic(self, S, Hs, c, mu_s, a, accumulate=False, stream=None):
         demag_apply_atomistic(self.handle, S, Hs, c, mu_s, a, accumulate, stream)

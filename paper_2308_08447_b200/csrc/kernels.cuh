@@ -378,6 +378,43 @@ __global__ void __launch_bounds__(512, ((LRF == 3 || sizeof(T) == 8) ? 1 : 2)) k
 
 // ------------------------------------------------------------------------------------------ energy
 // E += -(mu0/2) V sum M.H over this block's cells (fp64 accumulation; R12).
+// Polynomial extrapolation of the demagnetizing field at a sub-step of the time integrator (DESIGN.md
+// R19):  out (+)= sum_k w[k] H_k  over NP previously computed fields, w = the Lagrange weights L_k(t), computed on the
+// host in fp64.  One streaming pass: NP reads (+1 when accumulating) and one write per element, 16-byte accesses.
+constexpr int kMaxHist = 8;
+template <typename T> struct ExtrapArgs { const T* H[kMaxHist]; T w[kMaxHist]; };
+template <typename T, int NP>
+__global__ void __launch_bounds__(256) k_extrapolate(size_t n, ExtrapArgs<T> a, T* __restrict__ out, int acc)
+{
+    constexpr int V = 16 / (int)sizeof(T);
+    struct alignas(16) Vec { T v[V]; };
+    const size_t nvec = n / V;
+    const size_t stride = (size_t)gridDim.x * blockDim.x, i0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    for (size_t i = i0; i < nvec; i += stride) {
+        Vec h[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) h[k] = reinterpret_cast<const Vec*>(a.H[k])[i];
+        Vec r;
+        if (acc) r = reinterpret_cast<const Vec*>(out)[i];
+        else {
+#pragma unroll
+            for (int e = 0; e < V; ++e) r.v[e] = (T)0;
+        }
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+#pragma unroll
+            for (int e = 0; e < V; ++e) r.v[e] = fma(a.w[k], h[k].v[e], r.v[e]);
+        }
+        reinterpret_cast<Vec*>(out)[i] = r;
+    }
+    for (size_t i = nvec * V + i0; i < n; i += stride) {          // tail (n not a multiple of the vector width)
+        T r = acc ? out[i] : (T)0;
+#pragma unroll
+        for (int k = 0; k < NP; ++k) r = fma(a.w[k], a.H[k][i], r);
+        out[i] = r;
+    }
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256) k_energy(size_t n3, const T* __restrict__ M, const T* __restrict__ H,
                                                 double scale, double* __restrict__ E)

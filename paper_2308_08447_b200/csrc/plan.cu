@@ -1003,6 +1003,54 @@ extern "C" demag_status demag_energy(demag_plan_t p, const void* M_dev, const vo
     return DEMAG_OK;
 }
 
+namespace {
+template <typename T>
+demag_status extrapolate_impl(demag_plan_s* p, int npts, const void* const* H, const double* w, void* out, int acc,
+                              size_t n, cudaStream_t st)
+{
+    ExtrapArgs<T> a;
+    for (int k = 0; k < kMaxHist; ++k) { a.H[k] = k < npts ? (const T*)H[k] : nullptr; a.w[k] = k < npts ? (T)w[k] : (T)0; }
+    const unsigned grid = (unsigned)std::min<size_t>((n / (16 / sizeof(T)) + 255) / 256 + 1, (size_t)p->sm_count * 8);
+    switch (npts) {
+#define DEMAG_EXTRAP_CASE(NP) case NP: k_extrapolate<T, NP><<<grid, 256, 0, st>>>(n, a, (T*)out, acc); break;
+        DEMAG_EXTRAP_CASE(1) DEMAG_EXTRAP_CASE(2) DEMAG_EXTRAP_CASE(3) DEMAG_EXTRAP_CASE(4)
+        DEMAG_EXTRAP_CASE(5) DEMAG_EXTRAP_CASE(6) DEMAG_EXTRAP_CASE(7) DEMAG_EXTRAP_CASE(8)
+#undef DEMAG_EXTRAP_CASE
+    }
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}
+}  // namespace
+
+extern "C" demag_status demag_extrapolate(demag_plan_t p, int npts, const void* const* H_hist_dev, const double* t_hist_host,
+                                          double t, void* H_out_dev, int accumulate, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!p || !H_hist_dev || !t_hist_host || !H_out_dev) return fail(DEMAG_ERR_INVALID_ARG, "NULL argument");
+    if (npts < 1 || npts > kMaxHist) return fail(DEMAG_ERR_INVALID_ARG, "npts must be in 1..%d", kMaxHist);
+    if (!isfinite(t)) return fail(DEMAG_ERR_INVALID_ARG, "t is not finite");
+    const size_t n = (size_t)3 * p->on[0] * (p->sharded ? p->ny_loc : p->on[1]) * p->on[2];
+    const size_t bytes = n * p->esz;
+    if ((uintptr_t)H_out_dev & 15) return fail(DEMAG_ERR_INVALID_ARG, "device pointers must be 16-byte aligned");
+    double w[kMaxHist];
+    for (int k = 0; k < npts; ++k) {
+        if (!H_hist_dev[k] || ((uintptr_t)H_hist_dev[k] & 15)) return fail(DEMAG_ERR_INVALID_ARG, "field %d is NULL or not 16-byte aligned", k);
+        const char *pa = (const char*)H_hist_dev[k], *pb = (const char*)H_out_dev;
+        if (pa < pb + bytes && pb < pa + bytes) return fail(DEMAG_ERR_INVALID_ARG, "field %d overlaps the output", k);
+        if (!isfinite(t_hist_host[k])) return fail(DEMAG_ERR_INVALID_ARG, "time %d is not finite", k);
+        long double L = 1.0L;                                  // Lagrange weight L_k(t), PAPER.md:96 / R19
+        for (int j = 0; j < npts; ++j) {
+            if (j == k) continue;
+            if (t_hist_host[j] == t_hist_host[k]) return fail(DEMAG_ERR_INVALID_ARG, "times %d and %d coincide", j, k);
+            L *= ((long double)t - t_hist_host[j]) / ((long double)t_hist_host[k] - t_hist_host[j]);
+        }
+        w[k] = (double)L;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return p->prec == DEMAG_FP32 ? extrapolate_impl<float>(p, npts, H_hist_dev, w, H_out_dev, accumulate != 0, n, st)
+                                 : extrapolate_impl<double>(p, npts, H_hist_dev, w, H_out_dev, accumulate != 0, n, st);
+}
+
 extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev, void* Hs_dev, int cx, int cy, int cz,
                                               double mu_s_in_muB, double a, int accumulate, void* cuda_stream)
 {

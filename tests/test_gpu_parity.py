@@ -314,6 +314,79 @@ def test_dipole_dipole_field_through_set_kernel(torch, B, oracle, L, prec):
     assert np.abs(H - ref).max() / Ms <= (TOL32 if prec == 0 else TOL64)
 
 
+# --------------------------------------------------------------------------------- sub-step extrapolation
+@pytest.mark.parametrize("n", [(12, 10, 3), (5, 3, 1), (64, 32, 8)])
+@pytest.mark.parametrize("npts", [1, 2, 5, 6, 8])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_extrapolate_against_oracle(torch, B, oracle, n, npts, prec):
+    """demag_extrapolate == oracle.poly_extrapolate (the Lagrange polynomial through npts fields) entry by entry,
+    overwrite and accumulate modes, vector body and scalar tail (3 n_c not a multiple of 4).  Tolerance from the
+    arithmetic: npts FMAs and one rounding of each weight, (npts + 2) eps sum_k |L_k| max|H_k|."""
+    rng = np.random.default_rng(70 + npts + sum(n))
+    dt = torch.float32 if prec == 0 else torch.float64
+    npd = np.float32 if prec == 0 else np.float64
+    shape = (3, n[2], n[1], n[0])
+    ts = np.sort(rng.uniform(0.0, 1.0, npts)) + np.arange(npts) * 0.05
+    t = ts[-1] + 0.37 * (ts[-1] - ts[0] + 0.1)
+    H = [(rng.normal(size=shape) * 8e5).astype(npd) for _ in range(npts)]
+    ref = oracle.poly_extrapolate([h.astype(np.float64) for h in H], ts, t)
+    Lk = [np.prod([(t - tj) / (tk - tj) for j, tj in enumerate(ts) if j != k]) for k, tk in enumerate(ts)]
+    S = sum(abs(l) * np.abs(h).max() for l, h in zip(Lk, H))
+    tol = (npts + 2) * np.finfo(npd).eps * S
+    with B.Plan(n, (2e-9, 2e-9, 2e-9), 0, prec) as p:
+        Hd = [torch.from_numpy(h).cuda() for h in H]
+        out = torch.full(shape, float("nan"), dtype=dt, device="cuda")
+        p.extrapolate(Hd, ts, t, out)
+        torch.cuda.synchronize()
+        assert np.abs(out.cpu().numpy().astype(np.float64) - ref).max() <= tol
+        base = (rng.normal(size=shape) * 1e5).astype(npd)
+        acc = torch.from_numpy(base).cuda()
+        p.extrapolate(Hd, ts, t, acc, accumulate=True)
+        torch.cuda.synchronize()
+        assert np.abs(acc.cpu().numpy().astype(np.float64) - (ref + base.astype(np.float64))).max() <= tol + np.finfo(npd).eps * np.abs(ref).max()
+        for h, h0 in zip(Hd, H):
+            assert np.array_equal(h.cpu().numpy(), h0)                       # the history is read only
+
+
+def test_extrapolated_field_follows_a_rotating_magnetisation(torch, B, oracle):
+    """What the hook is for: fields computed at 5 past times, a quartic through them evaluated at a sub-step
+    half a step ahead, against the convolution actually carried out at that time.  M rotates by 0.1 rad per step, so
+    the quartic's error is O(0.1^5)."""
+    n, h, Ms = (32, 16, 4), (2e-9, 2e-9, 2e-9), 8e5
+    rng = np.random.default_rng(3)
+    phi = rng.uniform(0, 2 * np.pi, size=(n[2], n[1], n[0]))
+    Mt = lambda t: (Ms * np.stack([np.cos(phi + t), np.sin(phi + t), np.zeros_like(phi)])).astype(np.float32)
+    ts = [0.1 * k for k in range(5)]
+    with B.Plan(n, h, 0, 0) as p:
+        p.set_kernel(oracle.tensor_table(n, h))
+        Hs = []
+        for t in ts + [0.45]:
+            Md = torch.from_numpy(Mt(t)).cuda(); Hd = torch.empty_like(Md)
+            p.apply(Md, Hd)
+            Hs.append(Hd)
+        out = torch.empty_like(Hs[0])
+        p.extrapolate(Hs[:5], ts, 0.45, out)
+        torch.cuda.synchronize()
+        err = float((out - Hs[5]).abs().max()) / Ms
+        assert err < 2e-5, err
+        p.extrapolate(Hs[3:5], ts[3:5], 0.45, out)                          # a straight line through two fields is far worse
+        torch.cuda.synchronize()
+        assert float((out - Hs[5]).abs().max()) / Ms > 20 * err
+
+
+def test_extrapolate_error_paths(torch, B):
+    with B.Plan((8, 8, 2), (1e-9,) * 3) as p:
+        H = [torch.zeros((3, 2, 8, 8), device="cuda") for _ in range(9)]
+        out = torch.zeros_like(H[0])
+        for hist, ts in [([], []), (H, list(range(9))), (H[:2], [0.5, 0.5]), (H[:2], [0.0, float("nan")]), ([out, H[0]], [0, 1])]:
+            with pytest.raises(B.DemagError) as e:
+                p.extrapolate(hist, ts, 2.0, out)
+            assert e.value.status == 1
+        with pytest.raises(B.DemagError) as e:
+            B._check(B.lib().demag_extrapolate(p.handle, 1, None, None, 0.0, out.data_ptr(), 0, None))
+        assert e.value.status == 1
+
+
 # --------------------------------------------------------------------------------- accumulate into H_eff
 @pytest.mark.parametrize("n", [(32, 16, 8), (64, 32, 1), (12, 10, 3), (1, 8, 4), (4, 4, 2)])
 @pytest.mark.parametrize("prec", [0, 1])
