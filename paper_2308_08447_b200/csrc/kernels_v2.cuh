@@ -3,7 +3,7 @@
 // (x R2C -> y FFT -> z FFT . kernel multiplication . z IFFT -> y IFFT -> x C2R), different
 // data layout of the private workspaces:
 //
-//   W1v [3][nz][hq][ny] quads   one quad = x-frequencies (k, Lc-k) of one (y,z): the pair the Hermitian split of
+//   W1v [3][hq][nz][ny] quads   one quad = x-frequencies (k, Lc-k) of one (y,z): the pair the Hermitian split of
 //                               the real transform produces / consumes together (hq = Lc/2 + 1, Lc = Nx/2 = nx)
 //   W2v [3][nq][nz][Ny] quads   slab of nq pairs; y in the digit-reversed "position order" the forward passes
 //                               leave behind (the stored kernel spectrum uses the same order: nothing is permuted)

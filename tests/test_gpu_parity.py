@@ -538,3 +538,66 @@ def test_error_paths(torch, B):
             with pytest.raises(B.DemagError) as e:
                 p.set_pbc_images(bad)
             assert e.value.status == 1                  # image count out of range
+
+
+# --------------------------------------------------------------------------------- stream semantics of the hot path
+def test_apply_is_capturable_in_a_cuda_graph(torch, B, oracle):
+    """include/demag.h: demag_apply "never allocates, never synchronises, never touches the host" -- so a time
+    integrator can capture it (and demag_apply_add / demag_extrapolate / demag_energy) into a CUDA graph.  The replayed
+    graph must give the eager result bit for bit, for both kernel families and an embedded mesh."""
+    for n in [(32, 32, 2), (64, 32, 8), (12, 10, 3), (64, 64, 1)]:
+        h, Ms = (2e-9, 2e-9, 2e-9), 8e5
+        M = rand_M(n, Ms, 17)
+        with B.Plan(n, h, 0, 0) as p:
+            p.set_kernel(None)
+            Md = torch.from_numpy(M).cuda()
+            H0, H1, Heff = torch.empty_like(Md), torch.empty_like(Md), torch.zeros_like(Md)
+            E = torch.zeros(1, dtype=torch.float64, device="cuda")
+            p.apply(Md, H0); torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                with torch.cuda.graph(g, stream=s):
+                    p.apply(Md, H1)
+                    p.apply_add(Md, Heff)
+                    p.energy(Md, H1, E)
+            Md.copy_(torch.from_numpy(rand_M(n, Ms, 18)).cuda())          # new input, same addresses
+            p.apply(Md, H0); torch.cuda.synchronize()
+            for rep in range(3):
+                g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(H0, H1)
+            assert torch.allclose(Heff, 3 * H0, rtol=1e-5, atol=1e-5 * Ms)
+            assert abs(E.item() - oracle.energy(Md.cpu().numpy().astype(np.float64), H0.cpu().numpy().astype(np.float64), h)) <= 1e-6 * abs(E.item())
+
+
+def test_two_plans_on_two_streams_do_not_interfere(torch, B, oracle):
+    n, h, Ms = (64, 64, 8), (2e-9, 2e-9, 2e-9), 8e5
+    Ma, Mb = rand_M(n, Ms, 1), rand_M(n, Ms, 2)
+    with B.Plan(n, h, 0, 0) as pa, B.Plan(n, h, 0, 0) as pb:
+        pa.set_kernel(None); pb.set_kernel(None)
+        A, Bm = torch.from_numpy(Ma).cuda(), torch.from_numpy(Mb).cuda()
+        Ha0, Hb0 = torch.empty_like(A), torch.empty_like(A)
+        pa.apply(A, Ha0); pb.apply(Bm, Hb0); torch.cuda.synchronize()
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        Ha, Hb = torch.empty_like(A), torch.empty_like(A)
+        for _ in range(20):
+            pa.apply(A, Ha, stream=sa); pb.apply(Bm, Hb, stream=sb)
+        torch.cuda.synchronize()
+        assert torch.equal(Ha, Ha0) and torch.equal(Hb, Hb0)
+
+
+def test_create_destroy_returns_all_device_memory(torch, B):
+    torch.cuda.synchronize()
+    with B.Plan((64, 64, 8), (2e-9,) * 3) as p:                          # first plan: one-time context / module allocations
+        p.set_kernel(None)
+    free0, _ = torch.cuda.mem_get_info()
+    for i in range(20):
+        with B.Plan((64, 64, 8), (2e-9,) * 3, 0, i % 2) as p:
+            p.set_kernel(None)
+            assert p.workspace_bytes() > 0
+        sp = B.ShardedPlan((64, 64, 8), (2e-9,) * 3, 0, rank=i % 2, world=2, connect=False)
+        sp.set_kernel(None); sp.close()
+    torch.cuda.synchronize()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 <= (8 << 20), (free0, free1)                    # nothing of 20 plans' ~10 MB each is left behind
