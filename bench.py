@@ -316,6 +316,25 @@ def run_ours(args, cfg, fp64):
     b0.record(); barrier()
     ms_hot = a0.elapsed_time(b0) / args.steps
 
+    # the same back-to-back steps replayed from a CUDA graph (the hot path never allocates or synchronises, so an
+    # integrator can capture it): what the launch overhead costs on small meshes
+    ms_graph = None
+    if not atom:
+        try:
+            gs = torch.cuda.Stream()
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.stream(gs):
+                with torch.cuda.graph(gr, stream=gs):
+                    for _ in range(args.steps):
+                        plan.apply(X, Y, stream=gs)
+            gr.replay(); torch.cuda.synchronize()
+            a1, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a1.record(); gr.replay(); b1.record(); torch.cuda.synchronize()
+            ms_graph = a1.elapsed_time(b1) / args.steps
+            del gr
+        except Exception as ex:                                  # reported, never fatal for the bench line
+            ms_graph = f"failed: {ex}"
+
     # ---- end to end through the public API with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not atom:
@@ -442,6 +461,7 @@ def run_ours(args, cfg, fp64):
                    "kernel_family": "fast (kernels_v2.cuh)" if plan.path() == 1 else "generic (kernels.cuh)"},
         "conv_per_s": world * args.steps / (ms_total * 1e-3),
         "hot_ms_per_step": ms_hot, "hot_value": world * nc / (ms_hot * 1e-3) / 1e9,
+        "graph_hot_ms_per_step": ms_graph,
         "e2e": {"value": world * nc * args.steps / t_e2e / 1e9, "unit": UNIT,
                 "h2d_bytes_per_step": e2e_bytes[0], "d2h_bytes_per_step": e2e_bytes[1]},
         "gpu_launches": launches_per_step * args.steps,
