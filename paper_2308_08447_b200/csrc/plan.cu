@@ -363,6 +363,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         }
         p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
         p->cf.sm_count = p->cd.sm_count = p->sm_count;
+        p->cf.ylong = p->cd.ylong = getenv("DEMAG_NO_YLONG") == nullptr;
         const size_t qsz = 4 * p->esz;                      // one quad
         const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;
         size_t slab_bytes = kSlabBytes;

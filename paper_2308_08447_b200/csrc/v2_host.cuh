@@ -196,6 +196,7 @@ template <typename T> struct Ctx {
     GeoV gx;                    // x stages (several GPUs: ny = the rows this rank owns); = g on one GPU
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
+    bool ylong = true;          // long y lines (Ny >= 4096) through the staged persistent kernel (DEMAG_NO_YLONG, read at plan creation)
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;
     const CQ<T>* twpost;
@@ -273,8 +274,8 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
 template <typename T>
 bool y_fwd(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W1, CQ<T>* W2, cudaError_t* err)
 {
-    if (c.lNy == 12 && !getenv("DEMAG_NO_YLONG")) V2_BODY_YLONG(12)
-    if constexpr (sizeof(T) == 4) { if (c.lNy == 13 && !getenv("DEMAG_NO_YLONG")) V2_BODY_YLONG(13) }
+    if (c.lNy == 12 && c.ylong) V2_BODY_YLONG(12)
+    if constexpr (sizeof(T) == 4) { if (c.lNy == 13 && c.ylong) V2_BODY_YLONG(13) }
     switch (c.lNy) {
         V2_CASE_Y(4, k_y_fwd_v, W1, W2) V2_CASE_Y(5, k_y_fwd_v, W1, W2) V2_CASE_Y(6, k_y_fwd_v, W1, W2) V2_CASE_Y(7, k_y_fwd_v, W1, W2)
         V2_CASE_Y(8, k_y_fwd_v, W1, W2) V2_CASE_Y(9, k_y_fwd_v, W1, W2) V2_CASE_Y(10, k_y_fwd_v, W1, W2) V2_CASE_Y(11, k_y_fwd_v, W1, W2)

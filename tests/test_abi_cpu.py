@@ -56,3 +56,12 @@ def test_product_path_does_not_import_oracle():
                 assert "import oracle" not in txt and "from oracle" not in txt and "demag_oracle" not in txt, f
     otxt = open(os.path.join(ROOT, "oracle", "oracle.py")).read()
     assert "import paper_2308_08447_b200" not in otxt and "from paper_2308_08447_b200" not in otxt
+
+
+def test_launch_path_headers_do_not_read_the_environment():
+    """demag_apply never touches the host environment: the tuning toggles are read in plan.cu at
+    plan creation; the kernel and launcher headers hold no getenv."""
+    csrc = os.path.join(ROOT, "paper_2308_08447_b200", "csrc")
+    for f in os.listdir(csrc):
+        if f.endswith(".cuh"):
+            assert "getenv" not in open(os.path.join(csrc, f)).read(), f

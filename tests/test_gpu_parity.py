@@ -497,6 +497,76 @@ def test_atomistic_small_lattice(torch, B, oracle):
         assert np.abs(Hs.cpu().numpy() - want).max() / Ms <= TOL64
 
 
+# --------------------------------------------------------------------------------- no write outside H, M untouched
+GUARD = 1 << 16          # elements of sentinel on either side of every caller array
+
+
+def _guarded(torch, shape, dt, fill=None):
+    """A caller array cut out of the middle of a larger buffer whose margins hold a sentinel bit pattern."""
+    nel = int(np.prod(shape))
+    pad = (-nel) % 4                                     # keep the next view 16-byte aligned
+    buf = torch.full((GUARD + nel + pad + GUARD,), -7.25e33, device="cuda", dtype=dt)
+    view = buf[GUARD:GUARD + nel].view(*shape)
+    if fill is not None:
+        view.copy_(fill)
+    return buf, view
+
+
+def _margins_intact(torch, buf, nel):
+    s = torch.tensor(-7.25e33, device="cuda", dtype=buf.dtype)
+    return bool((buf[:GUARD] == s).all()) and bool((buf[GUARD + nel:] == s).all())
+
+
+@pytest.mark.parametrize("n", [(64, 64, 8), (16, 32, 16), (32, 16, 1), (256, 32, 1), (4, 128, 8), (24, 10, 6), (1, 1, 64)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_apply_writes_exactly_H_and_leaves_M_untouched(torch, B, oracle, n, prec):
+    """demag_apply / demag_apply_add / demag_energy on caller arrays surrounded by sentinel margins: every element of
+    H is written, nothing outside H is, M keeps its bits (include/demag.h: "does not modify M, overwrites H") --
+    both kernel families, one-cell-thick, embedded and one-cell-wide meshes."""
+    h, Ms = (2e-9, 3e-9, 1e-9), 8e5
+    dt = torch.float32 if prec == 0 else torch.float64
+    M = torch.from_numpy(rand_M(n, Ms, 90 + sum(n))).to(dt)
+    nel = 3 * int(np.prod(n))
+    shape = (3, n[2], n[1], n[0])
+    with B.Plan(n, h, 0, prec) as p:
+        p.set_kernel(None)
+        mb, Md = _guarded(torch, shape, dt, M.cuda())
+        hb, Hd = _guarded(torch, shape, dt)
+        ab, Ha = _guarded(torch, shape, dt, torch.zeros(shape, dtype=dt))
+        E = torch.zeros(1, device="cuda", dtype=torch.float64)
+        p.apply(Md, Hd); p.apply_add(Md, Ha); p.energy(Md, Hd, E)
+        torch.cuda.synchronize()
+        assert _margins_intact(torch, mb, nel) and _margins_intact(torch, hb, nel) and _margins_intact(torch, ab, nel)
+        assert torch.equal(Md.cpu(), M), "M was modified"
+        assert not bool((Hd == torch.tensor(-7.25e33, device="cuda", dtype=dt)).any()), "an element of H was not written"
+        assert bool(torch.isfinite(Hd).all())
+        assert (Ha.double() - Hd.double()).abs().max().item() / Ms <= (4e-7 if prec == 0 else 1e-15)
+        assert E.item() >= 0.0
+
+
+def test_atomistic_and_extrapolate_write_exactly_their_outputs(torch, B):
+    """The spin-field scatter and the sub-step extrapolation on sentinel-guarded arrays."""
+    from paper_2308_08447_b200 import workloads as W
+    L, c, a, mu_s = (32, 16, 8), (4, 2, 2), 0.3e-9, 2.0
+    n = (8, 8, 4); h = (4 * a, 2 * a, 2 * a)
+    S = torch.from_numpy(W.random_spins_numpy(L, 11))
+    shape = (3, L[2], L[1], L[0]); nel = 3 * int(np.prod(L))
+    with B.Plan(n, h, 0, B.DEMAG_FP32) as p:
+        p.set_kernel(None)
+        sb, Sd = _guarded(torch, shape, torch.float32, S.cuda())
+        ob, Hs = _guarded(torch, shape, torch.float32)
+        p.apply_atomistic(Sd, Hs, c, mu_s, a)
+        torch.cuda.synchronize()
+        assert _margins_intact(torch, sb, nel) and _margins_intact(torch, ob, nel)
+        assert torch.equal(Sd.cpu(), S) and bool(torch.isfinite(Hs).all())
+        mshape = (3, n[2], n[1], n[0]); mel = 3 * int(np.prod(n))
+        hist = [torch.randn(mshape, device="cuda") for _ in range(3)]
+        eb, He = _guarded(torch, mshape, torch.float32)
+        p.extrapolate(hist, [0.0, 1.0, 2.0], 2.5, He)
+        torch.cuda.synchronize()
+        assert _margins_intact(torch, eb, mel) and bool(torch.isfinite(He).all())
+
+
 # --------------------------------------------------------------------------------- ABI error paths
 def test_error_paths(torch, B):
     with pytest.raises(B.DemagError) as e:
