@@ -106,6 +106,16 @@ __device__ __forceinline__ CQ<double> ldsq(const CQ<double>* p)
 // ---- asynchronous bulk copy (TMA, 1D) signalled through an mbarrier -------------------------------------------
 // Used by the long-line y kernel (one line pair per block, one block per SM): the next line lands in a staging
 // buffer while the block transforms the current one.
+// Programmatic dependent launch: the five kernels of one demag_apply are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization (v2_host.cuh launch_pdl), so the blocks of kernel k+1 become resident
+// while the last wave of kernel k drains.  Every kernel calls this before its first global access: it waits until the
+// grid before it has completed and its stores are visible, then lets the grid after it be scheduled.  Without the
+// launch attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_enter()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
 {
@@ -366,6 +376,7 @@ template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
                                                CQ<T>* __restrict__ W2, TwSet<T> tw)
 {
+    pdl_enter();
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
     constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0);
@@ -415,6 +426,7 @@ template <typename T, int LNY, int POL, int NT>
 __global__ void __launch_bounds__(NT) k_y_fwd_long_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
                                                     CQ<T>* __restrict__ W2, TwSet<T> tw)
 {
+    pdl_enter();
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
     static_assert(NP >= 2, "long lines have several passes");
@@ -521,6 +533,7 @@ template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
                                                CQ<T>* __restrict__ W1, TwSet<T> tw)
 {
+    pdl_enter();
     y_inv_body<T, LNY, POL, BP, NT, false>(g, q0, nq, W2, W1, nullptr, tw);
 }
 // the same with the crop scattered to the ranks that own the rows (several GPUs)
@@ -528,6 +541,7 @@ template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_inv_sh_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
                                                   const __grid_constant__ ShardMap<T> map, TwSet<T> tw)
 {
+    pdl_enter();
     y_inv_body<T, LNY, POL, BP, NT, true>(g, q0, nq, W2, nullptr, &map, tw);
 }
 
@@ -605,6 +619,7 @@ template <typename T, int LNZ, int LRF, int KT> struct MulPoints<T, LNZ, LRF, KT
 template <typename T, int LNZ, int POL, int TY, int NT, int MINB, bool FILM = false>
 __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K, TwSet<T> tw)
 {
+    pdl_enter();
     constexpr int NZ = 1 << LNZ, B = 3 * TY;
     constexpr Sched SC = make_sched(LNZ, POL);
     constexpr int NP = SC.n, LRF = SC.lr[NP - 1], RF = 1 << LRF;
@@ -659,6 +674,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
 template <typename T, int LNZ>
 __global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K)
 {
+    pdl_enter();
     constexpr int RF = 1 << LNZ;
     const int cols = blockDim.x;
     const int tilesY = g.Ny / cols;
@@ -752,6 +768,7 @@ template <typename T, int LLC, int POL, int RP, int NT>
 __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
+    pdl_enter();
     x_r2c_body<T, LLC, POL, RP, NT, false>(g, M, W1, nullptr, tw, twpost);
 }
 // the same on this rank's rows only (g.ny = rows of this rank), every pair stored at the rank that owns it
@@ -759,6 +776,7 @@ template <typename T, int LLC, int POL, int RP, int NT>
 __global__ void __launch_bounds__(NT) k_x_r2c_sh_v(GeoV g, const T* __restrict__ M, const __grid_constant__ ShardMap<T> map,
                                                   TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
+    pdl_enter();
     x_r2c_body<T, LLC, POL, RP, NT, true>(g, M, nullptr, &map, tw, twpost);
 }
 
@@ -768,6 +786,7 @@ template <typename T, int LLC, int POL, int RP, int NT>
 __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict__ W1, T* __restrict__ H,
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
+    pdl_enter();
     using V = typename vec2<T>::type;
     constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true);
     constexpr Sched SC = make_sched(LLC, POL);

@@ -364,6 +364,12 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
         p->cf.sm_count = p->cd.sm_count = p->sm_count;
         p->cf.ylong = p->cd.ylong = getenv("DEMAG_NO_YLONG") == nullptr;
+        {   // programmatic dependent launch pays where the kernels are short (C2: 93.8 -> 89.6 us) and costs where they
+            // are long (C3: 365 -> 382 us, profiles/r1_07_pdl.md): on up to 2^21 cells
+            bool pdl = (long long)nx * ny * nz <= (1LL << 21);
+            if (const char* e = getenv("DEMAG_PDL")) pdl = atoi(e) != 0;      // A/B timing
+            p->cf.pdl = p->cd.pdl = pdl;
+        }
         const size_t qsz = 4 * p->esz;                      // one quad
         const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;
         size_t slab_bytes = kSlabBytes;

@@ -196,6 +196,7 @@ template <typename T> struct Ctx {
     GeoV gx;                    // x stages (several GPUs: ny = the rows this rank owns); = g on one GPU
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
+    bool pdl = false;           // programmatic dependent launch of the five kernels (short kernels only, plan.cu; DEMAG_PDL)
     bool ylong = true;          // long y lines (Ny >= 4096) through the staged persistent kernel (DEMAG_NO_YLONG, read at plan creation)
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;
@@ -204,12 +205,26 @@ template <typename T> struct Ctx {
     ShardMap<T> m_in, m_out;
 };
 
+// launch with programmatic stream serialization (kernels_v2.cuh pdl_enter): plain pointers / PODs by value
+// (pdl = false: an ordinary, fully serialised launch)
+template <typename... KA, typename... A>
+inline void launch_pdl(bool pdl, void (*kern)(KA...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, A&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kern, KA(args)...);
+}
+
 #define V2_CASE_X(L, KERN, ...)                                                                                     \
     case L: {                                                                                                        \
         using C = XCfg<L>;                                                                                           \
         constexpr int smem = x_tile_quads(L, C::POL, C::RP) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::RP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else KERN<T, L, C::POL, C::RP, C::NT><<<3u * c.gx.nz * (c.gx.ny / (2 * C::RP)), C::NT, smem, st>>>(__VA_ARGS__); \
+        else launch_pdl(c.pdl, KERN<T, L, C::POL, C::RP, C::NT>, 3u * c.gx.nz * (c.gx.ny / (2 * C::RP)), C::NT, smem, st, __VA_ARGS__); \
         return true;                                                                                                 \
     }
 
@@ -259,7 +274,7 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
         using C = YCfg<L>;                                                                                           \
         constexpr int smem = y_tile_quads(L, C::POL, C::BP) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::BP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else KERN<T, L, C::POL, C::BP, C::NT><<<(unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st>>>(c.g, q0, nq, A, B, c.twy); \
+        else launch_pdl(c.pdl, KERN<T, L, C::POL, C::BP, C::NT>, (unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st, c.g, q0, nq, A, B, c.twy); \
         return true;                                                                                                 \
     }
 #define V2_BODY_YLONG(L)                                                                                            \
@@ -268,7 +283,7 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
         constexpr int smem = (y_tile_quads(L, C::POL, 1) + (1 << (L - 1))) * (int)sizeof(CQ<T>);                      \
         if (mode == 0) *err = cudaFuncSetAttribute(k_y_fwd_long_v<T, L, C::POL, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
         else { const long long nl = 3LL * nq * c.g.nz;                                                               \
-               k_y_fwd_long_v<T, L, C::POL, C::NT><<<(unsigned)(nl < c.sm_count ? nl : c.sm_count), C::NT, smem, st>>>(c.g, q0, nq, W1, W2, c.twy); } \
+               launch_pdl(c.pdl, k_y_fwd_long_v<T, L, C::POL, C::NT>, (unsigned)(nl < c.sm_count ? nl : c.sm_count), C::NT, smem, st, c.g, q0, nq, W1, W2, c.twy); } \
         return true;                                                                                                 \
     }
 template <typename T>
@@ -321,16 +336,16 @@ bool y_inv_sh(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const 
         using C = ZCfg<L>;                                                                                           \
         constexpr int smem = z_tile_quads(L, C::POL, C::TY) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB><<<(unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st>>>(c.g, q0, nq, W2, K, c.twz); \
+        else launch_pdl(c.pdl, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, (unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st, c.g, q0, nq, W2, K, c.twz); \
         return true;                                                                                                 \
     }
 template <typename T>
 bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* K, cudaError_t* err)
 {
     switch (c.lNz) {
-    case 0: if (mode) k_z1_v<T, 0><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
-    case 2: if (mode) k_z1_v<T, 2><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
-    case 3: if (mode) k_z1_v<T, 3><<<(unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st>>>(c.g, q0, nq, W2, K); return true;
+    case 0: if (mode) launch_pdl(c.pdl, k_z1_v<T, 0>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K); return true;
+    case 2: if (mode) launch_pdl(c.pdl, k_z1_v<T, 2>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K); return true;
+    case 3: if (mode) launch_pdl(c.pdl, k_z1_v<T, 3>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K); return true;
         V2_CASE_Z(4) V2_CASE_Z(5) V2_CASE_Z(6) V2_CASE_Z(7) V2_CASE_Z(8) V2_CASE_Z(9) V2_CASE_Z(10) V2_CASE_Z(11)
     default: return false;
     }
@@ -341,7 +356,7 @@ bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2
     case L: {                                                                                                        \
         constexpr int smem = z_tile_quads(L, POL_, 1) * (int)sizeof(CQ<T>);                                          \
         if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, POL_, 1, NT_, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else k_z_v<T, L, POL_, 1, NT_, 1, true><<<(unsigned)c.g.hq, NT_, smem, st>>>(c.gfilm, 0, c.g.hq, W1, K, c.twy); \
+        else launch_pdl(c.pdl, k_z_v<T, L, POL_, 1, NT_, 1, true>, (unsigned)c.g.hq, NT_, smem, st, c.gfilm, 0, c.g.hq, W1, K, c.twy); \
         return true;                                                                                                 \
     }
 template <typename T>

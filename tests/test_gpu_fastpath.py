@@ -127,3 +127,37 @@ def test_fast_family_impulse_returns_tensor_column(torch, B, oracle, monkeypatch
         ref = oracle.direct_sum(T, M.astype(np.float64))
         H = _run(torch, B, n, h, T, M, 1, expect_path=1)
         assert np.abs(H - ref).max() <= 1e-13
+
+
+@pytest.mark.parametrize("n", [(64, 64, 8), (256, 32, 1), (2048, 16, 2), (16, 4096, 2), (256, 256, 64)])
+@pytest.mark.parametrize("pdl", ["1", "0"])
+def test_back_to_back_applies_are_ordered(torch, B, n, pdl, monkeypatch):
+    """Plans of up to 2^21 cells launch the kernels of the fast family with programmatic stream serialization (the next
+    kernel's blocks become resident while the last wave of the current one drains; kernels_v2.cuh pdl_enter); DEMAG_PDL
+    forces it on or off for any size (read at plan creation).  Eight applies queued
+    back to back on one plan, alternating between two magnetisations, without a host synchronisation in between,
+    must each equal bit for bit the field of the same magnetisation applied alone (workspaces are reused from apply
+    to apply: any early start would show up as a mixed field)."""
+    from paper_2308_08447_b200 import workloads as W
+    monkeypatch.setenv("DEMAG_PDL", pdl)
+    h, Ms = (2e-9, 2e-9, 1e-9), 8e5
+    Ma = torch.from_numpy(W.random_unit_vectors(n, Ms, 31)).to("cuda", torch.float32)
+    Mb = torch.from_numpy(W.random_unit_vectors(n, Ms, 32)).to("cuda", torch.float32)
+    with B.Plan(n, h, 0, B.DEMAG_FP32) as p:
+        p.set_kernel(None)
+        assert p.path() == 1
+        alone = []
+        for Md in (Ma, Mb):
+            Hd = torch.empty_like(Md)
+            p.apply(Md, Hd); torch.cuda.synchronize()
+            alone.append(Hd.clone())
+        assert not torch.equal(alone[0], alone[1])
+        outs = [torch.full_like(Ma, float("nan")) for _ in range(8)]
+        for i, Hd in enumerate(outs):
+            p.apply(Ma if i % 2 == 0 else Mb, Hd)
+        acc = torch.zeros_like(Ma)
+        p.apply_add(Ma, acc); p.apply_add(Mb, acc)
+        torch.cuda.synchronize()
+        for i, Hd in enumerate(outs):
+            assert torch.equal(Hd, alone[i % 2]), f"apply {i} differs from the same apply run alone"
+        assert (acc.double() - alone[0].double() - alone[1].double()).abs().max().item() / Ms <= 4e-7
