@@ -30,6 +30,7 @@ struct GeoV {
     int hq;              // number of (k, Lc-k) pairs = Lc/2 + 1
     int kpz;             // Nz/2 + 1
     int acc;             // x C2R: 0 = overwrite H, 1 = add into H (demag_apply_add)
+    int trig;            // programmatic dependent launch: 0 = let the next grid in at block start, 1 = at block end
 };
 
 template <typename T> struct TwSet { const CQ<T>* p[6]; };   // per-pass twiddle tables (NULL for stride-1 passes)
@@ -111,10 +112,16 @@ __device__ __forceinline__ CQ<double> ldsq(const CQ<double>* p)
 // while the last wave of kernel k drains.  Every kernel calls this before its first global access: it waits until the
 // grid before it has completed and its stores are visible, then lets the grid after it be scheduled.  Without the
 // launch attribute both instructions are no-ops.
-__device__ __forceinline__ void pdl_enter()
+__device__ __forceinline__ void pdl_enter(const GeoV& g)
 {
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (!g.trig) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+// after the block's last global store (g.trig = 1: only the launch gap is hidden, no block of the next grid is
+// resident while this one still works)
+__device__ __forceinline__ void pdl_leave(const GeoV& g)
+{
+    if (g.trig) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
@@ -376,7 +383,7 @@ template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
                                                CQ<T>* __restrict__ W2, TwSet<T> tw)
 {
-    pdl_enter();
+    pdl_enter(g);
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
     constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0);
@@ -426,7 +433,7 @@ template <typename T, int LNY, int POL, int NT>
 __global__ void __launch_bounds__(NT) k_y_fwd_long_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
                                                     CQ<T>* __restrict__ W2, TwSet<T> tw)
 {
-    pdl_enter();
+    pdl_enter(g);
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
     static_assert(NP >= 2, "long lines have several passes");
@@ -533,16 +540,18 @@ template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
                                                CQ<T>* __restrict__ W1, TwSet<T> tw)
 {
-    pdl_enter();
+    pdl_enter(g);
     y_inv_body<T, LNY, POL, BP, NT, false>(g, q0, nq, W2, W1, nullptr, tw);
+    pdl_leave(g);
 }
 // the same with the crop scattered to the ranks that own the rows (several GPUs)
 template <typename T, int LNY, int POL, int BP, int NT>
 __global__ void __launch_bounds__(NT) k_y_inv_sh_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
                                                   const __grid_constant__ ShardMap<T> map, TwSet<T> tw)
 {
-    pdl_enter();
+    pdl_enter(g);
     y_inv_body<T, LNY, POL, BP, NT, true>(g, q0, nq, W2, nullptr, &map, tw);
+    pdl_leave(g);
 }
 
 // =========================================================================================== K3v: z stage
@@ -619,7 +628,7 @@ template <typename T, int LNZ, int LRF, int KT> struct MulPoints<T, LNZ, LRF, KT
 template <typename T, int LNZ, int POL, int TY, int NT, int MINB, bool FILM = false>
 __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K, TwSet<T> tw)
 {
-    pdl_enter();
+    pdl_enter(g);
     constexpr int NZ = 1 << LNZ, B = 3 * TY;
     constexpr Sched SC = make_sched(LNZ, POL);
     constexpr int NP = SC.n, LRF = SC.lr[NP - 1], RF = 1 << LRF;
@@ -667,6 +676,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     InvPasses<T, LNZ, POL, 1, NP - 1, B, PE, NT>::run(s, tw, tid);
     auto st = [&](int b, int z, CQ<T> v) { const int c = FILM ? (b == 0 ? 0 : 3 - b) : b / TY, ty = FILM ? 0 : b - c * TY; stq(base + c * cstride + (size_t)z * Ny + ty, v); };
     pass_last<T, LNZ, POL, B, PE, NT, true>(s, tw.p[0], tid, st);
+    pdl_leave(g);
 }
 
 // Nz <= 8: the whole z transform of a column is one butterfly per component in registers; no shared memory.
@@ -674,7 +684,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
 template <typename T, int LNZ>
 __global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K)
 {
-    pdl_enter();
+    pdl_enter(g);
     constexpr int RF = 1 << LNZ;
     const int cols = blockDim.x;
     const int tilesY = g.Ny / cols;
@@ -768,16 +778,18 @@ template <typename T, int LLC, int POL, int RP, int NT>
 __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
-    pdl_enter();
+    pdl_enter(g);
     x_r2c_body<T, LLC, POL, RP, NT, false>(g, M, W1, nullptr, tw, twpost);
+    pdl_leave(g);
 }
 // the same on this rank's rows only (g.ny = rows of this rank), every pair stored at the rank that owns it
 template <typename T, int LLC, int POL, int RP, int NT>
 __global__ void __launch_bounds__(NT) k_x_r2c_sh_v(GeoV g, const T* __restrict__ M, const __grid_constant__ ShardMap<T> map,
                                                   TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
-    pdl_enter();
+    pdl_enter(g);
     x_r2c_body<T, LLC, POL, RP, NT, true>(g, M, nullptr, &map, tw, twpost);
+    pdl_leave(g);
 }
 
 // x C2R FFT fused with the crop; writes H:  W1v -> H
@@ -786,7 +798,7 @@ template <typename T, int LLC, int POL, int RP, int NT>
 __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict__ W1, T* __restrict__ H,
                                                TwSet<T> tw, const CQ<T>* __restrict__ twpost)
 {
-    pdl_enter();
+    pdl_enter(g);
     using V = typename vec2<T>::type;
     constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true);
     constexpr Sched SC = make_sched(LLC, POL);
@@ -828,6 +840,7 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
         *d0 = r0; *d1 = r1;
     };
     pass_last<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, st);
+    pdl_leave(g);
 }
 
 }  // namespace v2

@@ -342,7 +342,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
     }
     if (p->v2) {
         v2::GeoV gv;
-        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0;
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0;
         p->cf.gx = gv; p->cd.gx = gv;
         p->ny_loc = ny; p->nq_loc = gv.hq;
         if (sharded) {
@@ -364,11 +364,15 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
         p->cf.sm_count = p->cd.sm_count = p->sm_count;
         p->cf.ylong = p->cd.ylong = getenv("DEMAG_NO_YLONG") == nullptr;
-        {   // programmatic dependent launch pays where the kernels are short (C2: 93.8 -> 89.6 us) and costs where they
-            // are long (C3: 365 -> 382 us, profiles/r1_07_pdl.md): on up to 2^21 cells
-            bool pdl = (long long)nx * ny * nz <= (1LL << 21);
-            if (const char* e = getenv("DEMAG_PDL")) pdl = atoi(e) != 0;      // A/B timing
-            p->cf.pdl = p->cd.pdl = pdl;
+        {   // programmatic dependent launch (profiles/r1_07_pdl.md).  Letting the next grid in at block END hides the
+            // launch gap only (C3 365.6 -> 356.3 us, C2 92.0 -> 89.1 us, C4 unchanged); letting it in at block START
+            // also makes its blocks resident early, which pays on launch-bound tiny meshes (C1 23.6 -> 16.4 us) and
+            // costs on large ones (C3 382 us): mode 1 up to 2^16 cells, mode 2 above
+            int pdl = (long long)nx * ny * nz <= (1LL << 16) ? 1 : 2;
+            if (const char* e = getenv("DEMAG_PDL")) pdl = atoi(e);           // A/B timing: 0 off, 1 next grid let in at block start, 2 at block end
+            p->cf.pdl = p->cd.pdl = pdl != 0;
+            const int trig = pdl == 2 ? 1 : 0;
+            p->cf.g.trig = p->cd.g.trig = p->cf.gx.trig = p->cd.gx.trig = p->cf.gfilm.trig = p->cd.gfilm.trig = trig;
         }
         const size_t qsz = 4 * p->esz;                      // one quad
         const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;

@@ -196,7 +196,7 @@ template <typename T> struct Ctx {
     GeoV gx;                    // x stages (several GPUs: ny = the rows this rank owns); = g on one GPU
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
-    bool pdl = false;           // programmatic dependent launch of the five kernels (short kernels only, plan.cu; DEMAG_PDL)
+    bool pdl = false;           // programmatic dependent launch of the five kernels (plan.cu; DEMAG_PDL; GeoV::trig = where the next grid is let in)
     bool ylong = true;          // long y lines (Ny >= 4096) through the staged persistent kernel (DEMAG_NO_YLONG, read at plan creation)
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;

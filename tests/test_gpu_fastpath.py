@@ -130,11 +130,11 @@ def test_fast_family_impulse_returns_tensor_column(torch, B, oracle, monkeypatch
 
 
 @pytest.mark.parametrize("n", [(64, 64, 8), (256, 32, 1), (2048, 16, 2), (16, 4096, 2), (256, 256, 64)])
-@pytest.mark.parametrize("pdl", ["1", "0"])
+@pytest.mark.parametrize("pdl", ["2", "1", "0"])
 def test_back_to_back_applies_are_ordered(torch, B, n, pdl, monkeypatch):
-    """Plans of up to 2^21 cells launch the kernels of the fast family with programmatic stream serialization (the next
-    kernel's blocks become resident while the last wave of the current one drains; kernels_v2.cuh pdl_enter); DEMAG_PDL
-    forces it on or off for any size (read at plan creation).  Eight applies queued
+    """The kernels of the fast family are launched with programmatic stream serialization (kernels_v2.cuh pdl_enter /
+    pdl_leave): the next grid is let in when every block of the current one has started (mode 1, tiny meshes) or has
+    stored its last result (mode 2); DEMAG_PDL forces a mode, or 0 = off, for any size (read at plan creation).  Eight applies queued
     back to back on one plan, alternating between two magnetisations, without a host synchronisation in between,
     must each equal bit for bit the field of the same magnetisation applied alone (workspaces are reused from apply
     to apply: any early start would show up as a mixed field)."""
