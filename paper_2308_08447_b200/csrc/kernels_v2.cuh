@@ -31,6 +31,7 @@ struct GeoV {
     int kpz;             // Nz/2 + 1
     int acc;             // x C2R: 0 = overwrite H, 1 = add into H (demag_apply_add)
     int trig;            // programmatic dependent launch: 0 = let the next grid in at block start, 1 = at block end
+    int pf;              // L2 prefetch distance in blocks (0 = off): block b requests the input of tile b + pf
 };
 
 template <typename T> struct TwSet { const CQ<T>* p[6]; };   // per-pass twiddle tables (NULL for stride-1 passes)
@@ -104,6 +105,29 @@ __device__ __forceinline__ CQ<double> ldsq(const CQ<double>* p)
     return r;
 }
 
+// two adjacent quads (32 bytes, 32-byte aligned) in one 256-bit access (sm_100: LDG.256 / STG.256).  The x kernels move
+// the two rows of a row pair this way: a warp's access then touches each 32-byte piece once instead of twice (half as
+// many L1 wavefronts where the pieces of different threads lie in different lines: long rows, RP < 4).
+template <bool NA> __device__ __forceinline__ void ldq2(const CQ<float>* p, CQ<float>& a, CQ<float>& b)
+{
+    float v[8];
+    if (NA) asm volatile("ld.global.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                         : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]) : "l"(p));
+    else asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                      : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]) : "l"(p));
+    a.re = make_float2(v[0], v[1]); a.im = make_float2(v[2], v[3]); b.re = make_float2(v[4], v[5]); b.im = make_float2(v[6], v[7]);
+}
+template <bool NA> __device__ __forceinline__ void ldq2(const CQ<double>* p, CQ<double>& a, CQ<double>& b)
+{
+    a = NA ? ldsq(p) : ldgq(p); b = NA ? ldsq(p + 1) : ldgq(p + 1);
+}
+__device__ __forceinline__ void stq2(CQ<float>* p, CQ<float> a, CQ<float> b)
+{
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(a.re.x), "f"(a.re.y), "f"(a.im.x), "f"(a.im.y),
+                 "f"(b.re.x), "f"(b.re.y), "f"(b.im.x), "f"(b.im.y) : "memory");
+}
+__device__ __forceinline__ void stq2(CQ<double>* p, CQ<double> a, CQ<double> b) { stq(p, a); stq(p + 1, b); }
+
 // ---- asynchronous bulk copy (TMA, 1D) signalled through an mbarrier -------------------------------------------
 // Used by the long-line y kernel (one line pair per block, one block per SM): the next line lands in a staging
 // buffer while the block transforms the current one.
@@ -149,6 +173,23 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// ---- L2 prefetch of a FUTURE tile's input --------------------------------------------------------------------
+// The kernels hold 2-5 blocks of 2-8 warps per SM, each alternating between a load phase, shared-memory passes and a
+// store phase: too few loads are in flight to cover the DRAM latency (ncu: "long scoreboard" is the top stall of all
+// five kernels).  Blocks are dispatched in index order, so block b asks the memory system to bring the input of
+// tile b + pf (pf ~ the number of co-resident blocks: the tile that starts when this one ends) into L2 while it
+// works; that tile's loads then see the L2 latency instead of the DRAM latency.  Pure hint: no effect on results.
+__device__ __forceinline__ void pf_l2_bulk(const void* p, uint32_t bytes)      // 16-byte aligned, bytes % 16 == 0
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void pf_l2_line(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// a span of `bytes` bytes: one bulk request, or one plain request if it fits a 128-byte line
+__device__ __forceinline__ void pf_l2_span(const void* p, uint32_t bytes)
+{
+    if (bytes <= 128) pf_l2_line(p); else pf_l2_bulk(p, bytes);
 }
 
 // twiddles of one butterfly: w^(lo m), m = 1..R-1, from the pass table [m-1][lo].
@@ -380,19 +421,23 @@ __device__ __forceinline__ long long w1v_line_offset(const GeoV& g, int l, int q
 // spectrum follows the same order (ypos2freq, v2_host.cuh: y_w2_pos_to_tile_pos).
 // y forward FFT, zero padding synthesised (PAPER.md:309-315 yFFT): W1v -> W2v
 template <typename T, int LNY, int POL, int BP, int NT>
-__global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
+__global__ void __launch_bounds__(NT, (POL == 6 && NT <= 128 ? 3 : 0)) k_y_fwd_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W1,
                                                CQ<T>* __restrict__ W2, TwSet<T> tw)
 {
     pdl_enter(g);
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
-    constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0);
+    constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0, POL == 6);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     __shared__ long long loff[BP];
     const int tid = threadIdx.x;
     const int nlines = 3 * nq * g.nz;
     const int l0 = blockIdx.x * BP;
     if (tid < BP) loff[tid] = (l0 + tid < nlines) ? w1v_line_offset(g, l0 + tid, q0, nq) : -1;
+    if (g.pf && tid < BP) {
+        const long long lp = (long long)(blockIdx.x + g.pf) * BP + tid;
+        if (lp < nlines) pf_l2_bulk(W1 + w1v_line_offset(g, (int)lp, q0, nq), (uint32_t)(g.ny * sizeof(CQ<T>)));
+    }
     __syncthreads();
     auto ld = [&](int b, int p) { const long long o = loff[b]; return o >= 0 ? ldsq(W1 + o + p) : cq_zero<T>(); };
     pass_first<T, LNY, POL, BP, PITCH, NT, false>(s, tw.p[0], tid, ld);
@@ -404,7 +449,7 @@ __global__ void __launch_bounds__(NT) k_y_fwd_v(GeoV g, int q0, int nq, const CQ
         // last pass (stride 1, no twiddles): butterflies fastest, results straight to global
         constexpr int LR = SC.lr[NP - 1], R = 1 << LR, LNB = LNY - LR, NBF = 1 << LNB, TOT = NBF * BP;
         static_assert(SC.ls[NP - 1] == 0 && R >= 8, "last pass: stride 1, radix >= 8");
-#pragma unroll 2
+#pragma unroll(R >= 32 ? 1 : 2)
         for (int t = tid; t < TOT; t += NT) {
             const int i = t & (NBF - 1), b = t >> LNB;
             const CQ<T>* d = s + tile_addr<PITCH>(i << LR, b);
@@ -437,7 +482,7 @@ __global__ void __launch_bounds__(NT) k_y_fwd_long_v(GeoV g, int q0, int nq, con
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
     static_assert(NP >= 2, "long lines have several passes");
-    constexpr int NY = 1 << LNY, PITCH = tile_pe(1, 1), TQ = tile_quads(PITCH, NY, 1);
+    constexpr int NY = 1 << LNY, PITCH = tile_pe(1, 1, POL == 6), TQ = tile_quads(PITCH, NY, 1);
     constexpr uint32_t kBytes = (uint32_t)((NY / 2) * sizeof(CQ<T>));
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     CQ<T>* stage = s + TQ;
@@ -458,7 +503,7 @@ __global__ void __launch_bounds__(NT) k_y_fwd_long_v(GeoV g, int q0, int nq, con
         FwdPasses<T, LNY, POL, 1, NP - 1, 1, PITCH, NT>::run(s, tw, tid);
         constexpr int LR = SC.lr[NP - 1], R = 1 << LR, LNB = LNY - LR, NBF = 1 << LNB;
         CQ<T>* dst = W2 + (size_t)line * NY;
-#pragma unroll 2
+#pragma unroll(R >= 32 ? 1 : 2)
         for (int i = tid; i < NBF; i += NT) {
             const CQ<T>* d = s + tile_addr<PITCH>(i << LR, 0);
             CQ<T> a[R];
@@ -479,7 +524,7 @@ __device__ __forceinline__ void y_inv_body(const GeoV& g, int q0, int nq, const 
 {
     constexpr Sched SC = make_sched(LNY, POL);
     constexpr int NP = SC.n;
-    constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0);
+    constexpr int NY = 1 << LNY, PITCH = tile_pe(BP | 1, NP >= 2 ? 1 : 0, POL == 6);
     CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);
     __shared__ long long loff[BP];
     const int tid = threadIdx.x;
@@ -497,10 +542,14 @@ __device__ __forceinline__ void y_inv_body(const GeoV& g, int q0, int nq, const 
     }
     const CQ<T>* src = W2 + (size_t)l0 * NY;
     const int nvalid = min(BP, nlines - l0);
+    if (g.pf && tid < BP) {
+        const long long lp = (long long)(blockIdx.x + g.pf) * BP + tid;
+        if (lp < nlines) pf_l2_bulk(W2 + (size_t)lp * NY, (uint32_t)(NY * sizeof(CQ<T>)));
+    }
     if constexpr (NP >= 2) {
         // first inverse pass (stride 1, no twiddles): inputs straight from global, butterflies fastest
         constexpr int LR = SC.lr[NP - 1], R = 1 << LR, LNB = LNY - LR, NBF = 1 << LNB, TOT = NBF * BP;
-#pragma unroll 2
+#pragma unroll(R >= 32 ? 1 : 2)
         for (int t = tid; t < TOT; t += NT) {
             const int i = t & (NBF - 1), b = t >> LNB;
             CQ<T> a[R];
@@ -537,7 +586,7 @@ __device__ __forceinline__ void y_inv_body(const GeoV& g, int q0, int nq, const 
     }
 }
 template <typename T, int LNY, int POL, int BP, int NT>
-__global__ void __launch_bounds__(NT) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
+__global__ void __launch_bounds__(NT, (POL == 6 && NT <= 128 ? 3 : 0)) k_y_inv_v(GeoV g, int q0, int nq, const CQ<T>* __restrict__ W2,
                                                CQ<T>* __restrict__ W1, TwSet<T> tw)
 {
     pdl_enter(g);
@@ -642,6 +691,16 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     const size_t cstride = (size_t)nq * g.nz * g.Ny;
     CQ<T>* base = W2 + (size_t)ql * g.nz * g.Ny + py0;
     const int Ny = g.Ny;
+    if (g.pf && blockIdx.x + g.pf < gridDim.x) {
+        const int bn = blockIdx.x + g.pf, pytn = bn % tilesY, qln = bn / tilesY;
+        const CQ<T>* bnx = W2 + (size_t)qln * g.nz * g.Ny + pytn * TY;
+        if (FILM) { if (tid < 3) pf_l2_bulk(bnx + tid * cstride, (uint32_t)(g.nz * sizeof(CQ<T>))); }
+        else for (int r = tid; r < 3 * g.nz; r += NT) { const int c = r / g.nz, z = r - c * g.nz; pf_l2_span(bnx + c * cstride + (size_t)z * Ny, (uint32_t)(TY * sizeof(CQ<T>))); }
+        if (tid == NT - 1) {
+            const uint32_t kb = (uint32_t)(g.kpz * kchunks<T>::N * TY * sizeof(typename kchunks<T>::V));
+            pf_l2_bulk(K + ((size_t)(q0 + qln) * tilesY + pytn) * g.kpz * (kchunks<T>::N * TY), kb);
+        }
+    }
     auto ld = [&](int b, int z) { const int c = FILM ? (b == 0 ? 0 : 3 - b) : b / TY, ty = FILM ? 0 : b - c * TY; return ldsq(base + c * cstride + (size_t)z * Ny + ty); };
     pass_first<T, LNZ, POL, B, PE, NT, true>(s, tw.p[0], tid, ld);
     __syncthreads();
@@ -740,6 +799,8 @@ __device__ __forceinline__ void x_r2c_body(const GeoV& g, const T* __restrict__ 
     const int y0 = ty * 2 * RP;
     const int nx = g.nx;
     const T* rows = M + ((size_t)cz * g.ny + y0) * nx;
+    if (g.pf && tid == 0 && blockIdx.x + g.pf < gridDim.x)
+        pf_l2_bulk(M + (size_t)(blockIdx.x + g.pf) * (2 * RP) * nx, (uint32_t)(2 * RP * nx * sizeof(T)));
     auto ld = [&](int b, int m) {
         const V r0 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b) * nx + 2 * m));
         const V r1 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b + 1) * nx + 2 * m));
@@ -771,7 +832,7 @@ __device__ __forceinline__ void x_r2c_body(const GeoV& g, const T* __restrict__ 
             const int nqs = sr == map->G - 1 ? map->total - k0 : map->per;
             d = map->base[sr] + (((size_t)c * nqs + (k - k0)) * g.nz + z) * map->pitch + map->off + y0 + 2 * b;
         } else d = out + (size_t)k * plane + 2 * b;
-        stq(d, o0); stq(d + 1, o1);
+        stq2(d, o0, o1);
     }
 }
 template <typename T, int LLC, int POL, int RP, int NT>
@@ -810,12 +871,19 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     const int c = cz / g.nz, z = cz - c * g.nz;
     const size_t plane = (size_t)g.nz * g.ny;
     const CQ<T>* in = W1 + ((size_t)c * g.hq * g.nz + z) * g.ny + y0;
+    if (g.pf && blockIdx.x + g.pf < gridDim.x) {
+        const int bn = blockIdx.x + g.pf, tyn = bn % tilesY, czn = bn / tilesY, cn = czn / g.nz, zn = czn - cn * g.nz;
+        const CQ<T>* inn = W1 + ((size_t)cn * g.hq * g.nz + zn) * g.ny + tyn * 2 * RP;
+        for (int k = tid; k <= LC / 2; k += NT) pf_l2_span(inn + (size_t)k * plane, (uint32_t)(2 * RP * sizeof(CQ<T>)));
+    }
     constexpr int TOT = (LC / 2 + 1) * RP;
 #pragma unroll 2
     for (int t = tid; t < TOT; t += NT) {
         const int b = t % RP, k = t / RP;
         const CQ<T>* d = in + (size_t)k * plane + 2 * b;
-        const CQ<T> Q0 = RP >= 4 ? ldsq(d) : ldgq(d), Q1 = RP >= 4 ? ldsq(d + 1) : ldgq(d + 1);
+        CQ<T> Q0, Q1;
+        if (RP >= 8) { Q0 = ldsq(d); Q1 = ldsq(d + 1); }      // 256-byte runs: two 128-bit loads measured faster (C3)
+        else ldq2<(RP >= 4)>(d, Q0, Q1);
         V xkr, xmr, xki, xmi;
         xkr.x = Q0.re.x; xkr.y = Q1.re.x; xmr.x = Q0.re.y; xmr.y = Q1.re.y;
         xki.x = Q0.im.x; xki.y = Q1.im.x; xmi.x = Q0.im.y; xmi.y = Q1.im.y;

@@ -16,6 +16,25 @@
 #include "kernels_z.cuh"
 #include "v2_host.cuh"
 
+// The fast-path launchers are instantiated in their own translation units (v2_inst.cuh: one per stage and precision),
+// so that the library builds in parallel.
+namespace demag {
+namespace v2 {
+#define V2_EXTERN(T)                                                                                                      \
+    extern template bool x_fwd<T>(int, const Ctx<T>&, cudaStream_t, const T*, CQ<T>*, cudaError_t*);                     \
+    extern template bool x_fwd_sh<T>(int, const Ctx<T>&, cudaStream_t, const T*, cudaError_t*);                          \
+    extern template bool x_inv<T>(int, const Ctx<T>&, cudaStream_t, const CQ<T>*, T*, cudaError_t*, int);                \
+    extern template bool y_fwd<T>(int, const Ctx<T>&, cudaStream_t, int, int, const CQ<T>*, CQ<T>*, cudaError_t*);       \
+    extern template bool y_inv<T>(int, const Ctx<T>&, cudaStream_t, int, int, const CQ<T>*, CQ<T>*, cudaError_t*);       \
+    extern template bool y_inv_sh<T>(int, const Ctx<T>&, cudaStream_t, int, int, const CQ<T>*, cudaError_t*);            \
+    extern template bool z_mul<T>(int, const Ctx<T>&, cudaStream_t, int, int, CQ<T>*, const typename kchunks<T>::V*, cudaError_t*); \
+    extern template bool y_film<T>(int, const Ctx<T>&, cudaStream_t, CQ<T>*, const typename kchunks<T>::V*, cudaError_t*);
+V2_EXTERN(float)
+V2_EXTERN(double)
+#undef V2_EXTERN
+}  // namespace v2
+}  // namespace demag
+
 using namespace demag;
 
 namespace {
@@ -342,7 +361,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
     }
     if (p->v2) {
         v2::GeoV gv;
-        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0;
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0;
         p->cf.gx = gv; p->cd.gx = gv;
         p->ny_loc = ny; p->nq_loc = gv.hq;
         if (sharded) {
@@ -364,6 +383,13 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
         p->cf.sm_count = p->cd.sm_count = p->sm_count;
         p->cf.ylong = p->cd.ylong = getenv("DEMAG_NO_YLONG") == nullptr;
+        p->cf.y32 = precision == DEMAG_FP32 && !sharded && getenv("DEMAG_NO_Y32") == nullptr;
+        {   // L2 prefetch of the tile that starts when the current one ends (kernels_v2.cuh pf_l2_*), in waves of
+            // co-resident blocks; 0 = off
+            float w = 0.5f;
+            if (const char* e = getenv("DEMAG_PF")) { w = (float)atof(e); if (!(w >= 0.f && w <= 64.f)) w = 0.f; }
+            p->cf.pf_waves = p->cd.pf_waves = w;
+        }
         {   // programmatic dependent launch (profiles/r1_07_pdl.md).  Letting the next grid in at block END hides the
             // launch gap only (C3 365.6 -> 356.3 us, C2 92.0 -> 89.1 us, C4 unchanged); letting it in at block START
             // also makes its blocks resident early, which pays on launch-bound tiny meshes (C1 23.6 -> 16.4 us) and
@@ -402,7 +428,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         }
         if (p->v2) {
             const int LL[3] = {g.lLc, g.lNy, g.lNz};
-            const int POL[3] = {v2::x_pol(g.lLc), p->cf.film ? v2::film_pol(g.lNy) : v2::y_pol(g.lNy), v2::z_pol(g.lNz)};
+            const int POL[3] = {v2::x_pol(g.lLc), p->cf.film ? v2::film_pol(g.lNy) : v2::y_pol(g.lNy, p->cf.y32), v2::z_pol(g.lNz)};
             cudaError_t verr = cudaSuccess;
             if (precision == DEMAG_FP32) {
                 for (int a = 0; a < 3; ++a) {
@@ -437,10 +463,26 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                     v2::y_inv_sh<double>(0, p->cd, nullptr, 0, 0, nullptr, &verr); CUDA_TRY(verr);
                 }
             }
+            {   // which kernels prefetch (bit 0 x R2C, 1 y forward, 2 z / film, 3 y inverse, 4 x C2R)
+                // Measured (profiles/r2_01_prefetch.md): the y kernels gain 5-19 % (whole lines: one bulk request each), the
+                // z kernel gains 11 % when its rows are >= 512 bytes (C4, 32 columns) and loses with 64-128 byte rows, the
+                // x kernels do not gain (R2C) or lose (C2R: one request per 32-256 byte piece)
+                int mask = 2 | 8 | ((size_t)v2::z_ty(g.lNz) * 4 * p->esz >= 512 && g.lNz >= 4 ? 4 : 0);
+                if (const char* e = getenv("DEMAG_PF_MASK")) mask = atoi(e);
+                auto apply_mask = [&](auto& c) {
+                    if (!(mask & 1)) c.pf_xf = 0;
+                    if (!(mask & 2)) c.pf_yf = 0;
+                    if (!(mask & 4)) { c.pf_z = 0; c.pf_film = 0; }
+                    if (!(mask & 8)) c.pf_yi = 0;
+                    if (!(mask & 16)) c.pf_xi = 0;
+                };
+                apply_mask(p->cf); apply_mask(p->cd);
+            }
             {   // y position -> frequency map of the y schedule, for the plan-time pack
-                const v2::Sched sc = v2::make_sched(g.lNy, v2::y_pol(g.lNy));
+                const int ypol = v2::y_pol(g.lNy, p->cf.y32);
+                const v2::Sched sc = v2::make_sched(g.lNy, ypol);
                 std::vector<int> h((size_t)g.Ny);
-                for (int q = 0; q < g.Ny; ++q) h[q] = v2::sched_freq_of_pos(sc, v2::y_w2_pos_to_tile_pos(g.lNy, v2::y_pol(g.lNy), q));
+                for (int q = 0; q < g.Ny; ++q) h[q] = v2::sched_freq_of_pos(sc, v2::y_w2_pos_to_tile_pos(g.lNy, ypol, q));
                 CUDA_TRY(cudaMalloc(&p->ypos2freq, sizeof(int) * (size_t)g.Ny));
                 CUDA_TRY(cudaMemcpy(p->ypos2freq, h.data(), sizeof(int) * (size_t)g.Ny, cudaMemcpyHostToDevice));
                 p->tw_bytes += sizeof(int) * (size_t)g.Ny;

@@ -11,6 +11,7 @@
 // DFT conventions: forward exp(-2 pi i nk/R), inverse exp(+2 pi i nk/R), unnormalised; natural order in and out.
 #pragma once
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 #if defined(__CUDACC__)
 #define DM_HD __host__ __device__ __forceinline__
@@ -210,9 +211,43 @@ template <bool INV, bool HALF_IN, typename T> DM_HD void dft16(CQ<T>* a)
         for (int k2 = 0; k2 < 4; ++k2) a[k1 + 4 * k2] = t[k2];
     }
 }
+// a * (-i) (forward) / a * (+i) (inverse)
+template <bool INV, typename T> DM_HD CQ<T> crot(CQ<T> a)
+{
+    CQ<T> r;
+    if (!INV) { r.re = a.im; r.im = vneg(a.re); } else { r.re = vneg(a.im); r.im = a.re; }
+    return r;
+}
+// 32 = 2 x 16 (decimation in frequency): e[j] = a[j] + a[j+16], o[j] = (a[j] - a[j+16]) W32^j;
+// X[2k] = DFT16(e)[k], X[2k+1] = DFT16(o)[k].  Used as the stride-1 (twiddle-free) pass of long y lines, where it
+// removes one shared-memory sweep (512 = 16 . 32 instead of 8 . 8 . 8).
+template <bool INV, bool HALF_IN, typename T> DM_HD void dft32(CQ<T>* a)
+{
+    const T c1 = (T)0.98078528040323044913, s1 = (T)0.19509032201612826785;
+    const T c2 = (T)0.92387953251128675613, s2 = (T)0.38268343236508977173;
+    const T c3 = (T)0.83146961230254523708, s3 = (T)0.55557023301960222474;
+    CQ<T> o[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        if (HALF_IN) o[j] = a[j];
+        else { const CQ<T> t = a[j]; a[j] = cadd(t, a[j + 16]); o[j] = csub(t, a[j + 16]); }
+    }
+    o[1] = cmul_const<INV>(o[1], c1, -s1);   o[2] = cmul_const<INV>(o[2], c2, -s2);   o[3] = cmul_const<INV>(o[3], c3, -s3);
+    o[4] = cmul_w8<INV>(o[4]);
+    o[5] = cmul_const<INV>(o[5], s3, -c3);   o[6] = cmul_const<INV>(o[6], s2, -c2);   o[7] = cmul_const<INV>(o[7], s1, -c1);
+    o[8] = crot<INV>(o[8]);
+    o[9] = cmul_const<INV>(o[9], -s1, -c1);  o[10] = cmul_const<INV>(o[10], -s2, -c2); o[11] = cmul_const<INV>(o[11], -s3, -c3);
+    o[12] = cmul_w8_3<INV>(o[12]);
+    o[13] = cmul_const<INV>(o[13], -c3, -s3); o[14] = cmul_const<INV>(o[14], -c2, -s2); o[15] = cmul_const<INV>(o[15], -c1, -s1);
+    dft16<INV, false>(a);          // e, in place in a[0..15]
+    dft16<INV, false>(o);
+#pragma unroll
+    for (int k = 15; k >= 0; --k) { a[2 * k + 1] = o[k]; a[2 * k] = a[k]; }
+}
 template <int LR, bool INV, bool HALF_IN, typename T> DM_HD void dftR(CQ<T>* a)
 {
-    if (LR == 4) dft16<INV, HALF_IN>(a);
+    if (LR == 5) dft32<INV, HALF_IN>(a);
+    else if (LR == 4) dft16<INV, HALF_IN>(a);
     else if (LR == 3) dft8<INV, HALF_IN>(a);
     else if (LR == 2) dft4<INV, HALF_IN>(a);
     else if (LR == 1) dft2<INV, HALF_IN>(a);
@@ -226,6 +261,8 @@ template <int LR, bool INV, bool HALF_IN, typename T> DM_HD void dftR(CQ<T>* a)
 //   POL 2: as many radix-16 as the remainder allows: LL%3==1 -> 16,8,..; LL%3==2 -> 16,16,8,.. (LL >= 8)
 //   POL 3: radix 8 passes, remainder, radix 4 LAST (LL >= 4)
 //   POL 5: radix 16 passes, remainder LAST
+//   POL 6: radix 16 passes, remainder, and a radix-32 LAST pass (LL >= 8; the y stage: the last forward / first
+//          inverse pass runs straight against global memory, so 512 = 16 . 32 sweeps the tile once each way)
 struct Sched {
     int n;          // number of passes
     int lr[6];      // log2 radix of each pass
@@ -241,6 +278,11 @@ DM_HDC Sched make_sched(int LL, int POL)
     } else if (POL == 5) {          // radix 16 passes, remainder LAST (long x rows: fewest sweeps)
         while (rem >= 4) { s.lr[s.n++] = 4; rem -= 4; }
         if (rem) s.lr[s.n++] = rem;
+    } else if (POL == 6) {          // radix 16 passes, remainder, and a radix-32 LAST pass
+        rem -= 5;
+        while (rem >= 4) { s.lr[s.n++] = 4; rem -= 4; }
+        if (rem > 0) s.lr[s.n++] = rem;
+        s.lr[s.n++] = 5;
     } else if (POL == 3) {          // radix 8 passes, remainder, and a radix-4 LAST pass (small fused z stage)
         rem -= 2;
         while (rem >= 3) { s.lr[s.n++] = 3; rem -= 3; }

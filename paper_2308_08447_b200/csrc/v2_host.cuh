@@ -25,6 +25,12 @@ template <> struct YCfg<10> { static constexpr int POL = 1, BP = 4, NT = 256; };
 template <> struct YCfg<11> { static constexpr int POL = 1, BP = 2, NT = 256; };
 template <> struct YCfg<12> { static constexpr int POL = 1, BP = 1, NT = 256; };
 template <> struct YCfg<13> { static constexpr int POL = 1, BP = 1, NT = 512; };
+// fp32 lines whose LAST pass -- the one that runs straight against global memory -- is radix 32 (policy 6): the tile is
+// swept once each way instead of twice (512 = 16 . 32) or twice instead of three times (8192 = 16 . 16 . 32).  The
+// radix-32 butterfly holds 32 quads (128 registers), so blocks are smaller.
+template <int LNY> struct YCfg32 { static constexpr bool has = false; static constexpr int POL = 1, BP = 8, NT = 64; };
+template <> struct YCfg32<9>  { static constexpr bool has = true; static constexpr int POL = 6, BP = 8, NT = 128; };   // 16 . 32
+template <> struct YCfg32<13> { static constexpr bool has = true; static constexpr int POL = 6, BP = 1, NT = 256; };   // 16 . 16 . 32
 // z stage (K3v): radix policy (the LAST pass is the fused one), ky columns per tile, threads, min blocks per SM
 template <int LNZ> struct ZCfg { static constexpr int POL = 1, TY = 16, NT = 64, MINB = 1; };
 template <> struct ZCfg<4>  { static constexpr int POL = 0, TY = 32, NT = 128, MINB = 1; };   // 8 . 2
@@ -39,7 +45,7 @@ template <> struct ZCfg<11> { static constexpr int POL = 1, TY = 1,  NT = 64,  M
 // quads of the y tile (skewed when the schedule has >= 2 passes, kernels_v2.cuh "tile addressing")
 constexpr int y_tile_quads(int LNY, int POL, int BP)
 {
-    return tile_quads(tile_pe(BP | 1, make_sched(LNY, POL).n >= 2 ? 1 : 0), 1 << LNY, BP);
+    return tile_quads(tile_pe(BP | 1, make_sched(LNY, POL).n >= 2 ? 1 : 0, POL == 6), 1 << LNY, BP);
 }
 constexpr int x_tile_quads(int LLC, int POL, int RP) { return tile_quads(tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true), 1 << LLC, RP); }
 constexpr int z_tile_quads(int LNZ, int POL, int TY) { return tile_quads(tile_pe(3 * TY, (TY <= 2 && skew_ok(LNZ, POL)) ? TY : 0), 1 << LNZ, 3 * TY); }
@@ -59,7 +65,8 @@ inline int x_rp(int lLc)
     switch (lLc) { case 10: return XCfg<10>::RP; case 11: return XCfg<11>::RP; case 12: return XCfg<12>::RP; default: return 8; }
 }
 inline int x_pol(int lLc) { return lLc == 8 ? XCfg<8>::POL : lLc == 12 ? XCfg<12>::POL : 1; }
-inline int y_pol(int) { return 1; }
+inline bool y_has32(int lNy) { return lNy == 9 || lNy == 13; }
+inline int y_pol(int lNy, bool y32 = false) { return y32 && y_has32(lNy) ? 6 : 1; }
 inline int z_pol(int lNz) { return lNz == 4 ? ZCfg<4>::POL : 1; }
 inline int z_ty(int lNz)
 {
@@ -197,10 +204,15 @@ template <typename T> struct Ctx {
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
     bool pdl = false;           // programmatic dependent launch of the five kernels (plan.cu; DEMAG_PDL; GeoV::trig = where the next grid is let in)
+    bool y32 = false;           // fp32: y schedule with a radix-32 last pass where one is instantiated (YCfg32; DEMAG_NO_Y32)
     bool ylong = true;          // long y lines (Ny >= 4096) through the staged persistent kernel (DEMAG_NO_YLONG, read at plan creation)
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;
     const CQ<T>* twpost;
+    // L2 prefetch distance (kernels_v2.cuh pf_l2_*): pf_waves x (co-resident blocks of the kernel), per kernel; filled
+    // in at plan time (mode 0 of the launchers) from the occupancy the runtime reports
+    float pf_waves = 0.f;
+    mutable int pf_xf = 0, pf_xi = 0, pf_yf = 0, pf_yi = 0, pf_z = 0, pf_film = 0;
     bool sharded = false;       // several GPUs: x R2C stores through m_in, y inverse through m_out (kernels_v2.cuh ShardMap)
     ShardMap<T> m_in, m_out;
 };
@@ -219,11 +231,23 @@ inline void launch_pdl(bool pdl, void (*kern)(KA...), unsigned grid, unsigned bl
     cudaLaunchKernelEx(&cfg, kern, KA(args)...);
 }
 
+// co-resident blocks of a kernel on the whole device x pf_waves -> prefetch distance in blocks
+template <typename K> inline int pf_distance(float waves, int sm_count, K kern, int nt, int smem)
+{
+    if (waves <= 0.f) return 0;
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nt, (size_t)smem) != cudaSuccess || occ < 1) occ = 1;
+    const float d = waves * (float)occ * (float)sm_count;
+    return d < 1.f ? 1 : (int)d;
+}
+template <typename G> inline G with_pf(G g, int pf) { g.pf = pf; return g; }
+
 #define V2_CASE_X(L, KERN, ...)                                                                                     \
     case L: {                                                                                                        \
         using C = XCfg<L>;                                                                                           \
         constexpr int smem = x_tile_quads(L, C::POL, C::RP) * (int)sizeof(CQ<T>);                                    \
-        if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::RP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+        if (mode == 0) { *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::RP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                         *pfd = pf_distance(c.pf_waves, c.sm_count, KERN<T, L, C::POL, C::RP, C::NT>, C::NT, smem); }  \
         else launch_pdl(c.pdl, KERN<T, L, C::POL, C::RP, C::NT>, 3u * c.gx.nz * (c.gx.ny / (2 * C::RP)), C::NT, smem, st, __VA_ARGS__); \
         return true;                                                                                                 \
     }
@@ -232,12 +256,14 @@ inline void launch_pdl(bool pdl, void (*kern)(KA...), unsigned grid, unsigned bl
 template <typename T>
 bool x_fwd(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cudaError_t* err)
 {
+    int* pfd = &c.pf_xf;
+    const GeoV gp = with_pf(c.gx, c.pf_xf);
     switch (c.lLc) {
-        V2_CASE_X(4, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
-        V2_CASE_X(6, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
-        V2_CASE_X(8, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
-        V2_CASE_X(10, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
-        V2_CASE_X(12, k_x_r2c_v, c.gx, M, W1, c.twx, c.twpost)
+        V2_CASE_X(4, k_x_r2c_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(6, k_x_r2c_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(8, k_x_r2c_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(10, k_x_r2c_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(12, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
     default: return false;
     }
 }
@@ -245,6 +271,7 @@ bool x_fwd(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cu
 template <typename T>
 bool x_fwd_sh(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, cudaError_t* err)
 {
+    int pf_unused = 0; int* pfd = &pf_unused;          // the partitioned variant does not prefetch
     switch (c.lLc) {
         V2_CASE_X(4, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
         V2_CASE_X(6, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
@@ -257,7 +284,8 @@ bool x_fwd_sh(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, cudaError_
 template <typename T>
 bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cudaError_t* err, int acc = 0)
 {
-    GeoV ga = c.gx; ga.acc = acc;
+    int* pfd = &c.pf_xi;
+    GeoV ga = c.gx; ga.acc = acc; ga.pf = c.pf_xi;
     switch (c.lLc) {
         V2_CASE_X(4, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(5, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
         V2_CASE_X(6, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(7, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
@@ -269,17 +297,20 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
 }
 
 #define V2_CASE_Y(L, KERN, A, B) case L: V2_BODY_Y(L, KERN, A, B)
-#define V2_BODY_Y(L, KERN, A, B)                                                                                    \
+#define V2_BODY_Y(L, KERN, A, B) V2_BODY_Y_C(YCfg<L>, L, KERN, A, B)
+#define V2_BODY_Y_C(CFG, L, KERN, A, B)                                                                             \
     {                                                                                                                \
-        using C = YCfg<L>;                                                                                           \
+        using C = CFG;                                                                                               \
         constexpr int smem = y_tile_quads(L, C::POL, C::BP) * (int)sizeof(CQ<T>);                                    \
-        if (mode == 0) *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::BP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else launch_pdl(c.pdl, KERN<T, L, C::POL, C::BP, C::NT>, (unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st, c.g, q0, nq, A, B, c.twy); \
+        if (mode == 0) { *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::BP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                         *pfd = pf_distance(c.pf_waves, c.sm_count, KERN<T, L, C::POL, C::BP, C::NT>, C::NT, smem); }  \
+        else launch_pdl(c.pdl, KERN<T, L, C::POL, C::BP, C::NT>, (unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st, with_pf(c.g, *pfd), q0, nq, A, B, c.twy); \
         return true;                                                                                                 \
     }
-#define V2_BODY_YLONG(L)                                                                                            \
+#define V2_BODY_YLONG(L) V2_BODY_YLONG_C(YCfg<L>, L)
+#define V2_BODY_YLONG_C(CFG, L)                                                                                     \
     {                                                                                                                \
-        using C = YCfg<L>;                                                                                           \
+        using C = CFG;                                                                                               \
         constexpr int smem = (y_tile_quads(L, C::POL, 1) + (1 << (L - 1))) * (int)sizeof(CQ<T>);                      \
         if (mode == 0) *err = cudaFuncSetAttribute(k_y_fwd_long_v<T, L, C::POL, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
         else { const long long nl = 3LL * nq * c.g.nz;                                                               \
@@ -289,6 +320,12 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
 template <typename T>
 bool y_fwd(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W1, CQ<T>* W2, cudaError_t* err)
 {
+    int* pfd = &c.pf_yf;
+    if constexpr (sizeof(T) == 4) {
+        if (c.y32 && c.lNy == 9) V2_BODY_Y_C(YCfg32<9>, 9, k_y_fwd_v, W1, W2)
+        if (c.y32 && c.lNy == 13 && c.ylong) V2_BODY_YLONG_C(YCfg32<13>, 13)
+        if (c.y32 && c.lNy == 13) V2_BODY_Y_C(YCfg32<13>, 13, k_y_fwd_v, W1, W2)
+    }
     if (c.lNy == 12 && c.ylong) V2_BODY_YLONG(12)
     if constexpr (sizeof(T) == 4) { if (c.lNy == 13 && c.ylong) V2_BODY_YLONG(13) }
     switch (c.lNy) {
@@ -302,6 +339,11 @@ bool y_fwd(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<
 template <typename T>
 bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W2, CQ<T>* W1, cudaError_t* err)
 {
+    int* pfd = &c.pf_yi;
+    if constexpr (sizeof(T) == 4) {
+        if (c.y32 && c.lNy == 9) V2_BODY_Y_C(YCfg32<9>, 9, k_y_inv_v, W2, W1)
+        if (c.y32 && c.lNy == 13) V2_BODY_Y_C(YCfg32<13>, 13, k_y_inv_v, W2, W1)
+    }
     switch (c.lNy) {
         V2_CASE_Y(4, k_y_inv_v, W2, W1) V2_CASE_Y(5, k_y_inv_v, W2, W1) V2_CASE_Y(6, k_y_inv_v, W2, W1) V2_CASE_Y(7, k_y_inv_v, W2, W1)
         V2_CASE_Y(8, k_y_inv_v, W2, W1) V2_CASE_Y(9, k_y_inv_v, W2, W1) V2_CASE_Y(10, k_y_inv_v, W2, W1) V2_CASE_Y(11, k_y_inv_v, W2, W1)
@@ -335,8 +377,9 @@ bool y_inv_sh(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const 
     case L: {                                                                                                        \
         using C = ZCfg<L>;                                                                                           \
         constexpr int smem = z_tile_quads(L, C::POL, C::TY) * (int)sizeof(CQ<T>);                                    \
-        if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else launch_pdl(c.pdl, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, (unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st, c.g, q0, nq, W2, K, c.twz); \
+        if (mode == 0) { *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                         c.pf_z = pf_distance(c.pf_waves, c.sm_count, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, C::NT, smem); } \
+        else launch_pdl(c.pdl, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, (unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st, with_pf(c.g, c.pf_z), q0, nq, W2, K, c.twz); \
         return true;                                                                                                 \
     }
 template <typename T>
@@ -355,8 +398,9 @@ bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2
 #define V2_CASE_FILM(L, POL_, NT_)                                                                                  \
     case L: {                                                                                                        \
         constexpr int smem = z_tile_quads(L, POL_, 1) * (int)sizeof(CQ<T>);                                          \
-        if (mode == 0) *err = cudaFuncSetAttribute(k_z_v<T, L, POL_, 1, NT_, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-        else launch_pdl(c.pdl, k_z_v<T, L, POL_, 1, NT_, 1, true>, (unsigned)c.g.hq, NT_, smem, st, c.gfilm, 0, c.g.hq, W1, K, c.twy); \
+        if (mode == 0) { *err = cudaFuncSetAttribute(k_z_v<T, L, POL_, 1, NT_, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                         c.pf_film = pf_distance(c.pf_waves, c.sm_count, k_z_v<T, L, POL_, 1, NT_, 1, true>, NT_, smem); } \
+        else launch_pdl(c.pdl, k_z_v<T, L, POL_, 1, NT_, 1, true>, (unsigned)c.g.hq, NT_, smem, st, with_pf(c.gfilm, c.pf_film), 0, c.g.hq, W1, K, c.twy); \
         return true;                                                                                                 \
     }
 template <typename T>

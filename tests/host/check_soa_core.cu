@@ -1,5 +1,5 @@
 // Host-side check of the arithmetic building blocks of the fast kernel family (soa_core.cuh), compiled by
-// tests/test_host_logic.py with nvcc and run on the CPU: every butterfly (radix 2/4/8/16, forward / inverse, full and
+// tests/test_host_logic.py with nvcc and run on the CPU: every butterfly (radix 2/4/8/16/32, forward / inverse, full and
 // zero-padded "half" input) against the DFT definition X[k] = sum_n x[n] exp(-+ 2 pi i n k / R), on both lines of the
 // quads; every radix schedule is a bijection between positions and frequencies.  Prints "OK" or the first failure.
 #include <cmath>
@@ -12,8 +12,8 @@ using namespace demag::v2;
 template <int LR, bool INV, bool HALF> double butterfly_error()
 {
     const int R = 1 << LR;
-    CQ<double> a[16];
-    std::complex<double> x0[16], x1[16];
+    CQ<double> a[32];
+    std::complex<double> x0[32], x1[32];
     for (int i = 0; i < R; ++i) {
         const bool z = HALF && i >= R / 2;
         x0[i] = z ? 0 : std::complex<double>(sin(i * 1.3 + 0.2), cos(i * 0.7 + 1));
@@ -41,12 +41,13 @@ template <int LR> int check_radix()
     const double e[4] = {butterfly_error<LR, false, false>(), butterfly_error<LR, true, false>(),
                          butterfly_error<LR, false, true>(), butterfly_error<LR, true, true>()};
     for (int i = 0; i < 4; ++i)
-        if (!(e[i] < 1e-13)) { printf("FAIL radix %d variant %d error %g\n", 1 << LR, i, e[i]); return 1; }
+        if (!(e[i] < (LR >= 5 ? 4e-13 : 1e-13))) {     // rounding: the sums reach ~2 R in magnitude
+ printf("FAIL radix %d variant %d error %g\n", 1 << LR, i, e[i]); return 1; }
     return 0;
 }
 int main()
 {
-    int bad = check_radix<1>() + check_radix<2>() + check_radix<3>() + check_radix<4>();
+    int bad = check_radix<1>() + check_radix<2>() + check_radix<3>() + check_radix<4>() + check_radix<5>();
     // twiddle multiplication helpers
     {
         CQ<double> a, w;
@@ -58,8 +59,9 @@ int main()
             std::abs(A0 * std::conj(W) - std::complex<double>(c.re.x, c.im.x)) > 1e-15) { printf("FAIL cmul\n"); ++bad; }
     }
     for (int LL = 1; LL <= 13; ++LL)
-        for (int pol : {0, 1, 2, 3, 5}) {
+        for (int pol : {0, 1, 2, 3, 5, 6}) {
             if (pol == 3 && LL < 4) continue;
+            if (pol == 6 && LL < 8) continue;
             const Sched s = make_sched(LL, pol);
             int tot = 0;
             for (int j = 0; j < s.n; ++j) tot += s.lr[j];
