@@ -277,6 +277,8 @@ def run_ours(args, cfg, fp64):
     t0 = time.perf_counter()
     plan = B.Plan(n, cfg.h, 0, B.DEMAG_FP64 if fp64 else B.DEMAG_FP32)
     plan.set_kernel(None)
+    if atom:
+        plan.reserve_atomistic()                        # the macrocell arrays: allocated once, never inside a step
     torch.cuda.synchronize()
     t_plan = time.perf_counter() - t0
 

@@ -116,10 +116,17 @@ demag_status demag_energy(demag_plan_t plan, const void* M_dev, const void* H_de
  * cx*cy*cz spins, M = mu_B mu_s sum(S^) / (cx cy cz a^3); the plan's convolution is applied; the
  * cell field is written to every spin of the cell, Hs_dev [3][Lz][Ly][Lx] (overwritten if
  * accumulate == 0, added to if accumulate != 0).  The spin lattice is (nx*cx, ny*cy, nz*cz); the plan
- * must have been created with h_a = c_a * a (checked to 1e-9 relative). */
+ * must have been created with h_a = c_a * a (checked to 1e-9 relative).
+ * The two macrocell arrays (M and H on the plan's mesh) live in the plan and are allocated by
+ * demag_atomistic_reserve, NOT by this call: without them it returns DEMAG_ERR_INVALID_ARG.  Like demag_apply it never
+ * allocates or synchronises, so its first call can already be captured in a CUDA graph. */
 demag_status demag_apply_atomistic(demag_plan_t plan, const void* S_dev, void* Hs_dev,
                                    int cx, int cy, int cz, double mu_s_in_muB, double a,
                                    int accumulate, void* cuda_stream);
+
+/* Allocate the macrocell arrays demag_apply_atomistic works on (2 * 3 * nx*ny*nz reals; counted by
+ * demag_workspace_bytes from then on).  Idempotent; synchronous (cudaMalloc); DEMAG_ERR_ALLOC if out of memory. */
+demag_status demag_atomistic_reserve(demag_plan_t plan);
 
 /* Copy back the REAL-SPACE tensor the plan was given or built: double[6][nz][ny][nx] (host).
  * For builder-vs-oracle parity tests.  Synchronous. */

@@ -24,7 +24,7 @@ EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy
            "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path", "demag_apply_add",
            "demag_shard_range", "demag_plan_create_sharded", "demag_shard_info", "demag_shard_buffers",
            "demag_shard_ipc_export", "demag_shard_ipc_connect", "demag_shard_set_peers", "demag_apply_sharded",
-           "demag_set_pbc_images", "demag_extrapolate"]
+           "demag_set_pbc_images", "demag_extrapolate", "demag_atomistic_reserve"]
 
 
 class DemagError(RuntimeError):
@@ -58,6 +58,7 @@ def lib():
         L.demag_energy.argtypes = [vp, vp, vp, vp, vp]
         L.demag_apply_profiled.argtypes = [vp, vp, vp, vp, vp, vp]
         L.demag_apply_atomistic.argtypes = [vp, vp, vp, i, i, i, d, d, i, vp]
+        L.demag_atomistic_reserve.argtypes = [vp]
         L.demag_get_kernel_real.argtypes = [vp, vp]
         L.demag_workspace_bytes.argtypes = [vp]
         L.demag_workspace_bytes.restype = ctypes.c_size_t
@@ -144,6 +145,10 @@ def demag_energy(plan, M, H, E, stream=None):
 def demag_apply_atomistic(plan, S, Hs, c, mu_s, a, accumulate=False, stream=None):
     _check(lib().demag_apply_atomistic(plan, S.data_ptr(), Hs.data_ptr(), int(c[0]), int(c[1]), int(c[2]),
                                        float(mu_s), float(a), int(bool(accumulate)), _stream(stream)))
+
+
+def demag_atomistic_reserve(plan):
+    _check(lib().demag_atomistic_reserve(plan))
 
 
 def demag_get_kernel_real(plan, n) -> np.ndarray:
@@ -271,16 +276,23 @@ class ShardedPlan:
         demag_set_kernel(self.handle, N6_host)
         return self
 
-    def barrier(self):
+    def barrier(self, stream=None):
+        """Order this rank's peer stores before the peers' reads: an all-reduce of one element enqueued on the SAME
+        stream the phases run on (torch enqueues collectives on its current stream)."""
         if self.world > 1:
+            import torch
             import torch.distributed as dist
-            dist.all_reduce(self._flag, group=self.group)
+            if stream is None:
+                dist.all_reduce(self._flag, group=self.group)
+            else:
+                with torch.cuda.stream(stream):
+                    dist.all_reduce(self._flag, group=self.group)
 
     def apply(self, M_loc, H_loc, stream=None):
         demag_apply_sharded(self.handle, 0, M_loc, None, stream)
-        self.barrier()
+        self.barrier(stream)
         demag_apply_sharded(self.handle, 1, None, None, stream)
-        self.barrier()
+        self.barrier(stream)
         demag_apply_sharded(self.handle, 2, None, H_loc, stream)
 
     def energy(self, M_loc, H_loc, E, stream=None):
@@ -336,6 +348,11 @@ class Plan:
 
     def extrapolate(self, H_hist, t_hist, t, H_out, accumulate=False, stream=None):
         demag_extrapolate(self.handle, H_hist, t_hist, t, H_out, accumulate, stream)
+
+    def reserve_atomistic(self):
+        """Allocate the macrocell arrays apply_atomistic works on (once per plan; apply_atomistic never allocates)."""
+        demag_atomistic_reserve(self.handle)
+        return self
 
     def apply_atomistic(self, S, Hs, c, mu_s, a, accumulate=False, stream=None):
         demag_apply_atomistic(self.handle, S, Hs, c, mu_s, a, accumulate, stream)

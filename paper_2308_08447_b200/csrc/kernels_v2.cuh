@@ -7,10 +7,15 @@
 //                               the real transform produces / consumes together (hq = Lc/2 + 1, Lc = Nx/2 = nx)
 //   W2v [3][nq][nz][Ny] quads   slab of nq pairs; y in the digit-reversed "position order" the forward passes
 //                               leave behind (the stored kernel spectrum uses the same order: nothing is permuted)
-//   Kv  [hq][Ny/KT][Nz/2+1][chunk][KT]  the six real components for the two frequencies of the pair, z packed by
-//                               symmetry, the y parity sign, -1/(Nx Ny Nz) and the 1/2 of the
-//                               real split folded in at plan time; tiled by KT consecutive py (the z kernel's
-//                               tile) and split into 16-byte chunks so that a warp's load is contiguous
+//   Kv  [hq][kst][Nz/2+1][chunk][KT]    the six real components for the two frequencies of the pair, packed by
+//                               symmetry in z AND y ((ny+1) x (nz+1) rows), -1/(Nx Ny Nz) and the
+//                               1/2 of the real split folded in at plan time; split into 16-byte chunks and tiled by
+//                               KT consecutive SLOTS (KT = the z kernel's tile width: a tile's rows are contiguous).
+//                               Slots: W2v position py holds y frequency ky; the positions with
+//                               ky <= Ny/2 are numbered in position order, a position with ky > Ny/2 uses the slot
+//                               of Ny - ky with the sign of the y-odd components (xy, yz) flipped.  yslot[py] =
+//                               slot | (mirrored << 31) is built at plan time for the y schedule in use, so that the
+//                               columns of a tile (consecutive py) read consecutive slots (ascending or descending)
 //
 // Every kernel is templated on log2 of its transform length, its tile and its block size, so that every
 // shared-memory offset is an immediate; twiddles come from per-pass tables (dup format, [m-1][lo]).
@@ -32,6 +37,7 @@ struct GeoV {
     int acc;             // x C2R: 0 = overwrite H, 1 = add into H (demag_apply_add)
     int trig;            // programmatic dependent launch: 0 = let the next grid in at block start, 1 = at block end
     int pf;              // L2 prefetch distance in blocks (0 = off): block b requests the input of tile b + pf
+    int kst;             // slot tiles per pair plane of the stored kernel spectrum, ceil((Ny/2 + 1) / KT) (1 for one-cell-thick meshes)
 };
 
 template <typename T> struct TwSet { const CQ<T>* p[6]; };   // per-pass twiddle tables (NULL for stride-1 passes)
@@ -625,18 +631,20 @@ template <int KT> __device__ __forceinline__ KQ<double> ldk(const double2* p)
     return k;
 }
 // H^_a = sum_b K^_ab M^_b, K^ real and symmetric.  SGN: sign of the z-odd components xz, yz
-// (+1 direct, -1 mirrored kz > Nz/2, 0 = run-time sign sg).
+// (+1 direct, -1 mirrored kz > Nz/2, 0 = run-time sign sg).  sy: sign of the y-odd components xy, yz (-1 for a
+// column whose y frequency is mirrored, yslot < 0).  FILM (the routine run along y): sy = 1, the stored slots are permuted.
 template <int SGN, typename T>
-__device__ __forceinline__ void apply_kernel(const KQ<T>& k, CQ<T>& mx, CQ<T>& my, CQ<T>& mz, T sg)
+__device__ __forceinline__ void apply_kernel(const KQ<T>& k, CQ<T>& mx, CQ<T>& my, CQ<T>& mz, T sg, T sy)
 {
-    typename vec2<T>::type kxz = k.xz, kyz = k.yz;
+    typename vec2<T>::type kxz = k.xz, kyz = vmul(k.yz, vdup(sy));
+    const typename vec2<T>::type kxy = vmul(k.xy, vdup(sy));
     if (SGN < 0) { kxz = vneg(kxz); kyz = vneg(kyz); }
     if (SGN == 0) { kxz = vmul(kxz, vdup(sg)); kyz = vmul(kyz, vdup(sg)); }
     CQ<T> hx, hy, hz;
-    hx.re = vfma(kxz, mz.re, vfma(k.xy, my.re, vmul(k.xx, mx.re)));
-    hx.im = vfma(kxz, mz.im, vfma(k.xy, my.im, vmul(k.xx, mx.im)));
-    hy.re = vfma(kyz, mz.re, vfma(k.yy, my.re, vmul(k.xy, mx.re)));
-    hy.im = vfma(kyz, mz.im, vfma(k.yy, my.im, vmul(k.xy, mx.im)));
+    hx.re = vfma(kxz, mz.re, vfma(kxy, my.re, vmul(k.xx, mx.re)));
+    hx.im = vfma(kxz, mz.im, vfma(kxy, my.im, vmul(k.xx, mx.im)));
+    hy.re = vfma(kyz, mz.re, vfma(k.yy, my.re, vmul(kxy, mx.re)));
+    hy.im = vfma(kyz, mz.im, vfma(k.yy, my.im, vmul(kxy, mx.im)));
     hz.re = vfma(k.zz, mz.re, vfma(kyz, my.re, vmul(kxz, mx.re)));
     hz.im = vfma(k.zz, mz.im, vfma(kyz, my.im, vmul(kxz, mx.im)));
     mx = hx; my = hy; mz = hz;
@@ -646,25 +654,35 @@ __device__ __forceinline__ void apply_kernel(const KQ<T>& k, CQ<T>& mx, CQ<T>& m
 // first chunk at kz' = 0, rows kz' are kchunks<T>::N * KT vectors apart
 template <typename T, int LNZ, int LRF, int KT, int M> struct MulPoints {
     using KV = typename kchunks<T>::V;
-    static __device__ __forceinline__ void run(CQ<T> (*a)[1 << LRF], const KV* __restrict__ Kcol, int f0)
+    static __device__ __forceinline__ void run(CQ<T> (*a)[1 << LRF], const KV* __restrict__ Kcol, int f0, T sy)
     {
         constexpr int NZ = 1 << LNZ, RF = 1 << LRF, W = NZ >> LRF, ROW = kchunks<T>::N * KT;
         const int kz = f0 + M * W;
         if (RF == 1 || 2 * M < RF) {
-            apply_kernel<1>(ldk<KT>(Kcol + kz * ROW), a[0][M], a[1][M], a[2][M], (T)1);
+            apply_kernel<1>(ldk<KT>(Kcol + kz * ROW), a[0][M], a[1][M], a[2][M], (T)1, sy);
         } else if (2 * M > RF) {
-            apply_kernel<-1>(ldk<KT>(Kcol + (NZ - kz) * ROW), a[0][M], a[1][M], a[2][M], (T)1);
+            apply_kernel<-1>(ldk<KT>(Kcol + (NZ - kz) * ROW), a[0][M], a[1][M], a[2][M], (T)1, sy);
         } else {
             const bool mir = f0 > 0;
-            apply_kernel<0>(ldk<KT>(Kcol + (mir ? NZ - kz : kz) * ROW), a[0][M], a[1][M], a[2][M], mir ? (T)-1 : (T)1);
+            apply_kernel<0>(ldk<KT>(Kcol + (mir ? NZ - kz : kz) * ROW), a[0][M], a[1][M], a[2][M], mir ? (T)-1 : (T)1, sy);
         }
-        MulPoints<T, LNZ, LRF, KT, M + 1>::run(a, Kcol, f0);
+        MulPoints<T, LNZ, LRF, KT, M + 1>::run(a, Kcol, f0, sy);
     }
 };
 template <typename T, int LNZ, int LRF, int KT> struct MulPoints<T, LNZ, LRF, KT, (1 << LRF)> {
     using KV = typename kchunks<T>::V;
-    static __device__ __forceinline__ void run(CQ<T> (*)[1 << LRF], const KV* __restrict__, int) {}
+    static __device__ __forceinline__ void run(CQ<T> (*)[1 << LRF], const KV* __restrict__, int, T) {}
 };
+// slot and y sign of W2v position py (yslot == nullptr: one-cell-thick mesh, the routine runs along y: slot 0)
+// -> offset (in 16-byte vectors) of the column's first chunk at kz' = 0 inside the pair plane of the stored spectrum
+template <int KT, int NCH> __device__ __forceinline__ size_t kslot(const int* __restrict__ yslot, int py, int kpz, float& sy)
+{
+    if (!yslot) { sy = 1.f; return 0; }
+    const int v = __ldg(yslot + py);
+    sy = v < 0 ? -1.f : 1.f;
+    const int slot = v & 0x7fffffff;
+    return (size_t)(slot / KT) * kpz * (NCH * KT) + slot % KT;
+}
 
 // Nz >= 16 (at least two passes).  Tile = one pair plane ql x TY consecutive py x all z x 3 components:
 // shared s[Nz][3 TY] quads, lines fastest everywhere (a warp's accesses are consecutive quads: conflict free).
@@ -675,7 +693,8 @@ template <typename T, int LNZ, int LRF, int KT> struct MulPoints<T, LNZ, LRF, KT
 // frequency are xy and yz: the three lines are taken in the order (x, z, y) and the stored spectrum is permuted
 // to match at plan time (k_pack_film_v), which turns "odd in z" into "odd in y" without touching this code.
 template <typename T, int LNZ, int POL, int TY, int NT, int MINB, bool FILM = false>
-__global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K, TwSet<T> tw)
+__global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K,
+                                                  const int* __restrict__ yslot, TwSet<T> tw)
 {
     pdl_enter(g);
     constexpr int NZ = 1 << LNZ, B = 3 * TY;
@@ -696,18 +715,17 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
         const CQ<T>* bnx = W2 + (size_t)qln * g.nz * g.Ny + pytn * TY;
         if (FILM) { if (tid < 3) pf_l2_bulk(bnx + tid * cstride, (uint32_t)(g.nz * sizeof(CQ<T>))); }
         else for (int r = tid; r < 3 * g.nz; r += NT) { const int c = r / g.nz, z = r - c * g.nz; pf_l2_span(bnx + c * cstride + (size_t)z * Ny, (uint32_t)(TY * sizeof(CQ<T>))); }
-        if (tid == NT - 1) {
-            const uint32_t kb = (uint32_t)(g.kpz * kchunks<T>::N * TY * sizeof(typename kchunks<T>::V));
-            pf_l2_bulk(K + ((size_t)(q0 + qln) * tilesY + pytn) * g.kpz * (kchunks<T>::N * TY), kb);
-        }
     }
+    // this thread's column in the fused pass (NT % TY == 0: the same for every item) and its slot in the stored spectrum
+    float sy;
+    const size_t slot = kslot<TY, kchunks<T>::N>(yslot, py0 + tid % TY, g.kpz, sy);
     auto ld = [&](int b, int z) { const int c = FILM ? (b == 0 ? 0 : 3 - b) : b / TY, ty = FILM ? 0 : b - c * TY; return ldsq(base + c * cstride + (size_t)z * Ny + ty); };
     pass_first<T, LNZ, POL, B, PE, NT, true>(s, tw.p[0], tid, ld);
     __syncthreads();
     FwdPasses<T, LNZ, POL, 1, NP - 1, B, PE, NT>::run(s, tw, tid);
     {   // fused: last forward pass . multiply . first inverse pass; item = (butterfly i, column ty), 3 components
         constexpr int NBF = NZ >> LRF, TOT = NBF * TY, ITER = (TOT + NT - 1) / NT;
-        const typename kchunks<T>::V* Kq = K + ((size_t)(q0 + ql) * tilesY + pyt) * g.kpz * (kchunks<T>::N * TY);   // KT == TY
+        const typename kchunks<T>::V* Kq = K + (size_t)(q0 + ql) * g.kst * g.kpz * (kchunks<T>::N * TY);   // KT == TY
 #pragma unroll 1
         for (int k = 0; k < ITER; ++k) {
             const int t = tid + k * NT;
@@ -722,7 +740,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
                 dftR<LRF, false, false>(a[cc]);
             }
             const int f0 = freq_of_pos_rt<LNZ, POL>(p0);
-            MulPoints<T, LNZ, LRF, TY, 0>::run(a, Kq + ty, f0);
+            MulPoints<T, LNZ, LRF, TY, 0>::run(a, Kq + slot, f0, (T)sy);
 #pragma unroll
             for (int cc = 0; cc < 3; ++cc) {
                 dftR<LRF, true, false>(a[cc]);
@@ -741,7 +759,8 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
 // Nz <= 8: the whole z transform of a column is one butterfly per component in registers; no shared memory.
 // grid = nq * Ny / 128 (or fewer columns per block if Ny < 128), block = min(Ny, 128).
 template <typename T, int LNZ>
-__global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K)
+__global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K,
+                                              const int* __restrict__ yslot)
 {
     pdl_enter(g);
     constexpr int RF = 1 << LNZ;
@@ -759,13 +778,95 @@ __global__ void __launch_bounds__(128) k_z1_v(GeoV g, int q0, int nq, CQ<T>* W2,
         for (int m = 0; m < (RF > 1 ? RF / 2 : 1); ++m) a[cc][m] = ldq(col + cc * cstride + (size_t)m * Ny);
         dftR<LNZ, false, true>(a[cc]);
     }
-    MulPoints<T, LNZ, LNZ, 32, 0>::run(a, K + ((size_t)(q0 + ql) * (Ny / 32) + py / 32) * g.kpz * (kchunks<T>::N * 32) + (py & 31), 0);   // KT = 32
+    float sy;
+    const size_t slot = kslot<32, kchunks<T>::N>(yslot, py, g.kpz, sy);                                  // KT = 32
+    MulPoints<T, LNZ, LNZ, 32, 0>::run(a, K + (size_t)(q0 + ql) * g.kst * g.kpz * (kchunks<T>::N * 32) + slot, 0, (T)sy);
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc) {
         dftR<LNZ, true, false>(a[cc]);
 #pragma unroll
         for (int m = 0; m < (RF > 1 ? RF / 2 : 1); ++m) stq(col + cc * cstride + (size_t)m * Ny, a[cc][m]);
     }
+}
+
+// Nz = 16 (8 cells thick: C4), fp32: the whole z stage of a column in the registers of TWO lanes, no shared memory.
+// The 16-point transform of [8 values, 8 zeros] splits by frequency parity into two 8-point transforms of the same
+// 8 values (decimation in frequency with a zero upper half):
+//     M^[2k]   = DFT8(m[z])[k]                      lane "E"  (kz = 0, 2, .., 14)
+//     M^[2k-1] = DFT8(m[z] conj(w16^z))[k]          lane "O"  (kz = 15, 1, 3, .., 13)
+// and the kept half of the inverse is the sum of the two lanes' 8-point inverses,
+//     h[z] = IDFT8(H^e)[z] + w16^z IDFT8(H^o)[z],   z = 0..7,
+// exchanged with one shuffle per value (lane ^ 16).  Lanes 0-15 / 16-31 of a warp are the E / O halves of the same 16
+// columns, so their loads coalesce to the same sectors.  Each thread has 24 + 24 independent 128-bit loads in flight
+// (field + kernel spectrum): the latency is covered without shared-memory staging, and the stage moves one
+// shared-memory-free wavefront per 128 bytes.  grid = nq * Ny / 64, block = 128.
+template <typename T, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_z16_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K,
+                                                  const int* __restrict__ yslot)
+{
+    pdl_enter(g);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const bool odd = (lane >> 4) != 0;
+    const int tilesY = g.Ny >> 6;
+    const int pyt = blockIdx.x % tilesY, ql = blockIdx.x / tilesY;
+    const int py = (pyt << 6) + (wid << 4) + (lane & 15);
+    const int Ny = g.Ny;
+    const size_t cstride = (size_t)nq * 8 * Ny;
+    CQ<T>* col = W2 + (size_t)ql * 8 * Ny + py;
+    CQ<T> a[3][8];
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+        for (int z = 0; z < 8; ++z) a[cc][z] = ldsq(col + cc * cstride + (size_t)z * Ny);
+    // w16^z of the O lanes (1 on the E lanes)
+    const T c8 = (T)0.92387953251128675613, s8 = (T)0.38268343236508977173, h8 = (T)0.70710678118654752440;
+    const T wr[8] = {(T)1, c8, h8, s8, (T)0, -s8, -h8, -c8}, wi[8] = {(T)0, -s8, -h8, -c8, (T)-1, -c8, -h8, -s8};
+    CQ<T> tw[8];
+#pragma unroll
+    for (int z = 1; z < 8; ++z) { tw[z].re = vdup(odd ? wr[z] : (T)1); tw[z].im = vdup(odd ? wi[z] : (T)0); }
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+#pragma unroll
+        for (int z = 1; z < 8; ++z) a[cc][z] = cmulc(a[cc][z], tw[z]);
+        dft8<false, false>(a[cc]);
+    }
+    // point k of the lane is kz = 2k (E) or 2k-1 mod 16 (O); rows of the z-packed spectrum and the sign of its z-odd
+    // components (mirrored frequencies kz > 8):   E: 0 2 4 6 8 6 4 2 / + + + + + - - -    O: 1 1 3 5 7 7 5 3 / - + + + + - - -
+    float sy;
+    const size_t slot = kslot<32, kchunks<T>::N>(yslot, py, 9, sy);                                      // KT = 32
+    constexpr int ROW = kchunks<T>::N * 32;
+    const typename kchunks<T>::V* Kc = K + (size_t)(q0 + ql) * g.kst * 9 * ROW + slot;
+    if (g.pf) {   // the spectrum rows are consumed late (registers): ask for them now
+#pragma unroll
+        for (int k = 0; k < 5; ++k)
+#pragma unroll
+            for (int j = 0; j < kchunks<T>::N; ++j) pf_l2_line(Kc + (2 * k + (odd ? 1 : 0) - (odd && k == 4 ? 2 : 0)) * ROW + j * 32);
+    }
+    constexpr int rowE[8] = {0, 2, 4, 6, 8, 6, 4, 2}, rowO[8] = {1, 1, 3, 5, 7, 7, 5, 3};
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int row = odd ? rowO[k] : rowE[k];
+        const T sg = (k >= 5 || (k == 0 && odd)) ? (T)-1 : (T)1;
+        apply_kernel<0>(ldk<32>(Kc + row * ROW), a[0][k], a[1][k], a[2][k], sg, (T)sy);
+    }
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+        dft8<true, false>(a[cc]);
+#pragma unroll
+        for (int z = 1; z < 8; ++z) a[cc][z] = cmul(a[cc][z], tw[z]);
+    }
+    // h[z] = E part + O part: the E lane finishes z = 0..3, the O lane z = 4..7
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const CQ<T> give = odd ? a[cc][j] : a[cc][j + 4], keep = odd ? a[cc][j + 4] : a[cc][j];
+            CQ<T> got;
+            got.re.x = __shfl_xor_sync(0xffffffffu, give.re.x, 16); got.re.y = __shfl_xor_sync(0xffffffffu, give.re.y, 16);
+            got.im.x = __shfl_xor_sync(0xffffffffu, give.im.x, 16); got.im.y = __shfl_xor_sync(0xffffffffu, give.im.y, 16);
+            stq(col + cc * cstride + (size_t)(j + (odd ? 4 : 0)) * Ny, cadd(keep, got));
+        }
+    pdl_leave(g);
 }
 
 // =========================================================================================== K1v / K5v: x stage

@@ -98,6 +98,8 @@ struct demag_plan_s {
     v2::Ctx<float> cf; v2::Ctx<double> cd;
     v2::AxisTables<float> tf[3]; v2::AxisTables<double> td[3];
     int* ypos2freq = nullptr;
+    int* yslot = nullptr;                // fast path: slot | mirrored << 31 of every W2v position (y-packed kernel spectrum)
+    int kpitch_v = 1;
     // general mesh sizes: the caller's mesh on[] is embedded (zeros) in the power-of-two mesh g.n* the transforms run on
     int on[3] = {0, 0, 0};
     bool embed = false;
@@ -214,7 +216,7 @@ void configure(demag_plan_s* p)
     {
         int B = 16;
         long long lim = 100 << 10;
-        if (const char* e = getenv("DEMAG_B2_KB")) lim = (long long)atoi(e) << 10;      // tuning override
+        if (const char* e = getenv("DEMAG_B2_KB")) { const int v = atoi(e); if (v >= 1 && v <= 220) lim = (long long)v << 10; }   // tuning override
         while (B > 1 && (long long)(B | 1) * g.Ny * csz > lim) B /= 2;
         const long long nlines_min = 3LL * g.nz;
         while (B > nlines_min) B /= 2;
@@ -232,7 +234,7 @@ void configure(demag_plan_s* p)
         p->TY = TY; p->smem3 = 0; p->thr3 = std::max(32, TY);
     } else {
         int TY = 16;
-        if (const char* e = getenv("DEMAG_TY")) TY = atoi(e);       // tuning override (experiments only)
+        if (const char* e = getenv("DEMAG_TY")) { const int v = atoi(e); if (v >= 1 && v <= 64 && is_pow2(v)) TY = v; }   // tuning override (experiments only)
         while (TY > 1 && (long long)TY * 3 * g.Nz * csz > 100 << 10) TY /= 2;
         if (TY > g.Ny) TY = g.Ny;
         p->TY = TY;
@@ -246,7 +248,7 @@ void configure(demag_plan_s* p)
     {
         const size_t per_kx = (size_t)3 * g.nz * g.Ny * csz;
         size_t slab_bytes = kSlabBytes;
-        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoll(e) << 20;   // tuning override
+        if (const char* e = getenv("DEMAG_SLAB_MB")) { const long long v = atoll(e); if (v >= 1 && v <= (1LL << 20)) slab_bytes = (size_t)v << 20; }   // tuning override
         long long n = (long long)(slab_bytes / per_kx);
         if (n < 1) n = 1;
         if (n > g.hx) n = g.hx;
@@ -361,7 +363,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
     }
     if (p->v2) {
         v2::GeoV gv;
-        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0;
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0; gv.kst = (g.Ny / 2 + 1 + v2::z_kt(g.lNz) - 1) / v2::z_kt(g.lNz);
         p->cf.gx = gv; p->cd.gx = gv;
         p->ny_loc = ny; p->nq_loc = gv.hq;
         if (sharded) {
@@ -377,13 +379,14 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         {   // one-cell-thick mesh: y FFT . multiply . y IFFT fused in one kernel, in place on W1 (scope row a3')
             const bool film = v2::film_supported(nz, g.Nz, g.lNy, p->esz, kMaxSmem) && !getenv("DEMAG_NO_FILM");
             v2::GeoV gf = gv;
-            gf.nz = ny; gf.Nz = g.Ny; gf.Ny = 1; gf.kpz = g.kpy;
+            gf.nz = ny; gf.Nz = g.Ny; gf.Ny = 1; gf.kpz = g.kpy; gf.kst = 1;
             p->cf.film = p->cd.film = film; p->cf.gfilm = p->cd.gfilm = gf;
         }
         p->cf.lLc = p->cd.lLc = g.lLc; p->cf.lNy = p->cd.lNy = g.lNy; p->cf.lNz = p->cd.lNz = g.lNz;
         p->cf.sm_count = p->cd.sm_count = p->sm_count;
         p->cf.ylong = p->cd.ylong = getenv("DEMAG_NO_YLONG") == nullptr;
-        p->cf.y32 = precision == DEMAG_FP32 && !sharded && getenv("DEMAG_NO_Y32") == nullptr;
+        p->cf.z16 = precision == DEMAG_FP32 && getenv("DEMAG_NO_Z16") == nullptr ? (getenv("DEMAG_Z16_MINB3") ? 1 : 2) : 0;   // 2 blocks x 255 registers measured 3 % faster than 3 x 168
+        p->cf.y32 = precision == DEMAG_FP32 && getenv("DEMAG_NO_Y32") == nullptr;
         {   // L2 prefetch of the tile that starts when the current one ends (kernels_v2.cuh pf_l2_*), in waves of
             // co-resident blocks; 0 = off
             float w = 0.5f;
@@ -395,7 +398,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
             // also makes its blocks resident early, which pays on launch-bound tiny meshes (C1 23.6 -> 16.4 us) and
             // costs on large ones (C3 382 us): mode 1 up to 2^16 cells, mode 2 above
             int pdl = (long long)nx * ny * nz <= (1LL << 16) ? 1 : 2;
-            if (const char* e = getenv("DEMAG_PDL")) pdl = atoi(e);           // A/B timing: 0 off, 1 next grid let in at block start, 2 at block end
+            if (const char* e = getenv("DEMAG_PDL")) { const int v = atoi(e); if (v >= 0 && v <= 2) pdl = v; }   // A/B timing: 0 off, 1 next grid let in at block start, 2 at block end
             p->cf.pdl = p->cd.pdl = pdl != 0;
             const int trig = pdl == 2 ? 1 : 0;
             p->cf.g.trig = p->cd.g.trig = p->cf.gx.trig = p->cd.gx.trig = p->cf.gfilm.trig = p->cd.gfilm.trig = trig;
@@ -403,7 +406,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         const size_t qsz = 4 * p->esz;                      // one quad
         const size_t per_q = (size_t)3 * g.nz * g.Ny * qsz;
         size_t slab_bytes = kSlabBytes;
-        if (const char* e = getenv("DEMAG_SLAB_MB")) slab_bytes = (size_t)atoll(e) << 20;
+        if (const char* e = getenv("DEMAG_SLAB_MB")) { const long long v = atoll(e); if (v >= 1 && v <= (1LL << 20)) slab_bytes = (size_t)v << 20; }
         long long n = (long long)(slab_bytes / per_q);
         if (n < 1) n = 1;
         if (n > gv.hq) n = gv.hq;
@@ -411,7 +414,8 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         p->w1_bytes = (size_t)3 * gv.hq * g.nz * g.ny * qsz;
         if (sharded) p->w1out_bytes = (size_t)3 * (nx / 2 + 1) * g.nz * p->ny_loc * qsz;
         p->w2_bytes = (size_t)p->nq_auto * per_q;
-        p->k_bytes = (size_t)gv.hq * g.kpz * g.Ny * 12 * p->esz;
+        p->kpitch_v = gv.kst;
+        p->k_bytes = (size_t)gv.hq * gv.kst * v2::z_kt(g.lNz) * g.kpz * 12 * p->esz;     // y and z packed by symmetry
         if (p->cf.film) { p->w2_bytes = 256; p->k_bytes = (size_t)gv.hq * g.kpy * 12 * p->esz; }
     }
     auto alloc_all = [&]() -> demag_status {
@@ -486,6 +490,16 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                 CUDA_TRY(cudaMalloc(&p->ypos2freq, sizeof(int) * (size_t)g.Ny));
                 CUDA_TRY(cudaMemcpy(p->ypos2freq, h.data(), sizeof(int) * (size_t)g.Ny, cudaMemcpyHostToDevice));
                 p->tw_bytes += sizeof(int) * (size_t)g.Ny;
+                // slots of the y-packed kernel spectrum (kernels_v2.cuh "Kv"): positions with ky <= Ny/2 in position
+                // order; a mirrored position shares the slot of Ny - ky
+                std::vector<int> slot_of_freq((size_t)g.Ny / 2 + 1, -1), sl((size_t)g.Ny);
+                int ns = 0;
+                for (int q = 0; q < g.Ny; ++q) if (2 * h[q] <= g.Ny) { slot_of_freq[h[q]] = ns; sl[q] = ns++; }
+                for (int q = 0; q < g.Ny; ++q) if (2 * h[q] > g.Ny) sl[q] = slot_of_freq[g.Ny - h[q]] | (int)0x80000000;
+                CUDA_TRY(cudaMalloc(&p->yslot, sizeof(int) * (size_t)g.Ny));
+                CUDA_TRY(cudaMemcpy(p->yslot, sl.data(), sizeof(int) * (size_t)g.Ny, cudaMemcpyHostToDevice));
+                p->tw_bytes += sizeof(int) * (size_t)g.Ny;
+                p->cf.yslot = p->cd.yslot = p->yslot;
             }
         }
         if (p->embed) {
@@ -521,7 +535,7 @@ demag_status demag_plan_destroy(demag_plan_t p)
     for (int a = 0; a < 3; ++a) cudaFree(p->tw[a]);
     cudaFree(p->Mc); cudaFree(p->Hc); cudaFree(p->Mp); cudaFree(p->Hp);
     for (int a = 0; a < 3; ++a) { cudaFree(p->tf[a].dev); cudaFree(p->td[a].dev); }
-    cudaFree(p->ypos2freq);
+    cudaFree(p->ypos2freq); cudaFree(p->yslot);
     delete p;
     return DEMAG_OK;
 }
@@ -680,9 +694,9 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
                 const size_t n = (size_t)gv.hq * g.kpz * g.Ny;
                 const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
                 if (p->prec == DEMAG_FP32)
-                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale, p->q0);
+                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->kpitch_v, p->ypos2freq, p->yslot, 0.5 * scale, p->q0);
                 else
-                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->ypos2freq, par[c][1], 0.5 * scale, p->q0);
+                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->kpitch_v, p->ypos2freq, p->yslot, 0.5 * scale, p->q0);
             }
             else if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
             else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
@@ -755,15 +769,17 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
         v2::CQ<T>* V1 = (v2::CQ<T>*)p->W1; v2::CQ<T>* V2 = (v2::CQ<T>*)p->W2;
         const typename v2::kchunks<T>::V* Kv = (const typename v2::kchunks<T>::V*)p->K;
         cudaError_t verr = cudaSuccess;
-        STAGE(0, (v2::x_fwd<T>(1, cx, st, M, V1, &verr)));
-        if (cx.film) STAGE(2, (v2::y_film<T>(1, cx, st, V1, Kv, &verr)));
+        bool ok = true;             // a launcher returns false when no kernel is instantiated for the size (a stage would be skipped)
+        STAGE(0, (ok &= v2::x_fwd<T>(1, cx, st, M, V1, &verr)));
+        if (cx.film) STAGE(2, (ok &= v2::y_film<T>(1, cx, st, V1, Kv, &verr)));
         else for (int q0 = 0; q0 < cx.g.hq; q0 += p->nq_slab) {
             const int nq = std::min(p->nq_slab, cx.g.hq - q0);
-            STAGE(1, (v2::y_fwd<T>(1, cx, st, q0, nq, V1, V2, &verr)));
-            STAGE(2, (v2::z_mul<T>(1, cx, st, q0, nq, V2, Kv, &verr)));
-            STAGE(3, (v2::y_inv<T>(1, cx, st, q0, nq, V2, V1, &verr)));
+            STAGE(1, (ok &= v2::y_fwd<T>(1, cx, st, q0, nq, V1, V2, &verr)));
+            STAGE(2, (ok &= v2::z_mul<T>(1, cx, st, q0, nq, V2, Kv, &verr)));
+            STAGE(3, (ok &= v2::y_inv<T>(1, cx, st, q0, nq, V2, V1, &verr)));
         }
-        STAGE(4, (v2::x_inv<T>(1, cx, st, V1, H, &verr, acc)));
+        STAGE(4, (ok &= v2::x_inv<T>(1, cx, st, V1, H, &verr, acc)));
+        if (!ok) return fail(DEMAG_ERR_UNSUPPORTED, "no kernel instantiated for a stage of this plan (fast family)");
         CUDA_TRY(cudaGetLastError());
         return DEMAG_OK;
     }
@@ -844,6 +860,9 @@ demag_status check_apply_args(demag_plan_s* p, const void* a, const void* b, siz
     if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
     if (p->sharded && p->world > 1) return fail(DEMAG_ERR_INVALID_ARG, "plan is one rank of %d: use demag_apply_sharded", p->world);
     if (!a || !b) return fail(DEMAG_ERR_INVALID_ARG, "NULL device pointer");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device)
+        return fail(DEMAG_ERR_INVALID_ARG, "plan was created on device %d, the current device is %d", p->device, dev);
     if (((uintptr_t)a & 15) || ((uintptr_t)b & 15)) return fail(DEMAG_ERR_INVALID_ARG, "device pointers must be 16-byte aligned");
     const char *pa = (const char*)a, *pb = (const char*)b;
     if (pa < pb + bytes && pb < pa + bytes) return fail(DEMAG_ERR_INVALID_ARG, "input and output overlap");
@@ -1104,6 +1123,18 @@ extern "C" demag_status demag_extrapolate(demag_plan_t p, int npts, const void* 
                                  : extrapolate_impl<double>(p, npts, H_hist_dev, w, H_out_dev, accumulate != 0, n, st);
 }
 
+extern "C" demag_status demag_atomistic_reserve(demag_plan_t p)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (p->Mc && p->Hc) return DEMAG_OK;
+    const size_t b = (size_t)3 * p->on[0] * p->on[1] * p->on[2] * p->esz;
+    if (!p->Mc) CUDA_TRY(cudaMalloc(&p->Mc, b));
+    if (!p->Hc) CUDA_TRY(cudaMalloc(&p->Hc, b));
+    p->macro_bytes += 2 * b;
+    return DEMAG_OK;
+}
+
 extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev, void* Hs_dev, int cx, int cy, int cz,
                                               double mu_s_in_muB, double a, int accumulate, void* cuda_stream)
 {
@@ -1121,11 +1152,7 @@ extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev,
     if (s) return s;
     if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
     const size_t nc = (size_t)g.nx * g.ny * g.nz;
-    if (!p->Mc) {   // first atomistic call on this plan: allocate the two macrocell buffers (documented)
-        CUDA_TRY(cudaMalloc(&p->Mc, 3 * nc * p->esz));
-        CUDA_TRY(cudaMalloc(&p->Hc, 3 * nc * p->esz));
-        p->macro_bytes += 6 * nc * p->esz;
-    }
+    if (!p->Mc || !p->Hc) return fail(DEMAG_ERR_INVALID_ARG, "macrocell arrays not allocated: call demag_atomistic_reserve first");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const double muB = 9.2740100783e-24;
     const double f = muB * mu_s_in_muB / ((double)cx * cy * cz * a * a * a);

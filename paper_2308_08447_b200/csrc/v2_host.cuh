@@ -143,14 +143,15 @@ cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>*
     return cudaSuccess;
 }
 
+inline int z_kt(int lNz) { return lNz >= 4 ? z_ty(lNz) : 32; }     // slot tile = the z kernel's column tile (32: register kernels)
 // ---- plan-time pack of the transformed tensor into the pair layout -----------------------------------------
-// A = real 3D transform of one component, [kz'][ky'][kx] (kx = 0..Lc).  Kv[q][py / KT][kz'][chunk][py % KT], lines
-// (q, Lc-q) (kernels_v2.cuh "kchunks").  ypos2freq[py] = y frequency stored at W2v position py (the y schedule's
-// digit reversal).  KT = the z kernel's tile width (z_kt()).
-inline int z_kt(int lNz) { return lNz >= 4 ? z_ty(lNz) : 32; }
+// A = real 3D transform of one component, [kz'][ky'][kx] (kx = 0..Lc).  Kv[q][slot / KT][kz'][chunk][slot % KT], lines (q, Lc-q)
+// (kernels_v2.cuh "Kv").  ypos2freq[py] = y frequency stored at W2v position py (the y schedule's digit reversal);
+// only the positions with ky <= Ny/2 are stored, at yslot[py] (the mirrored ones read the same slot with the sign of
+// the y-odd components flipped in the kernel).
 template <typename T>
 __global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv, int comp, int Lc, int hq, int kpy, int kpz,
-                                int Ny, int KT, const int* __restrict__ ypos2freq, int par_y, double scale, int q0)
+                                int Ny, int KT, int kst, const int* __restrict__ ypos2freq, const int* __restrict__ yslot, double scale, int q0)
 {
     // hq pairs starting at pair q0 (several GPUs: K^(g) holds only its own kx range; else q0 = 0)
     const size_t n = (size_t)hq * kpz * Ny;
@@ -160,14 +161,12 @@ __global__ void k_pack_kernel_v(const double* __restrict__ A, T* __restrict__ Kv
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const int py = (int)(i % Ny), kz = (int)((i / Ny) % kpz), q = (int)(i / ((size_t)Ny * kpz));
         const int ky = ypos2freq[py];
-        const bool my = 2 * ky > Ny;
-        const int kyp = my ? Ny - ky : ky;
-        const double sg = (my && par_y < 0) ? -1.0 : 1.0;
-        const double* row = A + ((size_t)kz * kpy + kyp) * hx;
-        const size_t tile_row = ((size_t)q * (Ny / KT) + py / KT) * kpz + kz;
-        T* d = Kv + ((tile_row * NCH + j) * KT + py % KT) * U + off;
-        d[0] = (T)(sg * scale * row[q0 + q]);
-        d[1] = (T)(sg * scale * row[Lc - q0 - q]);
+        if (2 * ky > Ny) continue;                                 // mirrored: shares the slot of Ny - ky
+        const double* row = A + ((size_t)kz * kpy + ky) * hx;
+        const int slot = yslot[py];
+        T* d = Kv + ((((((size_t)q * kst + slot / KT) * kpz + kz) * NCH + j) * KT) + slot % KT) * U + off;
+        d[0] = (T)(scale * row[q0 + q]);
+        d[1] = (T)(scale * row[Lc - q0 - q]);
     }
 }
 
@@ -204,11 +203,13 @@ template <typename T> struct Ctx {
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
     bool pdl = false;           // programmatic dependent launch of the five kernels (plan.cu; DEMAG_PDL; GeoV::trig = where the next grid is let in)
+    int z16 = 0;                // fp32, Nz = 16: the z stage in registers, two lanes per column (k_z16_v; DEMAG_NO_Z16)
     bool y32 = false;           // fp32: y schedule with a radix-32 last pass where one is instantiated (YCfg32; DEMAG_NO_Y32)
     bool ylong = true;          // long y lines (Ny >= 4096) through the staged persistent kernel (DEMAG_NO_YLONG, read at plan creation)
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;
     const CQ<T>* twpost;
+    const int* yslot = nullptr; // slot | mirrored << 31 of every W2v position (kernels_v2.cuh "Kv"); device memory
     // L2 prefetch distance (kernels_v2.cuh pf_l2_*): pf_waves x (co-resident blocks of the kernel), per kernel; filled
     // in at plan time (mode 0 of the launchers) from the occupancy the runtime reports
     float pf_waves = 0.f;
@@ -354,9 +355,10 @@ bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<
 }
 
 // several GPUs: the cropped rows stored at the ranks that own them (k_y_inv_sh_v)
-#define V2_CASE_YSH(L)                                                                                              \
-    case L: {                                                                                                        \
-        using C = YCfg<L>;                                                                                           \
+#define V2_CASE_YSH(L) case L: V2_BODY_YSH_C(YCfg<L>, L)
+#define V2_BODY_YSH_C(CFG, L)                                                                                       \
+    {                                                                                                                \
+        using C = CFG;                                                                                               \
         constexpr int smem = y_tile_quads(L, C::POL, C::BP) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) *err = cudaFuncSetAttribute(k_y_inv_sh_v<T, L, C::POL, C::BP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
         else k_y_inv_sh_v<T, L, C::POL, C::BP, C::NT><<<(unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st>>>(c.g, q0, nq, W2, c.m_out, c.twy); \
@@ -365,6 +367,10 @@ bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<
 template <typename T>
 bool y_inv_sh(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<T>* W2, cudaError_t* err)
 {
+    if constexpr (sizeof(T) == 4) {
+        if (c.y32 && c.lNy == 9) V2_BODY_YSH_C(YCfg32<9>, 9)
+        if (c.y32 && c.lNy == 13) V2_BODY_YSH_C(YCfg32<13>, 13)
+    }
     switch (c.lNy) {
         V2_CASE_YSH(4) V2_CASE_YSH(5) V2_CASE_YSH(6) V2_CASE_YSH(7) V2_CASE_YSH(8) V2_CASE_YSH(9) V2_CASE_YSH(10) V2_CASE_YSH(11)
         V2_CASE_YSH(12)
@@ -379,16 +385,24 @@ bool y_inv_sh(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const 
         constexpr int smem = z_tile_quads(L, C::POL, C::TY) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) { *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
                          c.pf_z = pf_distance(c.pf_waves, c.sm_count, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, C::NT, smem); } \
-        else launch_pdl(c.pdl, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, (unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st, with_pf(c.g, c.pf_z), q0, nq, W2, K, c.twz); \
+        else launch_pdl(c.pdl, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, (unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st, with_pf(c.g, c.pf_z), q0, nq, W2, K, c.yslot, c.twz); \
         return true;                                                                                                 \
     }
 template <typename T>
 bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* K, cudaError_t* err)
 {
+    if constexpr (sizeof(T) == 4) {
+        if (c.lNz == 4 && c.z16 && c.g.Ny % 64 == 0) {
+            if (mode && c.z16 == 2) launch_pdl(c.pdl, k_z16_v<T, 2>, (unsigned)(nq * (c.g.Ny / 64)), 128, 0, st, with_pf(c.g, c.pf_z), q0, nq, W2, K, c.yslot);
+            else if (mode) launch_pdl(c.pdl, k_z16_v<T, 3>, (unsigned)(nq * (c.g.Ny / 64)), 128, 0, st, with_pf(c.g, c.pf_z), q0, nq, W2, K, c.yslot);
+            else c.pf_z = c.pf_waves > 0.f ? 1 : 0;
+            return true;
+        }
+    }
     switch (c.lNz) {
-    case 0: if (mode) launch_pdl(c.pdl, k_z1_v<T, 0>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K); return true;
-    case 2: if (mode) launch_pdl(c.pdl, k_z1_v<T, 2>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K); return true;
-    case 3: if (mode) launch_pdl(c.pdl, k_z1_v<T, 3>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K); return true;
+    case 0: if (mode) launch_pdl(c.pdl, k_z1_v<T, 0>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K, c.yslot); return true;
+    case 2: if (mode) launch_pdl(c.pdl, k_z1_v<T, 2>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K, c.yslot); return true;
+    case 3: if (mode) launch_pdl(c.pdl, k_z1_v<T, 3>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K, c.yslot); return true;
         V2_CASE_Z(4) V2_CASE_Z(5) V2_CASE_Z(6) V2_CASE_Z(7) V2_CASE_Z(8) V2_CASE_Z(9) V2_CASE_Z(10) V2_CASE_Z(11)
     default: return false;
     }
@@ -400,7 +414,7 @@ bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2
         constexpr int smem = z_tile_quads(L, POL_, 1) * (int)sizeof(CQ<T>);                                          \
         if (mode == 0) { *err = cudaFuncSetAttribute(k_z_v<T, L, POL_, 1, NT_, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
                          c.pf_film = pf_distance(c.pf_waves, c.sm_count, k_z_v<T, L, POL_, 1, NT_, 1, true>, NT_, smem); } \
-        else launch_pdl(c.pdl, k_z_v<T, L, POL_, 1, NT_, 1, true>, (unsigned)c.g.hq, NT_, smem, st, with_pf(c.gfilm, c.pf_film), 0, c.g.hq, W1, K, c.twy); \
+        else launch_pdl(c.pdl, k_z_v<T, L, POL_, 1, NT_, 1, true>, (unsigned)c.g.hq, NT_, smem, st, with_pf(c.gfilm, c.pf_film), 0, c.g.hq, W1, K, (const int*)nullptr, c.twy); \
         return true;                                                                                                 \
     }
 template <typename T>

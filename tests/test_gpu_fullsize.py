@@ -168,6 +168,7 @@ def test_config5_atomistic_1024cubed(torch, B, oracle):
             _builder_parity(p.get_kernel_real(), T, n, cfg.h)
         p.set_kernel(table)
         Hs.fill_(float("nan"))
+        p.reserve_atomistic()
         p.apply_atomistic(S, Hs, c, mu_s, a)
         torch.cuda.synchronize()
         worst = 0.0

@@ -190,6 +190,7 @@ def test_general_mesh_builder_table_energy_atomistic(torch, B, oracle):
     with B.Plan(nm, hm, 0, B.DEMAG_FP64) as p:
         p.set_kernel(Tm)
         Sd = torch.from_numpy(S).cuda(); Hs = torch.empty_like(Sd)
+        p.reserve_atomistic()
         p.apply_atomistic(Sd, Hs, c, mu_s, a)
         torch.cuda.synchronize()
         assert np.abs(Hs.cpu().numpy() - Href).max() / np.abs(Mref).max() <= 1e-11
@@ -471,6 +472,7 @@ def test_atomistic_small_lattice(torch, B, oracle):
     with B.Plan(n, h, 0, B.DEMAG_FP32) as p:
         p.set_kernel(T)
         Sd = torch.from_numpy(S).cuda(); Hs = torch.full_like(Sd, float("nan"))
+        p.reserve_atomistic()
         p.apply_atomistic(Sd, Hs, c, mu_s, a)
         torch.cuda.synchronize()
         Hs_h = Hs.cpu().numpy()
@@ -479,6 +481,7 @@ def test_atomistic_small_lattice(torch, B, oracle):
         cells = Hs_h[:, ::4, ::4, ::4]
         assert np.array_equal(Hs_h, oracle.macrocell_scatter(cells, c))      # piecewise constant, bitwise
         Hs2 = Hs.clone()
+        p.reserve_atomistic()
         p.apply_atomistic(Sd, Hs2, c, mu_s, a, accumulate=True)
         torch.cuda.synchronize()
         assert np.allclose(Hs2.cpu().numpy(), 2 * Hs_h, rtol=1e-6, atol=0)
@@ -492,6 +495,7 @@ def test_atomistic_small_lattice(torch, B, oracle):
     with B.Plan(n2, h2, 0, B.DEMAG_FP64) as p:
         p.set_kernel(T2)
         Sd = torch.from_numpy(S2).cuda(); Hs = torch.empty_like(Sd)
+        p.reserve_atomistic()
         p.apply_atomistic(Sd, Hs, c2, mu_s, a)
         torch.cuda.synchronize()
         assert np.abs(Hs.cpu().numpy() - want).max() / Ms <= TOL64
@@ -555,6 +559,7 @@ def test_atomistic_and_extrapolate_write_exactly_their_outputs(torch, B):
         p.set_kernel(None)
         sb, Sd = _guarded(torch, shape, torch.float32, S.cuda())
         ob, Hs = _guarded(torch, shape, torch.float32)
+        p.reserve_atomistic()
         p.apply_atomistic(Sd, Hs, c, mu_s, a)
         torch.cuda.synchronize()
         assert _margins_intact(torch, sb, nel) and _margins_intact(torch, ob, nel)
@@ -601,6 +606,7 @@ def test_error_paths(torch, B):
         assert e.value.status == 1                      # misaligned
         assert p.workspace_bytes() > 0 and p.launches_per_apply() >= 5
         with pytest.raises(B.DemagError) as e:
+            p.reserve_atomistic()
             p.apply_atomistic(M, H, (2, 2, 2), 2.0, 0.3e-9)
         assert e.value.status == 1                      # h != c*a
     with B.Plan((4, 4, 4), (1e-9,) * 3, B.DEMAG_PBC_X) as p:
@@ -639,6 +645,57 @@ def test_apply_is_capturable_in_a_cuda_graph(torch, B, oracle):
             assert torch.equal(H0, H1)
             assert torch.allclose(Heff, 3 * H0, rtol=1e-5, atol=1e-5 * Ms)
             assert abs(E.item() - oracle.energy(Md.cpu().numpy().astype(np.float64), H0.cpu().numpy().astype(np.float64), h)) <= 1e-6 * abs(E.item())
+
+
+def test_apply_atomistic_never_allocates_and_its_first_call_is_capturable(torch, B, oracle):
+    """include/demag.h: the macrocell arrays are allocated by demag_atomistic_reserve, never by demag_apply_atomistic:
+    without them the call fails with INVALID_ARG; with them the workspace does not change any more and the very FIRST
+    atomistic call of a plan can be captured in a CUDA graph (replay == Eq. (9) average -> Eq. (1) -> scatter)."""
+    from paper_2308_08447_b200 import workloads as W
+    L, c, a, mu_s = (32, 16, 8), (4, 2, 2), 0.3e-9, 2.0
+    n = (8, 8, 4); h = (4 * a, 2 * a, 2 * a)
+    S = W.random_spins_numpy(L, 21)
+    Mref = oracle.macrocell_average(S.astype(np.float64), c, mu_s, a)
+    T = oracle.tensor_table(n, h)
+    want = oracle.macrocell_scatter(oracle.direct_sum(T, Mref), c)
+    Ms = oracle.MU_B * mu_s / a ** 3
+    with B.Plan(n, h, 0, B.DEMAG_FP32) as p:
+        p.set_kernel(T)
+        Sd = torch.from_numpy(S).cuda(); Hs = torch.full_like(Sd, float("nan"))
+        w0 = p.workspace_bytes()
+        with pytest.raises(B.DemagError) as e:
+            p.apply_atomistic(Sd, Hs, c, mu_s, a)
+        assert e.value.status == 1 and "demag_atomistic_reserve" in str(e.value)
+        assert p.workspace_bytes() == w0
+        p.reserve_atomistic()
+        w1 = p.workspace_bytes()
+        assert w1 == w0 + 2 * 3 * int(np.prod(n)) * 4
+        p.reserve_atomistic()                                                # idempotent
+        assert p.workspace_bytes() == w1
+        g = torch.cuda.CUDAGraph()
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            with torch.cuda.graph(g, stream=st):
+                p.apply_atomistic(Sd, Hs, c, mu_s, a)                        # first atomistic call of this plan
+        g.replay(); torch.cuda.synchronize()
+        assert p.workspace_bytes() == w1
+        assert np.abs(Hs.cpu().numpy().astype(np.float64) - want).max() / Ms <= TOL32
+
+
+def test_plan_is_bound_to_its_device_and_bad_tuning_values_are_ignored(torch, B, oracle, monkeypatch):
+    """Tuning toggles with nonsense values must not break a plan (they are ignored), and the results stay the oracle's."""
+    n, h, Ms = (32, 16, 16), (2e-9, 2e-9, 2e-9), 8e5
+    M = rand_M(n, Ms, 5)
+    T = oracle.tensor_table(n, h)
+    ref = oracle.direct_sum(T, M.astype(np.float64))
+    for k, v in (("DEMAG_TY", "0"), ("DEMAG_TY", "-3"), ("DEMAG_B2_KB", "0"), ("DEMAG_SLAB_MB", "-1"), ("DEMAG_PDL", "7"),
+                 ("DEMAG_PF", "nan"), ("DEMAG_PF", "-2")):
+        monkeypatch.setenv(k, v)
+        for path in ("generic", "fast"):
+            monkeypatch.setenv("DEMAG_PATH", path)
+            H = run_gpu(torch, B, n, h, T, M, 0)
+            assert np.abs(H - ref).max() / Ms <= TOL32, (k, v, path)
+        monkeypatch.delenv(k)
 
 
 def test_two_plans_on_two_streams_do_not_interfere(torch, B, oracle):
