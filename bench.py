@@ -1,12 +1,15 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the demagnetizing-field convolution (arXiv 2308.08447, Eq. (1)) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3|C2|C4|C5|C1|C3d] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4|C3|C2|C5|C1|C3d] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (demag_apply: x R2C -> y FFT -> z FFT*multiply*z IFFT -> y IFFT ->
-x C2R; for C5 also the macrocell average and scatter) over one seeded synthetic magnetisation of the chosen
-BASELINE.json config.  Prints ONE JSON line (rank 0).  The path does not shard without an exchange step
-(replicas only), so --gpus N runs N independent replicas, one process per GPU.
+x C2R; for C5 also the macrocell average and scatter) over one seeded synthetic magnetisation of a
+BASELINE.json config.  Prints ONE JSON line (rank 0).  The headline workload is C4 (4096x4096x8, the largest
+single-GPU mesh of BASELINE.json; its `metric` names no config); with no --config the line also carries a
+`configs` block with the same fields for C2, C3, C3 fp64 and C5 (short step counts).  The path does not shard
+without an exchange step (replicas only), so --gpus N runs N independent replicas, one
+process per GPU.
 """
 from __future__ import annotations
 
@@ -36,7 +39,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C3", help="C1..C5, suffix d = fp64 (e.g. C3d)")
+    ap.add_argument("--config", default=None, help="C1..C5, suffix d = fp64 (e.g. C3d); default: headline C4 plus a "
+                                                   "`configs` block for C2, C3, C3d, C5")
+    ap.add_argument("--no-configs", action="store_true", help="default run without the `configs` block")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--sharded", action="store_true",
@@ -45,12 +50,23 @@ def parse():
     ap.add_argument("--virtual-ranks", type=int, default=0,
                     help="with --sharded on ONE GPU: emulate G ranks as G plans on this device, phase by phase, and "
                          "report the per-rank device time of each phase (a compute-share model, no NVLink involved)")
-    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-seconds", type=float, default=10.0)
     return ap.parse_args()
+
+
+HEADLINE = "C4"                                   # largest single-GPU mesh of BASELINE.json (its metric names no config)
+OTHER_CONFIGS = ["C2", "C3", "C3d", "C5"]
 
 
 def workload_name(cfg, fp64):
     return f"{cfg.name} ({'fp64' if fp64 else 'fp32'})"
+
+
+def config_of(cfg, fp64):
+    """The `config` object, identical in our arm and the reference arm (same workload, same metric)."""
+    n = cfg.n
+    return {"workload": workload_name(cfg, fp64), "mesh": list(n), "cells": int(np.prod(n)),
+            "padded": [v if v == 1 else 2 * v for v in n]}
 
 
 # ----------------------------------------------------------------------------------------------- oracle legs
@@ -99,8 +115,8 @@ def run_reference(args, cfg, fp64):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(cfg, fp64), "cells": int(np.prod(cfg.n)),
-                       "sample": f"{per_step} seeded output cells per step, direct O(N) sum each"},
+            "config": config_of(cfg, fp64),
+            "detail": {"sample": f"{per_step} seeded output cells per step, direct O(N) sum each"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": f"{per_step} sample cells x {int(np.prod(cfg.n))} pairs per step"},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -196,7 +212,7 @@ def cufft_baseline(torch, n, dt, dev, reps=10):
     Nx, Ny, Nz = P
     hx = Nx // 2 + 1
     cdt = torch.complex64 if dt == torch.float32 else torch.complex128
-    need = (3 * Nz * Ny * hx * (8 if dt == torch.float32 else 16)) * 3 + 6 * Nz * Ny * hx * (4 if dt == torch.float32 else 8)
+    need = (3 * Nz * Ny * hx * (8 if dt == torch.float32 else 16)) * 4 + 6 * Nz * Ny * hx * (4 if dt == torch.float32 else 8)
     free, _ = torch.cuda.mem_get_info()
     if need > 0.6 * free:
         return None
@@ -223,8 +239,14 @@ def cufft_baseline(torch, n, dt, dev, reps=10):
         Hh = torch.fft.ifft(Hh, dim=-2)[:, :, :ny] if Ny > 1 else Hh
         return torch.fft.irfft(Hh, n=Nx, dim=-1)[..., :nx] if Nx > 1 else Hh.real
 
+    Mpad = torch.zeros((3, Nz, Ny, Nx), dtype=dt, device=dev)
+    Mpad[:, :nz, :ny, :nx] = M
+
+    def fft_only():                                   # floor of any cuFFT-based convolution: no multiply, no pad, no crop
+        return torch.fft.irfftn(torch.fft.rfftn(Mpad, dim=(-3, -2, -1)), s=(Nz, Ny, Nx), dim=(-3, -2, -1))
+
     out = {}
-    for name, fn in (("naive", naive), ("pruned", pruned)):
+    for name, fn in (("naive", naive), ("pruned", pruned), ("fft_only", fft_only)):
         try:
             for _ in range(3):
                 fn()
@@ -241,20 +263,22 @@ def cufft_baseline(torch, n, dt, dev, reps=10):
     return out
 
 
-def run_ours(args, cfg, fp64):
-    import torch
-    import torch.distributed as dist
-    from paper_2308_08447_b200 import binding as B
-    B.lib()                                             # fail loudly if the CUDA extension is missing
-    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    dev = torch.device("cuda", local)
+def source_sha16():
+    """Hash of the CUDA sources the library was built from: ties profiles/traffic.json.txt (ncu DRAM counters) to a build."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2308_08447_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def measure(name, steps, warmup, cpu_seconds, with_cufft, with_cpu, env):
+    """One workload, timed as the bench contract says.  Returns the JSON line as a dict on rank 0, None elsewhere."""
+    torch, dist, B, rank, world, local, dev = env
+    fp64 = name.endswith("d")
+    cfg = W.CONFIGS[name[:2]]
     dt = torch.float64 if fp64 else torch.float32
     esz = 8 if fp64 else 4
     n = cfg.n
@@ -296,13 +320,13 @@ def run_ours(args, cfg, fp64):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(3, args.warmup)):
+    for _ in range(max(3, warmup)):
         flush.fill_(1); step()
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     # ---- timed region: exactly K steps, device time by CUDA events on the launching stream, L2 flushed
     #      between steps (the flush is outside each step's event pair)
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     barrier()
     for a, b in evs:
         flush.fill_(1)
@@ -313,10 +337,10 @@ def run_ours(args, cfg, fp64):
     # hot (no flush, back to back) for context
     a0, b0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     b0.record(); barrier()
-    ms_hot = a0.elapsed_time(b0) / args.steps
+    ms_hot = a0.elapsed_time(b0) / steps
 
     # the same back-to-back steps replayed from a CUDA graph (the hot path never allocates or synchronises, so an
     # integrator can capture it): what the launch overhead costs on small meshes
@@ -327,12 +351,12 @@ def run_ours(args, cfg, fp64):
             gr = torch.cuda.CUDAGraph()
             with torch.cuda.stream(gs):
                 with torch.cuda.graph(gr, stream=gs):
-                    for _ in range(args.steps):
+                    for _ in range(steps):
                         plan.apply(X, Y, stream=gs)
             gr.replay(); torch.cuda.synchronize()
             a1, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a1.record(); gr.replay(); b1.record(); torch.cuda.synchronize()
-            ms_graph = a1.elapsed_time(b1) / args.steps
+            ms_graph = a1.elapsed_time(b1) / steps
             del gr
         except Exception as ex:                                  # reported, never fatal for the bench line
             ms_graph = f"failed: {ex}"
@@ -371,7 +395,7 @@ def run_ours(args, cfg, fp64):
             e2e_step()
         barrier()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(steps):
             e2e_step()
         torch.cuda.synchronize()
         t_e2e = time.perf_counter() - t0
@@ -389,7 +413,7 @@ def run_ours(args, cfg, fp64):
             e2e_step()
         barrier()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(steps):
             e2e_step()
         torch.cuda.synchronize()
         t_e2e = time.perf_counter() - t0
@@ -431,15 +455,15 @@ def run_ours(args, cfg, fp64):
         del hist, heff
 
     cufft = None
-    if rank == 0 and not atom and not args.no_cufft:
+    if rank == 0 and not atom and with_cufft:
         cufft = cufft_baseline(torch, n, dt, dev)
 
     # ---- reduce over ranks: max time
     ms_total, ms_hot, t_e2e = allreduce_max([ms_total, ms_hot, t_e2e], dev, world)
+    del flush
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        plan.close()
+        return None
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -451,22 +475,22 @@ def run_ours(args, cfg, fp64):
     names = STAGE_NAMES_FAST if plan.path() == 1 else STAGE_NAMES
     dom = int(np.argmax(st_ms))
     achieved = sb[dom] / (st_ms[dom] * 1e-3) / 1e9
-    value = aggregate_throughput(world, nc, args.steps, ms_total) / 1e9
+    value = aggregate_throughput(world, nc, steps, ms_total) / 1e9
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": max(3, warmup),
+        "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if fp64 else "f32", "data": "synthetic",
-        "config": {"workload": workload_name(cfg, fp64), "mesh": list(n), "cells": nc, "padded": [v if v == 1 else 2 * v for v in n],
-                   "l2": "flushed between timed steps (256 MB write outside each step's event pair)",
+        "config": config_of(cfg, fp64),
+        "detail": {"l2": "flushed between timed steps (256 MB write outside each step's event pair)",
                    "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                    "kernel": "built-in Newell tensor (demag_set_kernel(NULL))",
                    "kernel_family": "fast (kernels_v2.cuh)" if plan.path() == 1 else "generic (kernels.cuh)"},
-        "conv_per_s": world * args.steps / (ms_total * 1e-3),
+        "conv_per_s": world * steps / (ms_total * 1e-3),
         "hot_ms_per_step": ms_hot, "hot_value": world * nc / (ms_hot * 1e-3) / 1e9,
         "graph_hot_ms_per_step": ms_graph,
-        "e2e": {"value": world * nc * args.steps / t_e2e / 1e9, "unit": UNIT,
+        "e2e": {"value": world * nc * steps / t_e2e / 1e9, "unit": UNIT,
                 "h2d_bytes_per_step": e2e_bytes[0], "d2h_bytes_per_step": e2e_bytes[1]},
-        "gpu_launches": launches_per_step * args.steps,
+        "gpu_launches": launches_per_step * steps,
         "launches_per_step": launches_per_step,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -475,31 +499,83 @@ def run_ours(args, cfg, fp64):
                      "launches_per_apply": int(st_n[dom] // reps)},
         "stages": {names[i]: {"ms": float(st_ms[i]), "model_bytes": sb[i],
                                     "model_GBps": sb[i] / max(st_ms[i], 1e-9) / 1e6} for i in range(5)},
-        "whole_apply_model": {"T2_5pass_bytes": sum(sb), "T2_GBps": sum(sb) / (ms_total / args.steps) / 1e6,
-                              "frac_of_peak": sum(sb) / (ms_total / args.steps) / 1e6 / peak},
+        "whole_apply_model": {"T2_5pass_bytes": sum(sb), "T2_GBps": sum(sb) / (ms_total / steps) / 1e6,
+                              "frac_of_peak": sum(sb) / (ms_total / steps) / 1e6 / peak},
         "plan_build_s": t_plan, "input_gen_s": t_inputs, "workspace_bytes": plan.workspace_bytes(),
     }
     if extrap:
         extrap["frac_of_peak"] = extrap["GBps"] / peak
         line["extrapolate"] = extrap
     if cufft:
-        best = min(v for v in cufft.values() if v)
-        cufft.update(best_ms=best, ours_over_cufft=best / (ms_total / args.steps),
-                     note="torch.fft (cuFFT) convolution of the same shape on the same GPU, L2 not flushed, timing only")
+        best = min(v for k, v in cufft.items() if v and k in ("naive_ms", "pruned_ms"))
+        per = ms_total / steps
+        cufft.update(best_ms=best, ours_over_cufft=best / per,
+                     note="torch.fft (cuFFT) convolution of the same shape on the same GPU, L2 not flushed, timing only; "
+                          "naive / pruned include an eager-PyTorch multiply, padding and crops; fft_only_ms is the floor of "
+                          "any cuFFT-based convolution: one rfftn and one irfftn of the already padded array, nothing else")
+        if cufft.get("fft_only_ms"):
+            cufft["ours_over_cufft_fft_only"] = cufft["fft_only_ms"] / per
         line["cufft"] = cufft
     if atom:
-        line["spins_per_s_G"] = world * units * args.steps / (ms_total * 1e-3) / 1e9
+        line["spins_per_s_G"] = world * units * steps / (ms_total * 1e-3) / 1e9
+    # ncu DRAM counters of this config (profiles/traffic.json.txt: dram__bytes_read.sum + dram__bytes_write.sum per launch,
+    # one --set full capture per config), used only if they were captured on THIS build of the kernels
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json.txt")
     try:
-        tr = json.load(open(traffic_file)).get(args.config, {}).get(names[dom])
-        if tr:
-            line["roofline"]["traffic"] = tr
+        tj = json.load(open(traffic_file))
+        ent = tj.get(name, {})
+        if tj.get("_src_sha16") != source_sha16():
+            line["roofline"]["traffic_note"] = "profiles/traffic.json.txt was captured on another build of the kernels: not used"
+        elif ent:
+            line["roofline"]["traffic"] = ent.get(names[dom])
+            tot = sum(v for k, v in ent.items() if not k.startswith("_"))
+            per = ms_total / steps
+            gbps = tot / per / 1e6
+            line["hbm_counter"] = {"dram_bytes_per_apply": tot, "GBps": gbps, "frac_of_measured_peak": gbps / peak,
+                                   "frac_of_8TBps_nominal": gbps / 8000.0,
+                                   "source": "ncu dram__bytes_read.sum + dram__bytes_write.sum, all kernels of one apply "
+                                             "(profiles/traffic.json.txt), divided by this run's ms_per_step"}
     except Exception:
         pass
-    if world == 1 and not args.no_cpu_baseline:
-        val, cores, desc, _, _ = oracle_sample_rate(cfg, args.cpu_seconds, M_host)
+    plan.close()
+    del X, Y, Mc, Hc
+    torch.cuda.empty_cache()
+    if world == 1 and with_cpu:
+        val, cores, desc, _, _ = oracle_sample_rate(cfg, cpu_seconds, M_host)
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
-    print(json.dumps(line), flush=True)
+    return line
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2308_08447_b200 import binding as B
+    B.lib()                                             # fail loudly if the CUDA extension is missing
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    env = (torch, dist, B, rank, world, local, torch.device("cuda", local))
+    head = args.config or HEADLINE
+    line = measure(head, args.steps, args.warmup, args.cpu_seconds, not args.no_cufft, not args.no_cpu_baseline, env)
+    if rank == 0 and world == 1 and args.config is None and not args.no_configs:
+        # the other configs BASELINE.json names, same fields, short step counts (the headline keeps --steps / --warmup)
+        line["configs"] = {}
+        for name in OTHER_CONFIGS:
+            try:
+                sub = measure(name, min(args.steps, 10), 3, min(args.cpu_seconds, 4.0), not args.no_cufft,
+                              not args.no_cpu_baseline, env)
+                for k in ("stages", "extrapolate", "plan_build_s", "input_gen_s", "detail"):
+                    sub.pop(k, None)
+                line["configs"][name] = sub
+            except Exception as ex:                     # a failing side config must not lose the headline
+                line["configs"][name] = {"error": f"{type(ex).__name__}: {ex}"}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
@@ -646,7 +722,7 @@ def run_sharded(args, cfg, fp64):
 
 def main():
     args = parse()
-    name = args.config
+    name = args.config or HEADLINE
     fp64 = name.endswith("d")
     cfg = W.CONFIGS[name[:2]]
     if args.impl == "reference":
@@ -656,7 +732,7 @@ def main():
     elif args.sharded:
         run_sharded(args, cfg, fp64)
     else:
-        run_ours(args, cfg, fp64)
+        run_ours(args)
 
 
 if __name__ == "__main__":

@@ -19,6 +19,10 @@ Citations are ``PAPER.md:<line>`` (arXiv 2308.08447) or a DESIGN.md reading (R<n
     dipole_field_eq8    Eq. (8) written out, O(n^2)                [NumPy]
     poly_extrapolate    polynomial through previously computed fields, evaluated at a sub-step time (R19)  [NumPy]
     periodic_tensor_table  image-summed, symmetrised tensor on periodic axes (R11)   [NumPy loops over N_at]
+    llg_rhs             Eq. (5) solved for dM/dt (R20)                          [NumPy]
+    llg_rk4_run         classical RK4 on Eq. (5) with H_eff = H_d + H_Zee, H_d by fft_conv at every stage, or by the
+                        quartic extrapolation of PAPER.md:96 at the sub-steps (R21, R22)       [NumPy]
+    fig2_error          mean relative error of the average magnetisation        [NumPy]
 
 All of them are pinned in tests/test_oracle_pins.py; none is "parity unpinned".
 """
@@ -339,3 +343,76 @@ def poly_extrapolate(H_hist, t_hist, t) -> np.ndarray:
                 Lk *= (float(t) - tj) / (ts[k] - tj)
         out += Lk * np.asarray(Hk, dtype=np.float64)
     return out
+
+
+# ------------------------------------------------------------------------------------------------ LLG (NEXT row 4)
+GAMMA_LLG = 2.212761569e5      # mu0 |gamma_e| in m / (A s): the gyromagnetic ratio of Eq. (5) when H is in A/m (R20)
+
+
+def llg_rhs(M, H, Ms, alpha, gamma=GAMMA_LLG) -> np.ndarray:
+    """Eq. (5):  dm/dt = -gamma m x H_eff + alpha m x dm/dt,  m = M / Ms, solved for the derivative
+    (cross the equation with m, use |m| = 1):
+
+        dM/dt = -gamma / (1 + alpha^2) * [ M x H + (alpha / Ms) M x (M x H) ].
+
+    M, H: [3][...] in A/m; returns dM/dt in A/(m s).  (R20: the paper prints only the implicit form.)"""
+    M = np.asarray(M, dtype=np.float64)
+    H = np.asarray(H, dtype=np.float64)
+    MxH = np.cross(M, H, axis=0)
+    MxMxH = np.cross(M, MxH, axis=0)
+    return (-gamma / (1.0 + alpha * alpha)) * (MxH + (alpha / Ms) * MxMxH)
+
+
+def llg_rk4_run(T, M0, Ms, Hzee, alpha, dt, nsteps, gamma=GAMMA_LLG, extrapolate=False, demag=None):
+    """Classical 4th-order Runge-Kutta on Eq. (5) ("typically evaluated using a higher order explicit
+    evaluation method, e.g. RK4") with H_eff = H_d + H_Zee (the other interactions are out of scope),
+    H_d = -N * M (Eq. (1)) through `demag` (default: fft_conv with the table T), H_Zee a uniform field (3-vector, A/m).
+
+    Stages of one step from (t, M):  K1 = f(M),  K2 = f(M + dt/2 K1),  K3 = f(M + dt/2 K2),  K4 = f(M + dt K3),
+    M(t + dt) = M + dt/6 (K1 + 2 K2 + 2 K3 + K4); no renormalisation of |M| (R21: none is stated).
+
+    extrapolate = False: H_d is convolved at every stage (4 per step).
+    extrapolate = True (R22): H_d is convolved only at the START of a step (stage 1, time t_n); the five
+    most recent such fields are kept, and once five exist the fields of stages 2-4 (times t_n + dt/2, t_n + dt/2,
+    t_n + dt) are the quartic polynomial through them (poly_extrapolate) evaluated at the stage time.
+
+    Returns (M_final, Mavg [nsteps+1][3] mesh-averaged magnetisation at t_0..t_nsteps, n_convolutions)."""
+    M = np.array(M0, dtype=np.float64)
+    Hz = np.asarray(Hzee, dtype=np.float64).reshape(3, 1, 1, 1)
+    conv = demag if demag is not None else (lambda X: fft_conv(T, X))
+    nconv = 0
+    hist, thist = [], []
+    avg = [M.reshape(3, -1).mean(axis=1)]
+    t = 0.0
+    for _ in range(int(nsteps)):
+        Hd1 = conv(M); nconv += 1
+        hist.append(Hd1); thist.append(t)
+        if len(hist) > 5:
+            hist.pop(0); thist.pop(0)
+        use = extrapolate and len(hist) == 5
+
+        def field(X, ts):
+            nonlocal nconv
+            if use:
+                return poly_extrapolate(hist, thist, ts)
+            nconv += 1
+            return conv(X)
+        K1 = llg_rhs(M, Hd1 + Hz, Ms, alpha, gamma)
+        X = M + 0.5 * dt * K1
+        K2 = llg_rhs(X, field(X, t + 0.5 * dt) + Hz, Ms, alpha, gamma)
+        X = M + 0.5 * dt * K2
+        K3 = llg_rhs(X, field(X, t + 0.5 * dt) + Hz, Ms, alpha, gamma)
+        X = M + dt * K3
+        K4 = llg_rhs(X, field(X, t + dt) + Hz, Ms, alpha, gamma)
+        M = M + (dt / 6.0) * (K1 + 2.0 * K2 + 2.0 * K3 + K4)
+        t += dt
+        avg.append(M.reshape(3, -1).mean(axis=1))
+    return M, np.array(avg), nconv
+
+
+def fig2_error(Mavg, Mavg_ref, Ms) -> float:
+    """PAPER.md:47:  eps = sum_i || M(t_i) - M~(t_i) || / (n Ms)  over the n recorded points of the average
+    magnetisation, M~ the reference dataset."""
+    A = np.asarray(Mavg, dtype=np.float64); R = np.asarray(Mavg_ref, dtype=np.float64)
+    assert A.shape == R.shape and A.shape[1] == 3
+    return float(np.sqrt(((A - R) ** 2).sum(axis=1)).sum() / (A.shape[0] * Ms))

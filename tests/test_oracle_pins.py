@@ -393,3 +393,99 @@ def test_poly_extrapolate_reproduces_polynomials(oracle):
         assert np.abs(oracle.poly_extrapolate(H, ts, 1.3) - ref).max() <= 1e-7 * np.abs(ref).max()
     one = oracle.poly_extrapolate([np.full((2, 2), 3.0)], [0.1], 9.0)                          # degree 0: constant
     assert np.array_equal(one, np.full((2, 2), 3.0))
+
+
+# ------------------------------------------------------------------------------------ LLG (NEXT row 4)
+def _macrospin(oracle, m0, H, alpha, dt, n, Ms=8e5):
+    """One cell, no demagnetizing field: Eq. (5) in a static uniform field has a closed-form solution."""
+    M0 = (Ms * np.asarray(m0, dtype=np.float64)).reshape(3, 1, 1, 1)
+    Mf, avg, _ = oracle.llg_rk4_run(None, M0, Ms, H, alpha, dt, n, demag=lambda X: np.zeros_like(X))
+    return Mf.ravel() / Ms, avg / Ms
+
+
+def test_llg_macrospin_matches_the_closed_form(oracle):
+    """Eq. (5) with H = H z^: m_z(t) = tanh(alpha g H t + atanh m_z(0)), azimuth phi(t) = phi(0) + g H t,
+    g = gamma / (1 + alpha^2) (textbook solution of the LLG equation for a macrospin).  Catches a wrong sign of the
+    precession or damping term, a missing 1/(1 + alpha^2), a wrong RK4 weight."""
+    alpha, H = 0.1, 1.0e5
+    g = oracle.GAMMA_LLG / (1.0 + alpha * alpha)
+    th0, ph0 = 0.7, 0.3
+    m0 = [np.sin(th0) * np.cos(ph0), np.sin(th0) * np.sin(ph0), np.cos(th0)]
+    dt, n = 1.0e-13, 500
+    m, avg = _macrospin(oracle, m0, (0.0, 0.0, H), alpha, dt, n)
+    for i in (1, 100, n):
+        t = i * dt
+        mz = np.tanh(alpha * g * H * t + np.arctanh(np.cos(th0)))
+        ph = ph0 + g * H * t
+        want = np.array([np.sqrt(1 - mz * mz) * np.cos(ph), np.sqrt(1 - mz * mz) * np.sin(ph), mz])
+        assert np.abs(avg[i] - want).max() < 1e-9, (i, avg[i], want)
+    assert abs(np.linalg.norm(m) - 1.0) < 1e-12
+
+
+def test_llg_rhs_is_orthogonal_to_m_and_vanishes_at_equilibrium(oracle):
+    rng = np.random.default_rng(3)
+    M = rng.standard_normal((3, 4, 5, 6)); H = 1e5 * rng.standard_normal((3, 4, 5, 6))
+    Ms = 8e5
+    M *= Ms / np.sqrt((M * M).sum(axis=0, keepdims=True))
+    K = oracle.llg_rhs(M, H, Ms, 0.3)
+    assert np.abs((K * M).sum(axis=0)).max() <= 1e-12 * np.abs(K).max() * Ms          # |M| is conserved by the flow
+    assert np.abs(oracle.llg_rhs(M, 2.5 * M, Ms, 0.3)).max() <= 1e-9 * oracle.GAMMA_LLG * Ms * Ms * 1e-6   # M || H: no torque
+    # alpha = 0: pure precession, dM/dt = -gamma M x H exactly
+    assert np.allclose(oracle.llg_rhs(M, H, Ms, 0.0), -oracle.GAMMA_LLG * np.cross(M, H, axis=0), rtol=1e-14, atol=0)
+
+
+def test_llg_rk4_is_fourth_order_and_conserves_energy_without_damping(oracle):
+    alpha, H = 0.05, 2.0e5
+    g = oracle.GAMMA_LLG / (1.0 + alpha * alpha)
+    th0 = 1.1
+    m0 = [np.sin(th0), 0.0, np.cos(th0)]
+    T = 2.0e-11
+    errs = []
+    for n in (50, 100, 200):
+        m, _ = _macrospin(oracle, m0, (0.0, 0.0, H), alpha, T / n, n)
+        mz = np.tanh(alpha * g * H * T + np.arctanh(np.cos(th0)))
+        ph = g * H * T
+        want = np.array([np.sqrt(1 - mz * mz) * np.cos(ph), np.sqrt(1 - mz * mz) * np.sin(ph), mz])
+        errs.append(np.abs(m - want).max())
+    assert 12.0 < errs[0] / errs[1] < 20.0 and 12.0 < errs[1] / errs[2] < 20.0, errs      # error ~ dt^4
+    m, avg = _macrospin(oracle, m0, (0.0, 0.0, H), 0.0, 1e-13, 300)
+    assert np.abs(avg[:, 2] - np.cos(th0)).max() < 1e-10                                   # m . H conserved when alpha = 0
+
+
+def test_llg_with_demag_dissipates_energy_and_extrapolation_tracks_the_full_run(oracle):
+    """Small film with the demagnetizing field: (i) E_d + E_Zee never increases for alpha > 0 (the LLG flow is a
+    gradient-like flow of the energy: dE/dt = -alpha mu0 g/Ms |M x H|^2 V <= 0); (ii) |M| stays Ms; (iii) the run that
+    replaces the sub-step convolutions by the quartic through the five last full-step fields stays within
+    1e-6 of the run that convolves at every stage, with 16 + (n - 4) convolutions instead of 4 n."""
+    n, h, Ms = (16, 8, 2), (5e-9, 5e-9, 5e-9), 8e5
+    Tn = oracle.tensor_table(n, h)
+    M0 = W.random_unit_vectors(n, Ms, 5).astype(np.float64)
+    M0[0] += 2.0 * Ms                                        # mostly along +x with a random tilt
+    M0 *= Ms / np.sqrt((M0 * M0).sum(axis=0, keepdims=True))
+    Hz = (-2.0e4, 1.0e3, 0.0)                                # the switching field of PAPER.md:47
+    alpha, dt, steps = 0.1, 1.0e-13, 60
+    V = float(np.prod(h))
+
+    def energy_of(M):
+        Hd = oracle.fft_conv(Tn, M)
+        return oracle.energy(M, Hd, h) - oracle.MU0 * V * float((M * np.asarray(Hz).reshape(3, 1, 1, 1)).sum())
+    Es, M = [energy_of(M0)], M0
+    for _ in range(6):
+        M, _, _ = oracle.llg_rk4_run(Tn, M, Ms, Hz, alpha, dt, 10)
+        Es.append(energy_of(M))
+        assert np.abs(np.sqrt((M * M).sum(axis=0)) / Ms - 1.0).max() < 1e-9
+    assert all(b <= a + 1e-12 * abs(a) for a, b in zip(Es, Es[1:])), Es
+    assert Es[-1] < Es[0]
+    Mf, avg_full, nc_full = oracle.llg_rk4_run(Tn, M0, Ms, Hz, alpha, dt, steps)
+    Mx, avg_ext, nc_ext = oracle.llg_rk4_run(Tn, M0, Ms, Hz, alpha, dt, steps, extrapolate=True)
+    assert nc_full == 4 * steps and nc_ext == 16 + (steps - 4)
+    assert np.allclose(M, Mf, rtol=0, atol=1e-9 * Ms)       # 6 x 10 steps == 60 steps (no hidden state)
+    assert oracle.fig2_error(avg_ext, avg_full, Ms) < 1e-6
+    assert np.abs(Mx - Mf).max() / Ms < 1e-5
+
+
+def test_fig2_error_metric_by_hand(oracle):
+    """eps = sum_i ||M(t_i) - M~(t_i)|| / (n Ms)."""
+    ref = np.array([[1.0, 0.0, 0.0], [0.0, 2.0, 0.0], [0.0, 0.0, 3.0]])
+    got = ref + np.array([[3.0, 4.0, 0.0], [0.0, 0.0, 0.0], [0.0, 0.0, -2.0]])
+    assert abs(oracle.fig2_error(got, ref, 10.0) - (5.0 + 0.0 + 2.0) / (3 * 10.0)) < 1e-15
