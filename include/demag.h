@@ -223,6 +223,39 @@ demag_status demag_shard_set_peers(demag_plan_t plan, void* const* w1in_of_rank,
  * world > 1 return DEMAG_ERR_INVALID_ARG; demag_energy returns this rank's partial sum over its rows. */
 demag_status demag_apply_sharded(demag_plan_t plan, int phase, const void* M_loc_dev, void* H_loc_dev, void* cuda_stream);
 
+/* ---- Minimal time integrator that consumes the convolution: LLG equation, RK4, sub-step extrapolation ------------------
+ * (only as far as needed to reproduce the error metric of PAPER.md:47.)
+ *
+ * Eq. (5):  dm/dt = -gamma m x H_eff + alpha m x dm/dt,  m = M / Ms,  H_eff = H_d + H_Zee  (the other
+ * interaction fields of PAPER.md:94 are out of scope), solved for the derivative (R20):
+ *     dM/dt = -gamma / (1 + alpha^2) [ M x H_eff + (alpha / Ms) M x (M x H_eff) ],
+ * integrated with the classical 4th-order Runge-Kutta method, no renormalisation of |M| (R21).
+ * H_d = -N * M is demag_apply of the plan.  With extrapolate != 0 (R22) it is convolved only at the START of
+ * a step; the five most recent such fields are kept, and once five exist the fields of the three later stages (times
+ * t + dt/2, t + dt/2, t + dt) are the quartic through them (demag_extrapolate): one convolution per step instead of four.
+ *
+ * The integrator owns eight field-sized work arrays (stage magnetisation, RK sum, sub-step field, five kept fields),
+ * allocated in demag_llg_create; demag_llg_step only enqueues kernels on the stream (four fused stage kernels, one or
+ * four convolutions, up to two extrapolation passes), never allocates, never synchronises.  gamma in m/(A s)
+ * (mu0 |gamma_e| = 2.212761569e5), Ms and the fields in A/m, dt in seconds.  One-GPU plans only. */
+typedef struct demag_llg_s* demag_llg_t;
+demag_status demag_llg_create(demag_llg_t* out, demag_plan_t plan, double Ms, double alpha, double gamma);
+/* Uniform applied field H_Zee (A/m); (0, 0, 0) after create. */
+demag_status demag_llg_set_field(demag_llg_t llg, double Hx, double Hy, double Hz);
+/* One RK4 step of size dt, in place on M_dev ([3][nz][ny][nx], plan precision, 16-byte aligned). */
+demag_status demag_llg_step(demag_llg_t llg, void* M_dev, double dt, int extrapolate, void* cuda_stream);
+/* Mesh average of M ("the average magnetization is recorded every time step"): mean3_dev[0..2] (double,
+ * device), fp64 accumulation.  Asynchronous on the stream. */
+demag_status demag_llg_mean(demag_llg_t llg, const void* M_dev, double* mean3_dev, void* cuda_stream);
+/* Convolutions and extrapolation passes enqueued so far, and the integrator's time (any of the pointers may be NULL). */
+demag_status demag_llg_counts(demag_llg_t llg, long long* n_convolutions, long long* n_extrapolations, double* time);
+/* Forget the kept fields and set the time to zero (a new trajectory). */
+demag_status demag_llg_reset(demag_llg_t llg);
+demag_status demag_llg_destroy(demag_llg_t llg);
+
+/* Mesh sizes (the caller's nx, ny, nz) and precision of a plan (any of the pointers may be NULL). */
+demag_status demag_plan_dims(demag_plan_t plan, int* nx, int* ny, int* nz, int* precision);
+
 /* Last error message of the calling thread ("" if none). */
 const char* demag_last_error(void);
 

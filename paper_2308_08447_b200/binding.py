@@ -24,7 +24,9 @@ EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy
            "demag_last_error", "demag_plan_destroy", "demag_apply_profiled", "demag_path", "demag_apply_add",
            "demag_shard_range", "demag_plan_create_sharded", "demag_shard_info", "demag_shard_buffers",
            "demag_shard_ipc_export", "demag_shard_ipc_connect", "demag_shard_set_peers", "demag_apply_sharded",
-           "demag_set_pbc_images", "demag_extrapolate", "demag_atomistic_reserve"]
+           "demag_set_pbc_images", "demag_extrapolate", "demag_atomistic_reserve",
+           "demag_plan_dims", "demag_llg_create", "demag_llg_set_field", "demag_llg_step", "demag_llg_mean",
+           "demag_llg_counts", "demag_llg_reset", "demag_llg_destroy"]
 
 
 class DemagError(RuntimeError):
@@ -59,6 +61,14 @@ def lib():
         L.demag_apply_profiled.argtypes = [vp, vp, vp, vp, vp, vp]
         L.demag_apply_atomistic.argtypes = [vp, vp, vp, i, i, i, d, d, i, vp]
         L.demag_atomistic_reserve.argtypes = [vp]
+        L.demag_plan_dims.argtypes = [vp, vp, vp, vp, vp]
+        L.demag_llg_create.argtypes = [ctypes.POINTER(vp), vp, d, d, d]
+        L.demag_llg_set_field.argtypes = [vp, d, d, d]
+        L.demag_llg_step.argtypes = [vp, vp, d, i, vp]
+        L.demag_llg_mean.argtypes = [vp, vp, vp, vp]
+        L.demag_llg_counts.argtypes = [vp, vp, vp, vp]
+        L.demag_llg_reset.argtypes = [vp]
+        L.demag_llg_destroy.argtypes = [vp]
         L.demag_get_kernel_real.argtypes = [vp, vp]
         L.demag_workspace_bytes.argtypes = [vp]
         L.demag_workspace_bytes.restype = ctypes.c_size_t
@@ -378,6 +388,89 @@ class Plan:
     def close(self):
         if self.handle:
             demag_plan_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+GAMMA_LLG = 2.212761569e5      # mu0 |gamma_e| in m / (A s)  (include/demag.h "Minimal time integrator")
+
+
+def demag_plan_dims(plan) -> dict:
+    nx, ny, nz, pr = ctypes.c_int(), ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    _check(lib().demag_plan_dims(plan, ctypes.byref(nx), ctypes.byref(ny), ctypes.byref(nz), ctypes.byref(pr)))
+    return {"n": (nx.value, ny.value, nz.value), "precision": pr.value}
+
+
+def demag_llg_create(plan, Ms, alpha, gamma=GAMMA_LLG) -> int:
+    h = ctypes.c_void_p()
+    _check(lib().demag_llg_create(ctypes.byref(h), plan, float(Ms), float(alpha), float(gamma)))
+    return h.value
+
+
+def demag_llg_set_field(llg, H):
+    _check(lib().demag_llg_set_field(llg, float(H[0]), float(H[1]), float(H[2])))
+
+
+def demag_llg_step(llg, M, dt, extrapolate=False, stream=None):
+    _check(lib().demag_llg_step(llg, M.data_ptr(), float(dt), int(bool(extrapolate)), _stream(stream)))
+
+
+def demag_llg_mean(llg, M, out3, stream=None):
+    _check(lib().demag_llg_mean(llg, M.data_ptr(), out3.data_ptr(), _stream(stream)))
+
+
+def demag_llg_counts(llg) -> dict:
+    a, b, t = ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_double()
+    _check(lib().demag_llg_counts(llg, ctypes.byref(a), ctypes.byref(b), ctypes.byref(t)))
+    return {"convolutions": a.value, "extrapolations": b.value, "time": t.value}
+
+
+def demag_llg_reset(llg):
+    _check(lib().demag_llg_reset(llg))
+
+
+def demag_llg_destroy(llg):
+    lib().demag_llg_destroy(llg)
+
+
+class LLG:
+    """RK4 integrator of the LLG equation on top of a Plan (include/demag.h demag_llg_*).  Argument
+    marshalling only: every stage runs in the library's kernels."""
+
+    def __init__(self, plan: "Plan", Ms, alpha, gamma=GAMMA_LLG):
+        self.handle = demag_llg_create(plan.handle, Ms, alpha, gamma)
+        self.plan = plan
+
+    def set_field(self, H):
+        demag_llg_set_field(self.handle, H)
+        return self
+
+    def step(self, M, dt, extrapolate=False, stream=None):
+        demag_llg_step(self.handle, M, dt, extrapolate, stream)
+
+    def mean(self, M, out3, stream=None):
+        demag_llg_mean(self.handle, M, out3, stream)
+
+    def counts(self):
+        return demag_llg_counts(self.handle)
+
+    def reset(self):
+        demag_llg_reset(self.handle)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            demag_llg_destroy(self.handle)
             self.handle = None
 
     def __enter__(self):

@@ -572,6 +572,20 @@ int demag_launches_per_apply(demag_plan_t p)
 
 int demag_path(demag_plan_t p) { return p && p->v2 ? 1 : 0; }
 
+demag_status demag_plan_dims(demag_plan_t p, int* nx, int* ny, int* nz, int* precision)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (nx) *nx = p->on[0];
+    if (ny) *ny = p->sharded ? p->ny_loc : p->on[1];
+    if (nz) *nz = p->on[2];
+    if (precision) *precision = p->prec;
+    return DEMAG_OK;
+}
+
+// llg.cu reports its errors through the same thread-local message
+void demag_set_last_error_(const char* msg) { snprintf(g_err, sizeof(g_err), "%s", msg ? msg : ""); }
+
 demag_status demag_set_pbc_images(demag_plan_t p, int images)
 {
     g_err[0] = 0;
