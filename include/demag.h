@@ -10,7 +10,7 @@
  * x R2C FFT -> y FFT -> z FFT -> multiply with the transformed tensor -> inverse z, y -> x C2R.
  *
  * Conventions (readings R3, R6, R8):
- *   - mesh of nx*ny*nz cuboid cells of size hx*hy*hz metres, 1 <= n_a <= 4096;
+ *   - mesh of nx*ny*nz cuboid cells of size hx*hy*hz metres, 1 <= nx <= 8192, 1 <= ny, nz <= 4096;
  *   - an axis is zero-padded to N_a = 2 m_a, m_a = the next power of two >= n_a (an exact linear convolution needs
  *     N_a >= 2 n_a - 1), unless n_a == 1 or its PBC flag is set (then N_a = n_a, and a periodic
  *     n_a must itself be a power of two).  A mesh whose sizes are not all powers of two is embedded, with zeros,
@@ -42,7 +42,7 @@ typedef struct demag_plan_s* demag_plan_t;            /* opaque; owned by the li
 typedef enum {
     DEMAG_OK = 0,
     DEMAG_ERR_INVALID_ARG = 1,   /* NULL / misaligned / aliased pointer, non-positive size          */
-    DEMAG_ERR_UNSUPPORTED = 2,   /* size > 4096, periodic size not a power of two, built-in tensor + PBC,
+    DEMAG_ERR_UNSUPPORTED = 2,   /* size above the limits, periodic size not a power of two, built-in tensor + PBC,
                                     fp64 with nz > 2048 (an 8192-point fp64 z line exceeds shared memory)   */
     DEMAG_ERR_ALLOC = 3,         /* cudaMalloc / malloc failed                                       */
     DEMAG_ERR_CUDA = 4,          /* a CUDA runtime call or launch failed (see demag_last_error)      */

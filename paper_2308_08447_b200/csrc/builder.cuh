@@ -217,6 +217,43 @@ __global__ void __launch_bounds__(512) k_sym_axis(const double* __restrict__ in,
     }
 }
 
+// The same for a line too long for a complex tile (N = 16384: the x axis of nx = 8192 meshes): the real extended
+// sequence is packed into N/2 complex points z[m] = ext[2m] + i ext[2m+1], transformed with a length-N/2 FFT and split,
+//     X[k] = E[k] + w_N^k O[k],  E = (Z[k] + conj Z[N/2-k]) / 2,  O = -i (Z[k] - conj Z[N/2-k]) / 2.
+// One line per block (B = 1), N > n (an extended axis); tw = exp(-2 pi i k / N).
+__global__ void __launch_bounds__(512) k_sym_axis_packed(const double* __restrict__ in, double* __restrict__ out,
+                                                         int n, int lN, int nout, int par, int ni,
+                                                         size_t so_in, size_t se_in, size_t so_out, size_t se_out,
+                                                         const double2* __restrict__ tw)
+{
+    double2* s = reinterpret_cast<double2*>(demag_smem);
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int N = 1 << lN, Nh = N >> 1;
+    const int i = blockIdx.x % ni;
+    const size_t o = blockIdx.x / ni;
+    const double* src = in + o * so_in + i;
+    auto ext = [&](int e) -> double {
+        if (e < n) return src[(size_t)e * se_in];
+        if (e == n) return 0.0;
+        return par * src[(size_t)(N - e) * se_in];
+    };
+    for (int m = tid; m < Nh; m += nthr) s[swz<3>(m)] = make_double2(ext(2 * m), ext(2 * m + 1));
+    __syncthreads();
+    fft_tile<double, false, true>(s, lN - 1, 1, 1, tw, 1, tid, nthr);
+    double* dst = out + o * so_out + i;
+    for (int k = tid; k < nout; k += nthr) {
+        const double2 a = s[swz<3>(pos_of_freq(k & (Nh - 1), lN - 1))];
+        double2 b = s[swz<3>(pos_of_freq((Nh - k) & (Nh - 1), lN - 1))];
+        b.y = -b.y;                                                    // conj Z[N/2 - k]
+        const double er = 0.5 * (a.x + b.x), ei = 0.5 * (a.y + b.y);
+        const double dr = 0.5 * (a.x - b.x), di = 0.5 * (a.y - b.y);   // (Z - conj Z') / 2;  O = -i d = (di, -dr)
+        const double orr = di, oi = -dr;
+        const double2 w = k == Nh ? make_double2(-1.0, 0.0) : tw[k];
+        const double xr = er + w.x * orr - w.y * oi, xi = ei + w.x * oi + w.y * orr;
+        dst[(size_t)k * se_out] = par > 0 ? xr : xi;
+    }
+}
+
 // K[kx][kz'][py] = sign_y * scale * A[kz'][ky'][kx],  ky = freq_of_pos(py), ky' = min(ky, Ny-ky),
 // sign_y = -1 on mirrored ky of a component that is odd in y (the y axis is stored unpacked, in the
 // digit-reversed "position" order in which the y FFT leaves W2, so the hot path never permutes).

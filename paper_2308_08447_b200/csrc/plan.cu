@@ -301,7 +301,9 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         return fail(DEMAG_ERR_INVALID_ARG, "cell sizes must be positive and finite");
     if (precision != DEMAG_FP32 && precision != DEMAG_FP64) return fail(DEMAG_ERR_INVALID_ARG, "bad precision");
     if (pbc_flags & ~7u) return fail(DEMAG_ERR_INVALID_ARG, "bad pbc_flags");
-    if (nx > 4096 || ny > 4096 || nz > 4096) return fail(DEMAG_ERR_UNSUPPORTED, "mesh sizes must be <= 4096");
+    // x rows up to 8192 cells (a 16384-point real transform = 8192 quads = 128 KB of shared memory: the paper's own
+    // 7680 x 3840 x 2 mesh); y and z lines up to 4096 cells (an 8192-point line pair is the largest tile)
+    if (nx > 8192 || ny > 4096 || nz > 4096) return fail(DEMAG_ERR_UNSUPPORTED, "mesh sizes must be <= 8192 x 4096 x 4096");
     if (((pbc_flags & DEMAG_PBC_X) && !is_pow2(nx)) || ((pbc_flags & DEMAG_PBC_Y) && !is_pow2(ny)) ||
         ((pbc_flags & DEMAG_PBC_Z) && !is_pow2(nz)))
         return fail(DEMAG_ERR_UNSUPPORTED, "a periodic axis cannot be padded: its size must be a power of two (got %d x %d x %d)", nx, ny, nz);
@@ -422,6 +424,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         if (precision == DEMAG_FP32) { demag_status s = set_func_attrs<float>(); if (s) return s; }
         else { demag_status s = set_func_attrs<double>(); if (s) return s; }
         CUDA_TRY(cudaFuncSetAttribute(k_sym_axis, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
+        CUDA_TRY(cudaFuncSetAttribute(k_sym_axis_packed, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem));
         {
             cudaError_t zerr = cudaSuccess;
             if (getenv("DEMAG_NO_ZSPEC")) p->z_spec = false; else
@@ -624,6 +627,15 @@ demag_status launch_sym_axis(const double* in, double* out, int n, int N, int pa
                              size_t so_in, size_t se_in, size_t so_out, size_t se_out, const double2* tw)
 {
     const int lN = ilog2(N);
+    if ((size_t)N * sizeof(double2) > (size_t)kMaxSmem) {      // a 16384-point line: packed real transform, one line per block
+        if (N == n || (size_t)(N / 2) * sizeof(double2) > (size_t)kMaxSmem)
+            return fail(DEMAG_ERR_UNSUPPORTED, "kernel transform: a %d-point line does not fit in shared memory", N);
+        const size_t grid = (size_t)ni * no;
+        if (grid > 0x7fffffffULL) return fail(DEMAG_ERR_UNSUPPORTED, "kernel transform grid too large");
+        k_sym_axis_packed<<<(unsigned)grid, 512, (N / 2) * sizeof(double2)>>>(in, out, n, lN, N / 2 + 1, par, ni, so_in, se_in, so_out, se_out, tw);
+        CUDA_TRY(cudaGetLastError());
+        return DEMAG_OK;
+    }
     int B = std::max(1, std::min(8, 8192 / N));
     if (B > ni) B = ni;
     const long long elems = (long long)B * N;

@@ -17,6 +17,7 @@ template <> struct XCfg<9>  { static constexpr int POL = 1, RP = 8, NT = 256; };
 template <> struct XCfg<10> { static constexpr int POL = 1, RP = 4, NT = 256; };
 template <> struct XCfg<11> { static constexpr int POL = 1, RP = 2, NT = 256; };
 template <> struct XCfg<12> { static constexpr int POL = 5, RP = 1, NT = 256; };   // 16 . 16 . 16
+template <> struct XCfg<13> { static constexpr int POL = 6, RP = 1, NT = 256; };   // 16 . 16 . 32 (nx = 8192: the paper's 7680-cell rows)
 // y stage (K2v / K4v): radix policy, line pairs per tile, threads
 template <int LNY> struct YCfg { static constexpr int POL = 1, BP = 8, NT = 64; };
 template <> struct YCfg<8>  { static constexpr int POL = 1, BP = 8, NT = 128; };
@@ -58,13 +59,13 @@ inline int y_w2_pos_to_tile_pos(int LNY, int POL, int pw)
     const int lr = sc.lr[sc.n - 1], lnb = LNY - lr;
     return ((pw & ((1 << lnb) - 1)) << lr) + (pw >> lnb);
 }
-constexpr int kXMin = 4, kXMax = 12, kYMin = 4, kYMax = 13, kZMin = 2, kZMax = 11;
+constexpr int kXMin = 4, kXMax = 13, kYMin = 4, kYMax = 13, kZMin = 2, kZMax = 11;
 
 inline int x_rp(int lLc)
 {
-    switch (lLc) { case 10: return XCfg<10>::RP; case 11: return XCfg<11>::RP; case 12: return XCfg<12>::RP; default: return 8; }
+    switch (lLc) { case 10: return XCfg<10>::RP; case 11: return XCfg<11>::RP; case 12: return XCfg<12>::RP; case 13: return XCfg<13>::RP; default: return 8; }
 }
-inline int x_pol(int lLc) { return lLc == 8 ? XCfg<8>::POL : lLc == 12 ? XCfg<12>::POL : 1; }
+inline int x_pol(int lLc) { return lLc == 8 ? XCfg<8>::POL : lLc == 12 ? XCfg<12>::POL : lLc == 13 ? XCfg<13>::POL : 1; }
 inline bool y_has32(int lNy) { return lNy == 9 || lNy == 13; }
 inline int y_pol(int lNy, bool y32 = false) { return y32 && y_has32(lNy) ? 6 : 1; }
 inline int z_pol(int lNz) { return lNz == 4 ? ZCfg<4>::POL : 1; }
@@ -265,6 +266,7 @@ bool x_fwd(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cu
         V2_CASE_X(8, k_x_r2c_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
         V2_CASE_X(10, k_x_r2c_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
         V2_CASE_X(12, k_x_r2c_v, gp, M, W1, c.twx, c.twpost)
+    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_X(13, k_x_r2c_v, gp, M, W1, c.twx, c.twpost) } } return false;
     default: return false;
     }
 }
@@ -279,6 +281,7 @@ bool x_fwd_sh(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, cudaError_
         V2_CASE_X(8, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
         V2_CASE_X(10, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
         V2_CASE_X(12, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost)
+    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_X(13, k_x_r2c_sh_v, c.gx, M, c.m_in, c.twx, c.twpost) } } return false;
     default: return false;
     }
 }
@@ -293,6 +296,7 @@ bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cu
         V2_CASE_X(8, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(9, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
         V2_CASE_X(10, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(11, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
         V2_CASE_X(12, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
+    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_X(13, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) } } return false;
     default: return false;
     }
 }

@@ -142,6 +142,19 @@ def test_config4_4096x4096x8(torch, B, oracle):
     _sampled_check(torch, B, oracle, cfg, M, (0,), 48, full_field=False)
 
 
+def test_papers_own_meshes(torch, B, oracle):
+    """The meshes the paper itself runs (not powers of two): the Fig. 2 film, 2.4 um x 1.2 um x 10 nm in 5 nm cells =
+    480 x 240 x 2, and the mesh of its only printed single-GPU demag time, 58,982,400 cells = 7680 x 3840 x
+    2.  General sizes are embedded in the next powers of two (R10); Ms = 800 kA/m."""
+    from paper_2308_08447_b200 import workloads as W
+    _need_host_gb(24)
+    Ms, h = 8e5, (5e-9, 5e-9, 5e-9)
+    for n, nsamp, full in (((480, 240, 2), 128, True), ((7680, 3840, 2), 32, False)):
+        cfg = W.Config(f"paper mesh {n[0]}x{n[1]}x{n[2]}", n, h, Ms, 4700 + n[0], "random")
+        M = W.random_unit_vectors(n, Ms, cfg.seed)
+        _sampled_check(torch, B, oracle, cfg, M, (0,), nsamp, full_field=full)
+
+
 def test_config5_atomistic_1024cubed(torch, B, oracle):
     """1024^3 spins -> 4x4x4 macrocells -> 256^3 mesh -> field scattered back per spin (Eq. (9))."""
     from paper_2308_08447_b200 import workloads as W

@@ -87,9 +87,10 @@ def test_shapes_against_oracle(torch, B, oracle, n, prec):
     assert err <= (TOL32 if prec == 0 else TOL64), err
 
 
-@pytest.mark.parametrize("n", [(16, 16, 2048), (4, 4, 4096), (4096, 4, 1), (2, 4096, 2)])
+@pytest.mark.parametrize("n", [(16, 16, 2048), (4, 4, 4096), (4096, 4, 1), (2, 4096, 2), (8192, 32, 2), (8192, 4, 1)])
 def test_maximum_axis_lengths(torch, B, oracle, n):
-    """The longest transforms the library accepts (n_a = 4096 -> N_a = 8192) on every axis, incl. the z lengths beyond
+    """The longest transforms the library accepts (n_x = 8192 -> a 16384-point real transform; n_y, n_z = 4096 ->
+    N_a = 8192) on every axis, incl. the z lengths beyond
     the fast family's range (size-generic kernels); full field against the NumPy-FFT cross-check O-C, which is itself
     checked against Eq. (1) at sampled cells."""
     from paper_2308_08447_b200 import workloads as W
@@ -108,6 +109,10 @@ def test_maximum_axis_lengths(torch, B, oracle, n):
             continue
         H = run_gpu(torch, B, n, h, T, M, prec)
         assert np.abs(H - ref).max() / Ms <= (TOL32 if prec == 0 else TOL64)
+    for bad in ((8193, 4, 1), (4, 4097, 1), (4, 4, 4097)):
+        with pytest.raises(B.DemagError) as e:
+            B.demag_plan_create(*bad, *h, 0, 0)
+        assert e.value.status == 2
 
 
 @pytest.mark.parametrize("slab", [1, 3, 7])
