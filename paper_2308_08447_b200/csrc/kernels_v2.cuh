@@ -37,6 +37,8 @@ struct GeoV {
     int acc;             // x C2R: 0 = overwrite H, 1 = add into H (demag_apply_add)
     int trig;            // programmatic dependent launch: 0 = let the next grid in at block start, 1 = at block end
     int pf;              // L2 prefetch distance in blocks (0 = off): block b requests the input of tile b + pf
+    int onx, ony, onz;   // the caller's mesh when it is embedded in the power-of-two mesh nx, ny, nz (R10): the x
+                         // kernels read M / write H straight from / to the caller's arrays and supply the zeros themselves
     int kst;             // slot tiles per pair plane of the stored kernel spectrum, ceil((Ny/2 + 1) / KT) (1 for one-cell-thick meshes)
 };
 
@@ -898,19 +900,23 @@ __device__ __forceinline__ void x_r2c_body(const GeoV& g, const T* __restrict__ 
     const int tilesY = g.ny / (2 * RP);
     const int ty = blockIdx.x % tilesY, cz = blockIdx.x / tilesY;
     const int y0 = ty * 2 * RP;
-    const int nx = g.nx;
-    const T* rows = M + ((size_t)cz * g.ny + y0) * nx;
-    if (g.pf && tid == 0 && blockIdx.x + g.pf < gridDim.x)
-        pf_l2_bulk(M + (size_t)(blockIdx.x + g.pf) * (2 * RP) * nx, (uint32_t)(2 * RP * nx * sizeof(T)));
+    const int c = cz / g.nz, z = cz - c * g.nz;
+    // caller's array [3][onz][ony][onx] (= the transform mesh unless embedded); cells outside it are zeros
+    const int onx = g.onx, ony = g.ony;
+    const bool zin = z < g.onz;
+    const T* rows = M + (((size_t)c * g.onz + z) * ony + y0) * onx;
+    if (g.pf && tid == 0 && blockIdx.x + g.pf < gridDim.x && onx == g.nx && ony == g.ny)
+        pf_l2_bulk(M + (size_t)(blockIdx.x + g.pf) * (2 * RP) * onx, (uint32_t)(2 * RP * onx * sizeof(T)));
     auto ld = [&](int b, int m) {
-        const V r0 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b) * nx + 2 * m));
-        const V r1 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b + 1) * nx + 2 * m));
+        const bool xin = zin && 2 * m < onx;
+        V r0, r1; r0.x = r0.y = r1.x = r1.y = (T)0;
+        if (xin && y0 + 2 * b < ony) r0 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b) * onx + 2 * m));
+        if (xin && y0 + 2 * b + 1 < ony) r1 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b + 1) * onx + 2 * m));
         CQ<T> q; q.re.x = r0.x; q.re.y = r1.x; q.im.x = r0.y; q.im.y = r1.y; return q;
     };
     pass_first<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, ld);
     __syncthreads();
     FwdPasses<T, LLC, POL, 1, SC.n, RP, PITCH, NT>::run(s, tw, tid);
-    const int c = cz / g.nz, z = cz - c * g.nz;
     const size_t plane = (size_t)g.nz * g.ny;
     CQ<T>* out = SH ? nullptr : W1 + ((size_t)c * g.hq * g.nz + z) * g.ny + y0;
     constexpr int TOT = (LC / 2 + 1) * RP;
@@ -999,14 +1005,16 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     }
     __syncthreads();
     InvPasses<T, LLC, POL, 1, SC.n, RP, PITCH, NT>::run(s, tw, tid);
-    const int nx = g.nx, acc = g.acc;
-    T* rows = H + ((size_t)cz * g.ny + y0) * nx;
+    const int onx = g.onx, ony = g.ony, acc = g.acc;
+    const bool zin = z < g.onz;
+    T* rows = H + (((size_t)c * g.onz + z) * ony + y0) * onx;      // caller's array; cells outside it are dropped
     auto st = [&](int b, int m, CQ<T> v) {
+        if (!zin || 2 * m >= onx) return;
         V r0, r1; r0.x = v.re.x; r0.y = v.im.x; r1.x = v.re.y; r1.y = v.im.y;
-        V* d0 = reinterpret_cast<V*>(rows + (size_t)(2 * b) * nx + 2 * m);
-        V* d1 = reinterpret_cast<V*>(rows + (size_t)(2 * b + 1) * nx + 2 * m);
-        if (acc) { const V o0 = *d0, o1 = *d1; r0.x += o0.x; r0.y += o0.y; r1.x += o1.x; r1.y += o1.y; }
-        *d0 = r0; *d1 = r1;
+        V* d0 = reinterpret_cast<V*>(rows + (size_t)(2 * b) * onx + 2 * m);
+        V* d1 = reinterpret_cast<V*>(rows + (size_t)(2 * b + 1) * onx + 2 * m);
+        if (y0 + 2 * b < ony) { if (acc) { const V o0 = *d0; r0.x += o0.x; r0.y += o0.y; } *d0 = r0; }
+        if (y0 + 2 * b + 1 < ony) { if (acc) { const V o1 = *d1; r1.x += o1.x; r1.y += o1.y; } *d1 = r1; }
     };
     pass_last<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, st);
     pdl_leave(g);

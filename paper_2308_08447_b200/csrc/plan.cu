@@ -103,6 +103,7 @@ struct demag_plan_s {
     // general mesh sizes: the caller's mesh on[] is embedded (zeros) in the power-of-two mesh g.n* the transforms run on
     int on[3] = {0, 0, 0};
     bool embed = false;
+    bool embed_fused = false;            // fast path, even caller nx: the x kernels read M / write H of the caller directly (no copies)
     void* Mp = nullptr; void* Hp = nullptr;
     // several GPUs (demag_plan_create_sharded): W1 is W1in [3][nq_loc][nz][ny], W1out is [3][hq][nz][ny_loc]
     bool sharded = false, peers_set = false;
@@ -365,7 +366,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
     }
     if (p->v2) {
         v2::GeoV gv;
-        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0; gv.kst = (g.Ny / 2 + 1 + v2::z_kt(g.lNz) - 1) / v2::z_kt(g.lNz);
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0; gv.onx = nx; gv.ony = ny; gv.onz = nz; gv.kst = (g.Ny / 2 + 1 + v2::z_kt(g.lNz) - 1) / v2::z_kt(g.lNz);
         p->cf.gx = gv; p->cd.gx = gv;
         p->ny_loc = ny; p->nq_loc = gv.hq;
         if (sharded) {
@@ -377,6 +378,11 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
             gv.hq = p->nq_loc;                              // the y / z stages see only this rank's pairs
             p->cf.sharded = p->cd.sharded = true;
         }
+        if (p->embed && !sharded && p->on[0] % 2 == 0 && !getenv("DEMAG_NO_EMBED_FUSE")) {
+            p->embed_fused = true;                          // zeros supplied on load, crop on store (kernels_v2.cuh GeoV::onx)
+            p->cf.gx.onx = p->cd.gx.onx = p->on[0]; p->cf.gx.ony = p->cd.gx.ony = p->on[1]; p->cf.gx.onz = p->cd.gx.onz = p->on[2];
+        }
+        if (sharded) p->cf.gx.ony = p->cd.gx.ony = p->ny_loc;
         p->cf.g = gv; p->cd.g = gv;
         {   // one-cell-thick mesh: y FFT . multiply . y IFFT fused in one kernel, in place on W1 (scope row a3')
             const bool film = v2::film_supported(nz, g.Nz, g.lNy, p->esz, kMaxSmem) && !getenv("DEMAG_NO_FILM");
@@ -505,7 +511,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                 p->cf.yslot = p->cd.yslot = p->yslot;
             }
         }
-        if (p->embed) {
+        if (p->embed && !p->embed_fused) {
             const size_t b = (size_t)3 * nx * ny * nz * p->esz;
             CUDA_TRY(cudaMalloc(&p->Mp, b));
             CUDA_TRY(cudaMalloc(&p->Hp, b));
@@ -568,9 +574,10 @@ demag_status demag_set_slab(demag_plan_t p, int kx_per_slab)
 int demag_launches_per_apply(demag_plan_t p)
 {
     if (!p) return 0;
-    if (p->v2 && p->cf.film) return 3 + (p->embed ? 2 : 0);
+    const bool copies = p->embed && !p->embed_fused;
+    if (p->v2 && p->cf.film) return 3 + (copies ? 2 : 0);
     const int nslab = p->v2 ? (p->cf.g.hq + p->nq_slab - 1) / p->nq_slab : (p->g.hx + p->nkx_slab - 1) / p->nkx_slab;
-    return 2 + 3 * nslab + (p->embed ? 2 : 0);
+    return 2 + 3 * nslab + (copies ? 2 : 0);
 }
 
 int demag_path(demag_plan_t p) { return p && p->v2 ? 1 : 0; }
@@ -869,7 +876,7 @@ __global__ void __launch_bounds__(256) k_crop(int onx, int ony, int onz, int nx,
 template <typename T>
 demag_status apply_outer(demag_plan_s* p, const T* M, T* H, cudaStream_t st, StageTimer* tm = nullptr, int acc = 0)
 {
-    if (!p->embed) return apply_impl<T>(p, M, H, st, tm, acc);
+    if (!p->embed || p->embed_fused) return apply_impl<T>(p, M, H, st, tm, acc);
     const Geo& g = p->g;
     k_embed<T><<<dim3((unsigned)((g.nx + 255) / 256), (unsigned)g.ny, (unsigned)(3 * g.nz)), 256, 0, st>>>(
         p->on[0], p->on[1], p->on[2], g.nx, g.ny, g.nz, M, (T*)p->Mp);

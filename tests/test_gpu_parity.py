@@ -586,7 +586,7 @@ def test_error_paths(torch, B):
         B.demag_plan_create(12, 4, 4, 1e-9, 1e-9, 1e-9, B.DEMAG_PBC_X)
     assert e.value.status == 2                          # a periodic axis cannot be padded
     with pytest.raises(B.DemagError) as e:
-        B.demag_plan_create(8192, 4, 4, 1e-9, 1e-9, 1e-9)
+        B.demag_plan_create(8193, 4, 4, 1e-9, 1e-9, 1e-9)
     assert e.value.status == 2
     with pytest.raises(B.DemagError) as e:
         B.demag_plan_create(4, 4, 4, -1e-9, 1e-9, 1e-9)
