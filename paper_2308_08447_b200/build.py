@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
-UNITS = ["plan", "llg"] + [f"v2_{s}_{t}" for s in "xyz" for t in "fd"]
+UNITS = ["plan", "llg"] + [f"v2_{s}_{t}" for s in ("x", "y", "z", "xe") for t in "fd"]
 LIB = os.path.join(HERE, "libdemag_b200.so")
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]

@@ -20,6 +20,7 @@
 // Every kernel is templated on log2 of its transform length, its tile and its block size, so that every
 // shared-memory offset is an immediate; twiddles come from per-pass tables (dup format, [m-1][lo]).
 #pragma once
+#include <cuda.h>          // CUtensorMap (type only: the encoder is fetched through the runtime, v2_host.cuh)
 #include "soa_core.cuh"
 
 
@@ -39,6 +40,7 @@ struct GeoV {
     int pf;              // L2 prefetch distance in blocks (0 = off): block b requests the input of tile b + pf
     int onx, ony, onz;   // the caller's mesh when it is embedded in the power-of-two mesh nx, ny, nz (R10): the x
                          // kernels read M / write H straight from / to the caller's arrays and supply the zeros themselves
+    int pft;             // 1: the kernel's tensor map is valid -> the prefetch of a tile is ONE TMA request (pf_l2_tensor)
     int kst;             // slot tiles per pair plane of the stored kernel spectrum, ceil((Ny/2 + 1) / KT) (1 for one-cell-thick meshes)
 };
 
@@ -194,6 +196,13 @@ __device__ __forceinline__ void pf_l2_bulk(const void* p, uint32_t bytes)      /
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void pf_l2_line(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// a whole strided tile (box of the kernel's tensor map) in one request: the TMA unit walks the rows, no LSU instruction
+// per row (the per-row form costs the z kernel more than the prefetch gains when rows are 64-128 bytes)
+__device__ __forceinline__ void pf_l2_tensor(const CUtensorMap* tm, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 // a span of `bytes` bytes: one bulk request, or one plain request if it fits a 128-byte line
 __device__ __forceinline__ void pf_l2_span(const void* p, uint32_t bytes)
 {
@@ -696,7 +705,7 @@ template <int KT, int NCH> __device__ __forceinline__ size_t kslot(const int* __
 // to match at plan time (k_pack_film_v), which turns "odd in z" into "odd in y" without touching this code.
 template <typename T, int LNZ, int POL, int TY, int NT, int MINB, bool FILM = false>
 __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K,
-                                                  const int* __restrict__ yslot, TwSet<T> tw)
+                                                  const int* __restrict__ yslot, TwSet<T> tw, const __grid_constant__ CUtensorMap tmap)
 {
     pdl_enter(g);
     constexpr int NZ = 1 << LNZ, B = 3 * TY;
@@ -716,6 +725,7 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
         const int bn = blockIdx.x + g.pf, pytn = bn % tilesY, qln = bn / tilesY;
         const CQ<T>* bnx = W2 + (size_t)qln * g.nz * g.Ny + pytn * TY;
         if (FILM) { if (tid < 3) pf_l2_bulk(bnx + tid * cstride, (uint32_t)(g.nz * sizeof(CQ<T>))); }
+        else if (g.pft) { if (tid == 0) pf_l2_tensor(&tmap, pytn * TY * 4, 0, qln, 0); }       // box {TY quads, nz, 1 pair plane, 3 components}
         else for (int r = tid; r < 3 * g.nz; r += NT) { const int c = r / g.nz, z = r - c * g.nz; pf_l2_span(bnx + c * cstride + (size_t)z * Ny, (uint32_t)(TY * sizeof(CQ<T>))); }
     }
     // this thread's column in the fused pass (NT % TY == 0: the same for every item) and its slot in the stored spectrum
@@ -888,7 +898,7 @@ template <int LLC, typename T> __device__ __forceinline__ CQ<T> split_tw(const C
 
 // x R2C FFT fused with the zero padding and the transposition to y-contiguous storage
 // (PAPER.md:35, :296-300 xFFT_R2C; :343 "xy transposition ... to avoid strided y FFTs"):  M -> W1v
-template <typename T, int LLC, int POL, int RP, int NT, bool SH>
+template <typename T, int LLC, int POL, int RP, int NT, bool SH, bool EMB = false>
 __device__ __forceinline__ void x_r2c_body(const GeoV& g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
                                            const ShardMap<T>* map, const TwSet<T>& tw, const CQ<T>* __restrict__ twpost)
 {
@@ -908,10 +918,16 @@ __device__ __forceinline__ void x_r2c_body(const GeoV& g, const T* __restrict__ 
     if (g.pf && tid == 0 && blockIdx.x + g.pf < gridDim.x && onx == g.nx && ony == g.ny)
         pf_l2_bulk(M + (size_t)(blockIdx.x + g.pf) * (2 * RP) * onx, (uint32_t)(2 * RP * onx * sizeof(T)));
     auto ld = [&](int b, int m) {
-        const bool xin = zin && 2 * m < onx;
-        V r0, r1; r0.x = r0.y = r1.x = r1.y = (T)0;
-        if (xin && y0 + 2 * b < ony) r0 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b) * onx + 2 * m));
-        if (xin && y0 + 2 * b + 1 < ony) r1 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b + 1) * onx + 2 * m));
+        V r0, r1;
+        if (EMB) {      // embedded mesh: cells outside the caller's array are zeros (only these plans pay for the tests)
+            const bool xin = zin && 2 * m < onx;
+            r0.x = r0.y = r1.x = r1.y = (T)0;
+            if (xin && y0 + 2 * b < ony) r0 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b) * onx + 2 * m));
+            if (xin && y0 + 2 * b + 1 < ony) r1 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b + 1) * onx + 2 * m));
+        } else {
+            r0 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b) * onx + 2 * m));
+            r1 = __ldg(reinterpret_cast<const V*>(rows + (size_t)(2 * b + 1) * onx + 2 * m));
+        }
         CQ<T> q; q.re.x = r0.x; q.re.y = r1.x; q.im.x = r0.y; q.im.y = r1.y; return q;
     };
     pass_first<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, ld);
@@ -950,6 +966,15 @@ __global__ void __launch_bounds__(NT) k_x_r2c_v(GeoV g, const T* __restrict__ M,
     x_r2c_body<T, LLC, POL, RP, NT, false>(g, M, W1, nullptr, tw, twpost);
     pdl_leave(g);
 }
+// the same reading an embedded (smaller, any even nx) caller array
+template <typename T, int LLC, int POL, int RP, int NT>
+__global__ void __launch_bounds__(NT) k_x_r2c_e_v(GeoV g, const T* __restrict__ M, CQ<T>* __restrict__ W1,
+                                                 TwSet<T> tw, const CQ<T>* __restrict__ twpost)
+{
+    pdl_enter(g);
+    x_r2c_body<T, LLC, POL, RP, NT, false, true>(g, M, W1, nullptr, tw, twpost);
+    pdl_leave(g);
+}
 // the same on this rank's rows only (g.ny = rows of this rank), every pair stored at the rank that owns it
 template <typename T, int LLC, int POL, int RP, int NT>
 __global__ void __launch_bounds__(NT) k_x_r2c_sh_v(GeoV g, const T* __restrict__ M, const __grid_constant__ ShardMap<T> map,
@@ -962,11 +987,10 @@ __global__ void __launch_bounds__(NT) k_x_r2c_sh_v(GeoV g, const T* __restrict__
 
 // x C2R FFT fused with the crop; writes H:  W1v -> H
 //   2 Z[k] = A + i u,  2 Z[Lc-k] = conj(A - i u),  A = X[k] + conj X[Lc-k],  u = conj(w^k) (X[k] - conj X[Lc-k])
-template <typename T, int LLC, int POL, int RP, int NT>
-__global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict__ W1, T* __restrict__ H,
-                                               TwSet<T> tw, const CQ<T>* __restrict__ twpost)
+template <typename T, int LLC, int POL, int RP, int NT, bool EMB>
+__device__ __forceinline__ void x_c2r_body(const GeoV& g, const CQ<T>* __restrict__ W1, T* __restrict__ H,
+                                           const TwSet<T>& tw, const CQ<T>* __restrict__ twpost, const CUtensorMap& tmap)
 {
-    pdl_enter(g);
     using V = typename vec2<T>::type;
     constexpr int LC = 1 << LLC, PITCH = tile_pe(RP | 1, (RP < 8 && skew_ok(LLC, POL)) ? RP : 0, true);
     constexpr Sched SC = make_sched(LLC, POL);
@@ -981,7 +1005,8 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     if (g.pf && blockIdx.x + g.pf < gridDim.x) {
         const int bn = blockIdx.x + g.pf, tyn = bn % tilesY, czn = bn / tilesY, cn = czn / g.nz, zn = czn - cn * g.nz;
         const CQ<T>* inn = W1 + ((size_t)cn * g.hq * g.nz + zn) * g.ny + tyn * 2 * RP;
-        for (int k = tid; k <= LC / 2; k += NT) pf_l2_span(inn + (size_t)k * plane, (uint32_t)(2 * RP * sizeof(CQ<T>)));
+        if (g.pft) { for (int k0 = tid * 256; k0 <= LC / 2; k0 += NT * 256) pf_l2_tensor(&tmap, tyn * 2 * RP * 4, zn, k0, cn); }   // box {2 RP quads, 1, 256 pairs, 1}
+        else for (int k = tid; k <= LC / 2; k += NT) pf_l2_span(inn + (size_t)k * plane, (uint32_t)(2 * RP * sizeof(CQ<T>)));
     }
     constexpr int TOT = (LC / 2 + 1) * RP;
 #pragma unroll 2
@@ -1009,14 +1034,35 @@ __global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict_
     const bool zin = z < g.onz;
     T* rows = H + (((size_t)c * g.onz + z) * ony + y0) * onx;      // caller's array; cells outside it are dropped
     auto st = [&](int b, int m, CQ<T> v) {
-        if (!zin || 2 * m >= onx) return;
+        if (EMB && (!zin || 2 * m >= onx)) return;
         V r0, r1; r0.x = v.re.x; r0.y = v.im.x; r1.x = v.re.y; r1.y = v.im.y;
         V* d0 = reinterpret_cast<V*>(rows + (size_t)(2 * b) * onx + 2 * m);
         V* d1 = reinterpret_cast<V*>(rows + (size_t)(2 * b + 1) * onx + 2 * m);
-        if (y0 + 2 * b < ony) { if (acc) { const V o0 = *d0; r0.x += o0.x; r0.y += o0.y; } *d0 = r0; }
-        if (y0 + 2 * b + 1 < ony) { if (acc) { const V o1 = *d1; r1.x += o1.x; r1.y += o1.y; } *d1 = r1; }
+        if (EMB) {
+            if (y0 + 2 * b < ony) { if (acc) { const V o0 = *d0; r0.x += o0.x; r0.y += o0.y; } *d0 = r0; }
+            if (y0 + 2 * b + 1 < ony) { if (acc) { const V o1 = *d1; r1.x += o1.x; r1.y += o1.y; } *d1 = r1; }
+        } else {
+            if (acc) { const V o0 = *d0, o1 = *d1; r0.x += o0.x; r0.y += o0.y; r1.x += o1.x; r1.y += o1.y; }
+            *d0 = r0; *d1 = r1;
+        }
     };
     pass_last<T, LLC, POL, RP, PITCH, NT, false>(s, tw.p[0], tid, st);
+}
+template <typename T, int LLC, int POL, int RP, int NT>
+__global__ void __launch_bounds__(NT) k_x_c2r_v(GeoV g, const CQ<T>* __restrict__ W1, T* __restrict__ H,
+                                               TwSet<T> tw, const CQ<T>* __restrict__ twpost, const __grid_constant__ CUtensorMap tmap)
+{
+    pdl_enter(g);
+    x_c2r_body<T, LLC, POL, RP, NT, false>(g, W1, H, tw, twpost, tmap);
+    pdl_leave(g);
+}
+// the same writing an embedded caller array (the crop of the cells outside it)
+template <typename T, int LLC, int POL, int RP, int NT>
+__global__ void __launch_bounds__(NT) k_x_c2r_e_v(GeoV g, const CQ<T>* __restrict__ W1, T* __restrict__ H,
+                                                 TwSet<T> tw, const CQ<T>* __restrict__ twpost, const __grid_constant__ CUtensorMap tmap)
+{
+    pdl_enter(g);
+    x_c2r_body<T, LLC, POL, RP, NT, true>(g, W1, H, tw, twpost, tmap);
     pdl_leave(g);
 }
 

@@ -24,6 +24,8 @@ namespace v2 {
     extern template bool x_fwd<T>(int, const Ctx<T>&, cudaStream_t, const T*, CQ<T>*, cudaError_t*);                     \
     extern template bool x_fwd_sh<T>(int, const Ctx<T>&, cudaStream_t, const T*, cudaError_t*);                          \
     extern template bool x_inv<T>(int, const Ctx<T>&, cudaStream_t, const CQ<T>*, T*, cudaError_t*, int);                \
+    extern template bool x_fwd_e<T>(int, const Ctx<T>&, cudaStream_t, const T*, CQ<T>*, cudaError_t*);                   \
+    extern template bool x_inv_e<T>(int, const Ctx<T>&, cudaStream_t, const CQ<T>*, T*, cudaError_t*, int);              \
     extern template bool y_fwd<T>(int, const Ctx<T>&, cudaStream_t, int, int, const CQ<T>*, CQ<T>*, cudaError_t*);       \
     extern template bool y_inv<T>(int, const Ctx<T>&, cudaStream_t, int, int, const CQ<T>*, CQ<T>*, cudaError_t*);       \
     extern template bool y_inv_sh<T>(int, const Ctx<T>&, cudaStream_t, int, int, const CQ<T>*, cudaError_t*);            \
@@ -366,7 +368,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
     }
     if (p->v2) {
         v2::GeoV gv;
-        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0; gv.onx = nx; gv.ony = ny; gv.onz = nz; gv.kst = (g.Ny / 2 + 1 + v2::z_kt(g.lNz) - 1) / v2::z_kt(g.lNz);
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0; gv.pft = 0; gv.onx = nx; gv.ony = ny; gv.onz = nz; gv.kst = (g.Ny / 2 + 1 + v2::z_kt(g.lNz) - 1) / v2::z_kt(g.lNz);
         p->cf.gx = gv; p->cd.gx = gv;
         p->ny_loc = ny; p->nq_loc = gv.hq;
         if (sharded) {
@@ -451,6 +453,10 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                 p->cf.twx = p->tf[0].set; p->cf.twy = p->tf[1].set; p->cf.twz = p->tf[2].set;
                 v2::x_fwd<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::x_inv<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                if (p->embed_fused) {
+                    v2::x_fwd_e<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                    v2::x_inv_e<float>(0, p->cf, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                }
                 v2::y_fwd<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::y_inv<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::z_mul<float>(0, p->cf, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
@@ -467,6 +473,10 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                 p->cd.twx = p->td[0].set; p->cd.twy = p->td[1].set; p->cd.twz = p->td[2].set;
                 v2::x_fwd<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::x_inv<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                if (p->embed_fused) {
+                    v2::x_fwd_e<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                    v2::x_inv_e<double>(0, p->cd, nullptr, nullptr, nullptr, &verr); CUDA_TRY(verr);
+                }
                 v2::y_fwd<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::y_inv<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
                 v2::z_mul<double>(0, p->cd, nullptr, 0, 0, nullptr, nullptr, &verr); CUDA_TRY(verr);
@@ -480,7 +490,10 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                 // Measured (profiles/r2_01_prefetch.md): the y kernels gain 5-19 % (whole lines: one bulk request each), the
                 // z kernel gains 11 % when its rows are >= 512 bytes (C4, 32 columns) and loses with 64-128 byte rows, the
                 // x kernels do not gain (R2C) or lose (C2R: one request per 32-256 byte piece)
-                int mask = 2 | 8 | ((size_t)v2::z_ty(g.lNz) * 4 * p->esz >= 512 && g.lNz >= 4 ? 4 : 0);
+                // With a tensor map the whole strided tile is ONE request (profiles/r2_01_prefetch.md): the z kernel then gains
+                // 4 % with narrow rows too (C3, C5), the x C2R kernel 5 % where its pieces are 32-64 bytes (long rows, C4)
+                const bool z_wide = (size_t)v2::z_ty(g.lNz) * 4 * p->esz >= 512, z_tmap = g.nz <= 256 && !getenv("DEMAG_NO_TMAP");
+                int mask = 2 | 8 | (g.lNz >= 4 && (z_wide || z_tmap) ? 4 : 0) | (v2::x_rp(g.lLc) <= 2 && !sharded && !getenv("DEMAG_NO_TMAP") ? 16 : 0);
                 if (const char* e = getenv("DEMAG_PF_MASK")) mask = atoi(e);
                 auto apply_mask = [&](auto& c) {
                     if (!(mask & 1)) c.pf_xf = 0;
@@ -522,6 +535,29 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         CUDA_TRY(cudaMalloc(&p->W2, p->w2_bytes));
         CUDA_TRY(cudaMalloc(&p->K, p->k_bytes));
         CUDA_TRY(cudaMemset(p->K, 0, p->k_bytes));
+        if (p->v2 && !p->cf.film && !getenv("DEMAG_NO_TMAP")) {
+            // tensor maps for the one-request tile prefetch (kernels_v2.cuh pf_l2_tensor); a failure only disables it
+            const v2::GeoV& gv = p->cf.g;
+            const unsigned long long q = 4 * p->esz;                                   // bytes per quad
+            const int ty = v2::z_ty(g.lNz);
+            if (g.lNz >= 4 && g.nz <= 256 && ty * 4 <= 256) {                          // z kernel: box {TY quads, nz, 1, 3}
+                const unsigned long long dim[4] = {(unsigned long long)g.Ny * 4, (unsigned long long)g.nz, (unsigned long long)p->nq_auto, 3};
+                const unsigned long long sb[3] = {g.Ny * q, (unsigned long long)g.nz * g.Ny * q, (unsigned long long)p->nq_auto * g.nz * g.Ny * q};
+                const unsigned box[4] = {(unsigned)ty * 4, (unsigned)g.nz, 1, 3};
+                v2::TMap tm;
+                if (v2::encode_tmap4(&tm, p->esz, p->W2, dim, sb, box)) { p->cf.tm_z = p->cd.tm_z = tm; p->cf.tm_z_nq = p->cd.tm_z_nq = p->nq_auto; }
+                else if (ty * 4 * p->esz < 512) p->cf.pf_z = p->cd.pf_z = 0;          // no map: narrow rows do not prefetch
+            }
+            if (!sharded) {                                                             // x C2R: box {2 RP quads, 1, 256 pairs, 1}
+                const int rp = v2::x_rp(g.lLc);
+                const unsigned long long dim[4] = {(unsigned long long)g.ny * 4, (unsigned long long)g.nz, (unsigned long long)gv.hq, 3};
+                const unsigned long long sb[3] = {g.ny * q, (unsigned long long)g.nz * g.ny * q, (unsigned long long)gv.hq * g.nz * g.ny * q};
+                const unsigned box[4] = {(unsigned)(2 * rp * 4), 1, (unsigned)std::min(gv.hq, 256), 1};
+                v2::TMap tm;
+                if (v2::encode_tmap4(&tm, p->esz, p->W1, dim, sb, box)) { p->cf.tm_xi = p->cd.tm_xi = tm; p->cf.tm_xi_ok = p->cd.tm_xi_ok = true; }
+                else p->cf.pf_xi = p->cd.pf_xi = 0;
+            }
+        }
         const int N[3] = {g.Nx, g.Ny, g.Nz};
         for (int a = 0; a < 3; ++a) {
             demag_status s = precision == DEMAG_FP32 ? make_twiddles<float2>(N[a], &p->tw[a], &p->tw_bytes)
@@ -803,7 +839,8 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
         const typename v2::kchunks<T>::V* Kv = (const typename v2::kchunks<T>::V*)p->K;
         cudaError_t verr = cudaSuccess;
         bool ok = true;             // a launcher returns false when no kernel is instantiated for the size (a stage would be skipped)
-        STAGE(0, (ok &= v2::x_fwd<T>(1, cx, st, M, V1, &verr)));
+        if (p->embed_fused) STAGE(0, (ok &= v2::x_fwd_e<T>(1, cx, st, M, V1, &verr)));
+        else STAGE(0, (ok &= v2::x_fwd<T>(1, cx, st, M, V1, &verr)));
         if (cx.film) STAGE(2, (ok &= v2::y_film<T>(1, cx, st, V1, Kv, &verr)));
         else for (int q0 = 0; q0 < cx.g.hq; q0 += p->nq_slab) {
             const int nq = std::min(p->nq_slab, cx.g.hq - q0);
@@ -811,7 +848,8 @@ demag_status apply_impl(demag_plan_s* p, const T* M, T* H, cudaStream_t st, Stag
             STAGE(2, (ok &= v2::z_mul<T>(1, cx, st, q0, nq, V2, Kv, &verr)));
             STAGE(3, (ok &= v2::y_inv<T>(1, cx, st, q0, nq, V2, V1, &verr)));
         }
-        STAGE(4, (ok &= v2::x_inv<T>(1, cx, st, V1, H, &verr, acc)));
+        if (p->embed_fused) STAGE(4, (ok &= v2::x_inv_e<T>(1, cx, st, V1, H, &verr, acc)));
+        else STAGE(4, (ok &= v2::x_inv<T>(1, cx, st, V1, H, &verr, acc)));
         if (!ok) return fail(DEMAG_ERR_UNSUPPORTED, "no kernel instantiated for a stage of this plan (fast family)");
         CUDA_TRY(cudaGetLastError());
         return DEMAG_OK;

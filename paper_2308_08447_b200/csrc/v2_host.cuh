@@ -196,6 +196,36 @@ inline bool film_supported(int nz, int Nz, int lNy, size_t esz, int max_smem)
     return nz == 1 && Nz == 1 && lNy >= 4 && lNy <= 12 && (size_t)z_tile_quads(lNy, film_pol(lNy), 1) * 4 * esz <= (size_t)max_smem;
 }
 
+// ---- tensor maps (TMA descriptors) for the one-request prefetch of a strided tile (kernels_v2.cuh pf_l2_tensor) --------
+// 4D views of a workspace, dimension 0 = the contiguous axis in REALS (4 per quad).  The encoder is a driver function;
+// it is fetched through the runtime so that the library does not link libcuda.
+struct TMap { alignas(64) CUtensorMap m; };
+inline bool encode_tmap4(TMap* out, size_t esz, const void* base, const unsigned long long dim[4],
+                         const unsigned long long stride_bytes[3], const unsigned box[4])
+{
+    typedef CUresult (*Fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                           const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                           CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static Fn fn = nullptr;
+    if (!fn) {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess || !f) {
+            cudaGetLastError();
+            return false;
+        }
+        fn = (Fn)f;
+    }
+    for (int i = 0; i < 4; ++i) if (box[i] < 1 || box[i] > 256 || dim[i] < 1) return false;
+    if ((box[0] * esz) % 16 != 0) return false;
+    for (int i = 0; i < 3; ++i) if (stride_bytes[i] % 16 != 0 || stride_bytes[i] >= (1ULL << 40)) return false;
+    cuuint64_t d[4] = {dim[0], dim[1], dim[2], dim[3]}, sb[3] = {stride_bytes[0], stride_bytes[1], stride_bytes[2]};
+    cuuint32_t b[4] = {box[0], box[1], box[2], box[3]}, es[4] = {1, 1, 1, 1};
+    return fn(&out->m, esz == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), d, sb, b, es,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // ---- launchers ---------------------------------------------------------------------------------------------
 template <typename T> struct Ctx {
     int sm_count;
@@ -210,6 +240,9 @@ template <typename T> struct Ctx {
     int lLc, lNy, lNz;
     TwSet<T> twx, twy, twz;
     const CQ<T>* twpost;
+    TMap tm_z = {}, tm_xi = {}; // W2v as the z kernel tiles it / W1v as the x C2R kernel tiles it (valid iff tm_z_nq > 0 / tm_xi_ok)
+    int tm_z_nq = 0;            // pair planes per slab the W2v map was encoded for (its component stride)
+    bool tm_xi_ok = false;
     const int* yslot = nullptr; // slot | mirrored << 31 of every W2v position (kernels_v2.cuh "Kv"); device memory
     // L2 prefetch distance (kernels_v2.cuh pf_l2_*): pf_waves x (co-resident blocks of the kernel), per kernel; filled
     // in at plan time (mode 0 of the launchers) from the occupancy the runtime reports
@@ -243,6 +276,7 @@ template <typename K> inline int pf_distance(float waves, int sm_count, K kern, 
     return d < 1.f ? 1 : (int)d;
 }
 template <typename G> inline G with_pf(G g, int pf) { g.pf = pf; return g; }
+template <typename G> inline G with_pft(G g, bool on) { g.pft = on ? 1 : 0; return g; }
 
 #define V2_CASE_X(L, KERN, ...)                                                                                     \
     case L: {                                                                                                        \
@@ -270,6 +304,22 @@ bool x_fwd(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cu
     default: return false;
     }
 }
+// the same for an embedded caller array (kernels_v2.cuh GeoV::onx)
+template <typename T>
+bool x_fwd_e(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, CQ<T>* W1, cudaError_t* err)
+{
+    int* pfd = &c.pf_xf;
+    const GeoV gp = with_pf(c.gx, c.pf_xf);
+    switch (c.lLc) {
+        V2_CASE_X(4, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(5, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(6, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(7, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(8, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(9, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(10, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost) V2_CASE_X(11, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost)
+        V2_CASE_X(12, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost)
+    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_X(13, k_x_r2c_e_v, gp, M, W1, c.twx, c.twpost) } } return false;
+    default: return false;
+    }
+}
 // several GPUs: rows of this rank in, pairs stored at their owners (k_x_r2c_sh_v)
 template <typename T>
 bool x_fwd_sh(int mode, const Ctx<T>& c, cudaStream_t st, const T* M, cudaError_t* err)
@@ -289,14 +339,30 @@ template <typename T>
 bool x_inv(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cudaError_t* err, int acc = 0)
 {
     int* pfd = &c.pf_xi;
-    GeoV ga = c.gx; ga.acc = acc; ga.pf = c.pf_xi;
+    GeoV ga = c.gx; ga.acc = acc; ga.pf = c.pf_xi; ga.pft = c.tm_xi_ok ? 1 : 0;
     switch (c.lLc) {
-        V2_CASE_X(4, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(5, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
-        V2_CASE_X(6, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(7, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
-        V2_CASE_X(8, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(9, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
-        V2_CASE_X(10, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) V2_CASE_X(11, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
-        V2_CASE_X(12, k_x_c2r_v, ga, W1, H, c.twx, c.twpost)
-    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_X(13, k_x_c2r_v, ga, W1, H, c.twx, c.twpost) } } return false;
+        V2_CASE_X(4, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(5, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(6, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(7, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(8, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(9, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(10, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(11, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(12, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_X(13, k_x_c2r_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) } } return false;
+    default: return false;
+    }
+}
+
+template <typename T>
+bool x_inv_e(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, cudaError_t* err, int acc = 0)
+{
+    int* pfd = &c.pf_xi;
+    GeoV ga = c.gx; ga.acc = acc; ga.pf = c.pf_xi; ga.pft = c.tm_xi_ok ? 1 : 0;
+    switch (c.lLc) {
+        V2_CASE_X(4, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(5, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(6, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(7, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(8, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(9, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(10, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) V2_CASE_X(11, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+        V2_CASE_X(12, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m)
+    case 13: if constexpr (sizeof(T) == 4) { switch (13) { V2_CASE_X(13, k_x_c2r_e_v, ga, W1, H, c.twx, c.twpost, c.tm_xi.m) } } return false;
     default: return false;
     }
 }
@@ -389,7 +455,7 @@ bool y_inv_sh(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const 
         constexpr int smem = z_tile_quads(L, C::POL, C::TY) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) { *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
                          c.pf_z = pf_distance(c.pf_waves, c.sm_count, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, C::NT, smem); } \
-        else launch_pdl(c.pdl, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, (unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st, with_pf(c.g, c.pf_z), q0, nq, W2, K, c.yslot, c.twz); \
+        else launch_pdl(c.pdl, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, (unsigned)(nq * (c.g.Ny / C::TY)), C::NT, smem, st, with_pft(with_pf(c.g, c.pf_z), nq == c.tm_z_nq), q0, nq, W2, K, c.yslot, c.twz, c.tm_z.m); \
         return true;                                                                                                 \
     }
 template <typename T>
@@ -418,7 +484,7 @@ bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2
         constexpr int smem = z_tile_quads(L, POL_, 1) * (int)sizeof(CQ<T>);                                          \
         if (mode == 0) { *err = cudaFuncSetAttribute(k_z_v<T, L, POL_, 1, NT_, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
                          c.pf_film = pf_distance(c.pf_waves, c.sm_count, k_z_v<T, L, POL_, 1, NT_, 1, true>, NT_, smem); } \
-        else launch_pdl(c.pdl, k_z_v<T, L, POL_, 1, NT_, 1, true>, (unsigned)c.g.hq, NT_, smem, st, with_pf(c.gfilm, c.pf_film), 0, c.g.hq, W1, K, (const int*)nullptr, c.twy); \
+        else launch_pdl(c.pdl, k_z_v<T, L, POL_, 1, NT_, 1, true>, (unsigned)c.g.hq, NT_, smem, st, with_pf(c.gfilm, c.pf_film), 0, c.g.hq, W1, K, (const int*)nullptr, c.twy, c.tm_z.m); \
         return true;                                                                                                 \
     }
 template <typename T>

@@ -1,0 +1,3 @@
+#define V2_INST_STAGE 3
+#define V2_INST_T float
+#include "v2_inst.cuh"
