@@ -213,10 +213,14 @@ __device__ __forceinline__ void pf_l2_span(const void* p, uint32_t bytes)
 // Long strides (S >= 64): only w^lo is loaded and the powers are formed by multiplication (depth <= 4, i.e. a few
 // ulp, far inside the tolerances): the full table of a long pass ((R-1) S quads, 57 KB for a 4096-point line) does not
 // stay in L1 next to the tile and was measured to triple the L2 read traffic of the long-line kernels (C4).
-template <int LR, int LS, typename T>
+// SPREAD: the lanes of a warp hold (nearly) all different lo -- points-fastest thread order, or fewer than 8 lines per
+// tile -- so every table load costs a full 512-byte register writeback: the powers are formed from w^lo for any stride
+// >= 8 (measured on the x kernels: -13 % at C3).  With lines-fastest order over >= 8 lines a warp reads 1-4 distinct
+// entries per load (cheap broadcasts) and loading stays faster up to stride 32.
+template <int LR, int LS, bool SPREAD, typename T>
 __device__ __forceinline__ void load_tw(CQ<T>* w, const CQ<T>* __restrict__ tab, int lo)
 {
-    if (LS >= 6 && LR >= 2) {
+    if (LS >= (SPREAD ? 3 : 6) && LR >= 2) {
         w[1] = ldgq(tab + lo);
         w[2] = cmul(w[1], w[1]); w[3] = cmul(w[2], w[1]);
         if (LR >= 3) { w[4] = cmul(w[2], w[2]); w[5] = cmul(w[4], w[1]); w[6] = cmul(w[3], w[3]); w[7] = cmul(w[4], w[3]); }
@@ -283,8 +287,9 @@ __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab,
     constexpr int TOT = NBF * BL;
     constexpr int ITER = (TOT + NT - 1) / NT;
     constexpr bool HOIST = (LS > 0) && (NT % BL == 0) && ((NT / BL) % S == 0) && ITER > 1;
+    constexpr bool SPREAD = BL < 8;
     CQ<T> w[R];
-    if (HOIST) load_tw<LR, LS>(w, tab, (tid / BL) & (S - 1));
+    if (HOIST) load_tw<LR, LS, SPREAD>(w, tab, (tid / BL) & (S - 1));
 #pragma unroll(ITER <= 2 ? ITER : 1)
     for (int k = 0; k < ITER; ++k) {
         const int t = tid + k * NT;
@@ -298,9 +303,9 @@ __device__ __forceinline__ void pass_ss(CQ<T>* s, const CQ<T>* __restrict__ tab,
         for (int r = 0; r < R; ++r) a[r] = ldq(d + tile_leg<PITCH, S>(r));
         if (!INV) {
             dftR<LR, false, false>(a);
-            if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, lo); apply_tw<LR, false>(a, w); }
+            if (LS > 0) { if (!HOIST) load_tw<LR, LS, SPREAD>(w, tab, lo); apply_tw<LR, false>(a, w); }
         } else {
-            if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, lo); apply_tw<LR, true>(a, w); }
+            if (LS > 0) { if (!HOIST) load_tw<LR, LS, SPREAD>(w, tab, lo); apply_tw<LR, true>(a, w); }
             dftR<LR, true, false>(a);
         }
 #pragma unroll
@@ -366,8 +371,9 @@ __device__ __forceinline__ void pass_first(CQ<T>* s, const CQ<T>* __restrict__ t
     constexpr int TOT = S * BL;
     constexpr int ITER = (TOT + NT - 1) / NT;
     constexpr bool HOIST = (LS > 0) && ITER > 1 && (LF ? (NT % BL == 0 && (NT / BL) % S == 0) : (NT % S == 0));
+    constexpr bool SPREAD = !LF || BL < 8;
     CQ<T> w[R];
-    if (HOIST) load_tw<LR, LS>(w, tab, LF ? ((tid / BL) & (S - 1)) : (tid & (S - 1)));
+    if (HOIST) load_tw<LR, LS, SPREAD>(w, tab, LF ? ((tid / BL) & (S - 1)) : (tid & (S - 1)));
     // software pipeline (short loops): the (global) inputs of butterfly k+1 are requested before butterfly k is computed
     constexpr int H = R > 1 ? R / 2 : 1;
     CQ<T> nxt[H];
@@ -391,7 +397,7 @@ __device__ __forceinline__ void pass_first(CQ<T>* s, const CQ<T>* __restrict__ t
         for (int r = 0; r < H; ++r) a[r] = nxt[r];
         if (ITER <= 4 && k + 1 < ITER) fetch(k + 1);
         dftR<LR, false, true>(a);
-        if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, false>(a, w); }
+        if (LS > 0) { if (!HOIST) load_tw<LR, LS, SPREAD>(w, tab, i); apply_tw<LR, false>(a, w); }
         CQ<T>* d = s + tile_addr<PITCH>(i, b);
 #pragma unroll
         for (int r = 0; r < R; ++r) stq(d + tile_leg<PITCH, S>(r), a[r]);
@@ -406,8 +412,9 @@ __device__ __forceinline__ void pass_last(const CQ<T>* s, const CQ<T>* __restric
     constexpr int TOT = S * BL;
     constexpr int ITER = (TOT + NT - 1) / NT;
     constexpr bool HOIST = (LS > 0) && ITER > 1 && (LF ? (NT % BL == 0 && (NT / BL) % S == 0) : (NT % S == 0));
+    constexpr bool SPREAD = !LF || BL < 8;
     CQ<T> w[R];
-    if (HOIST) load_tw<LR, LS>(w, tab, LF ? ((tid / BL) & (S - 1)) : (tid & (S - 1)));
+    if (HOIST) load_tw<LR, LS, SPREAD>(w, tab, LF ? ((tid / BL) & (S - 1)) : (tid & (S - 1)));
 #pragma unroll(ITER <= 2 ? ITER : 1)
     for (int k = 0; k < ITER; ++k) {
         const int t = tid + k * NT;
@@ -417,7 +424,7 @@ __device__ __forceinline__ void pass_last(const CQ<T>* s, const CQ<T>* __restric
         CQ<T> a[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) a[r] = ldq(d + tile_leg<PITCH, S>(r));
-        if (LS > 0) { if (!HOIST) load_tw<LR, LS>(w, tab, i); apply_tw<LR, true>(a, w); }
+        if (LS > 0) { if (!HOIST) load_tw<LR, LS, SPREAD>(w, tab, i); apply_tw<LR, true>(a, w); }
         dftR<LR, true, false>(a);
 #pragma unroll
         for (int r = 0; r < R / 2; ++r) st(b, i + r * S, a[r]);
@@ -727,6 +734,12 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
         if (FILM) { if (tid < 3) pf_l2_bulk(bnx + tid * cstride, (uint32_t)(g.nz * sizeof(CQ<T>))); }
         else if (g.pft) { if (tid == 0) pf_l2_tensor(&tmap, pytn * TY * 4, 0, qln, 0); }       // box {TY quads, nz, 1 pair plane, 3 components}
         else for (int r = tid; r < 3 * g.nz; r += NT) { const int c = r / g.nz, z = r - c * g.nz; pf_l2_span(bnx + c * cstride + (size_t)z * Ny, (uint32_t)(TY * sizeof(CQ<T>))); }
+        if (!FILM && tid >= NT - 2) {
+            // the spectrum rows of that tile: the slot tile(s) its first and last column fall into (contiguous kpz rows each)
+            const int sl = __ldg(yslot + pytn * TY + (tid == NT - 1 ? TY - 1 : 0)) & 0x7fffffff;
+            const uint32_t kb = (uint32_t)(g.kpz * kchunks<T>::N * TY * sizeof(typename kchunks<T>::V));
+            pf_l2_bulk(K + ((size_t)(q0 + qln) * g.kst + sl / TY) * g.kpz * (kchunks<T>::N * TY), kb);
+        }
     }
     // this thread's column in the fused pass (NT % TY == 0: the same for every item) and its slot in the stored spectrum
     float sy;
@@ -735,9 +748,71 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
     pass_first<T, LNZ, POL, B, PE, NT, true>(s, tw.p[0], tid, ld);
     __syncthreads();
     FwdPasses<T, LNZ, POL, 1, NP - 1, B, PE, NT>::run(s, tw, tid);
-    {   // fused: last forward pass . multiply . first inverse pass; item = (butterfly i, column ty), 3 components
+    const typename kchunks<T>::V* Kq = K + (size_t)(q0 + ql) * g.kst * g.kpz * (kchunks<T>::N * TY);   // KT == TY
+    auto load_fwd = [&](CQ<T> (*a)[RF], int p0, int ty) {
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) {
+#pragma unroll
+            for (int m = 0; m < RF; ++m) a[cc][m] = ldq(s + tile_addr<PE>(p0, cc * TY + ty) + tile_leg<PE, 1>(m));
+            dftR<LRF, false, false>(a[cc]);
+        }
+    };
+    auto inv_store = [&](CQ<T> (*a)[RF], int p0, int ty) {
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) {
+            dftR<LRF, true, false>(a[cc]);
+#pragma unroll
+            for (int m = 0; m < RF; ++m) stq(s + tile_addr<PE>(p0, cc * TY + ty) + tile_leg<PE, 1>(m), a[cc][m]);
+        }
+    };
+    if constexpr (LRF == 3 && sizeof(T) == 4 && ((NZ >> 4) * TY >= NT)) {      // (enough pairs to occupy every thread)
+        // fused: last forward pass . multiply . first inverse pass, TWO butterflies per work unit.  Butterfly f (0 <= f < W,
+        // W = Nz / 8) holds kz = f + m W, m = 0..7; its points m >= 4 are mirrored frequencies whose packed rows
+        // Nz - kz = (W - f) + (7 - m) W are the DIRECT rows of butterfly W - f, and vice versa: the pair (f, W - f) shares
+        // its eight spectrum rows, which are loaded once (they were loaded twice when every butterfly fetched its own:
+        // 1/8 of the z stage's L1 wavefronts).  Unit 0 is the self-mirrored pair (0, W/2): same code, a select picks its
+        // rows (butterfly 0: rows 0, W, .., 4W, 3W, .., W; butterfly W/2: its own four rows both ways).
+        constexpr int W = NZ >> 3, UNITS = (W / 2) * TY, ITER = (UNITS + NT - 1) / NT, ROW = kchunks<T>::N * TY;
+        const typename kchunks<T>::V* Kcol = Kq + slot;
+#pragma unroll 1
+        for (int k = 0; k < ITER; ++k) {
+            const int t = tid + k * NT;
+            if (UNITS % NT != 0 && t >= UNITS) break;
+            const int ty = t % TY, u = t / TY;
+            const bool self = u == 0;
+            const int fA = u, fB = self ? W / 2 : W - u;
+            KQ<T> KA[4], KB[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { KA[j] = ldk<TY>(Kcol + (fA + j * W) * ROW); KB[j] = ldk<TY>(Kcol + (fB + j * W) * ROW); }
+            const KQ<T> KN = ldk<TY>(Kcol + (self ? 4 * W : fB + 3 * W) * ROW);      // row Nz/2 (unit 0 only; else KB[3] again: a hit)
+            auto ksel = [](bool c, const KQ<T>& x, const KQ<T>& y) {
+                KQ<T> r;
+                r.xx = c ? x.xx : y.xx; r.yy = c ? x.yy : y.yy; r.zz = c ? x.zz : y.zz; r.xy = c ? x.xy : y.xy; r.xz = c ? x.xz : y.xz; r.yz = c ? x.yz : y.yz;
+                return r;
+            };
+            CQ<T> a[3][RF];
+            {   // butterfly A
+                const int p0 = pos_of_freq_rt<LNZ, POL>(fA);
+                load_fwd(a, p0, ty);
+#pragma unroll
+                for (int m = 0; m < 4; ++m) apply_kernel<1>(KA[m], a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+                apply_kernel<0>(ksel(self, KN, KB[3]), a[0][4], a[1][4], a[2][4], self ? (T)1 : (T)-1, (T)sy);
+#pragma unroll
+                for (int m = 5; m < 8; ++m) apply_kernel<-1>(ksel(self, KA[8 - m], KB[7 - m]), a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+                inv_store(a, p0, ty);
+            }
+            {   // butterfly B
+                const int p0 = pos_of_freq_rt<LNZ, POL>(fB);
+                load_fwd(a, p0, ty);
+#pragma unroll
+                for (int m = 0; m < 4; ++m) apply_kernel<1>(KB[m], a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+#pragma unroll
+                for (int m = 4; m < 8; ++m) apply_kernel<-1>(ksel(self, KB[7 - m], KA[7 - m]), a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+                inv_store(a, p0, ty);
+            }
+        }
+    } else {   // fused: last forward pass . multiply . first inverse pass; item = (butterfly i, column ty), 3 components
         constexpr int NBF = NZ >> LRF, TOT = NBF * TY, ITER = (TOT + NT - 1) / NT;
-        const typename kchunks<T>::V* Kq = K + (size_t)(q0 + ql) * g.kst * g.kpz * (kchunks<T>::N * TY);   // KT == TY
 #pragma unroll 1
         for (int k = 0; k < ITER; ++k) {
             const int t = tid + k * NT;
@@ -745,20 +820,10 @@ __global__ void __launch_bounds__(NT, MINB) k_z_v(GeoV g, int q0, int nq, CQ<T>*
             const int ty = t % TY, i = t / TY;
             const int p0 = i << LRF;
             CQ<T> a[3][RF];
-#pragma unroll
-            for (int cc = 0; cc < 3; ++cc) {
-#pragma unroll
-                for (int m = 0; m < RF; ++m) a[cc][m] = ldq(s + tile_addr<PE>(p0, cc * TY + ty) + tile_leg<PE, 1>(m));
-                dftR<LRF, false, false>(a[cc]);
-            }
+            load_fwd(a, p0, ty);
             const int f0 = freq_of_pos_rt<LNZ, POL>(p0);
             MulPoints<T, LNZ, LRF, TY, 0>::run(a, Kq + slot, f0, (T)sy);
-#pragma unroll
-            for (int cc = 0; cc < 3; ++cc) {
-                dftR<LRF, true, false>(a[cc]);
-#pragma unroll
-                for (int m = 0; m < RF; ++m) stq(s + tile_addr<PE>(p0, cc * TY + ty) + tile_leg<PE, 1>(m), a[cc][m]);
-            }
+            inv_store(a, p0, ty);
         }
     }
     __syncthreads();
