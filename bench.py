@@ -474,6 +474,20 @@ def measure(name, steps, warmup, cpu_seconds, with_cufft, with_cpu, env):
     sb = stage_bytes(n, esz)
     names = STAGE_NAMES_FAST if plan.path() == 1 else STAGE_NAMES
     dom = int(np.argmax(st_ms))
+    # the instantiation behind each stage name (kernels_v2.cuh): register-resident z stages for thin meshes, the fused film
+    # stage, the staged persistent kernel for long y lines
+    actual = list(names)
+    if plan.path() == 1:
+        Nz = 1 if n[2] == 1 else 2 * n[2]
+        Ny = 2 * n[1]
+        if n[2] == 1:
+            actual[2] = "k_z_v<FILM> (y FFT . multiply . y IFFT along y)"
+        elif Nz <= 8:
+            actual[2] = "k_z1_v"
+        elif Nz == 16 and not fp64 and Ny % 64 == 0:
+            actual[2] = "k_z16_v"
+        if Ny >= 4096 and n[2] > 1:
+            actual[1] = "k_y_fwd_long_v"
     achieved = sb[dom] / (st_ms[dom] * 1e-3) / 1e9
     value = aggregate_throughput(world, nc, steps, ms_total) / 1e9
     line = {
@@ -493,7 +507,7 @@ def measure(name, steps, warmup, cpu_seconds, with_cufft, with_cpu, env):
         "gpu_launches": launches_per_step * steps,
         "launches_per_step": launches_per_step,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": names[dom], "kernel_instance": actual[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                      "bytes_per_apply_model": sb[dom], "ms_per_apply": float(st_ms[dom]),
                      "launches_per_apply": int(st_n[dom] // reps)},
