@@ -368,12 +368,12 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
     }
     if (p->v2) {
         v2::GeoV gv;
-        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0; gv.pft = 0; gv.onx = nx; gv.ony = ny; gv.onz = nz; gv.kst = (g.Ny / 2 + 1 + v2::z_kt(g.lNz) - 1) / v2::z_kt(g.lNz);
+        gv.nx = nx; gv.ny = ny; gv.nz = nz; gv.Ny = g.Ny; gv.Nz = g.Nz; gv.Lc = nx; gv.hq = nx / 2 + 1; gv.kpz = g.kpz; gv.acc = 0; gv.trig = 0; gv.pf = 0; gv.pft = 0; gv.onx = nx; gv.ony = ny; gv.onz = nz; gv.kst = (g.Ny / 2 + 1 + v2::z_kt(g.lNz, p->esz) - 1) / v2::z_kt(g.lNz, p->esz);
         p->cf.gx = gv; p->cd.gx = gv;
         p->ny_loc = ny; p->nq_loc = gv.hq;
         if (sharded) {
             // rows of M / H (tiles of the x kernels: 2 RP rows) and frequency pairs of this rank
-            demag_status s1 = demag_shard_range(ny, world, rank, 2 * v2::x_rp(g.lLc), &p->y0, &p->ny_loc);
+            demag_status s1 = demag_shard_range(ny, world, rank, 2 * v2::x_rp(g.lLc, p->esz), &p->y0, &p->ny_loc);
             demag_status s2 = s1 ? s1 : demag_shard_range(gv.hq, world, rank, 1, &p->q0, &p->nq_loc);
             if (s2) { delete p; return s2; }
             p->cf.gx.ny = p->cd.gx.ny = p->ny_loc;
@@ -425,7 +425,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         if (sharded) p->w1out_bytes = (size_t)3 * (nx / 2 + 1) * g.nz * p->ny_loc * qsz;
         p->w2_bytes = (size_t)p->nq_auto * per_q;
         p->kpitch_v = gv.kst;
-        p->k_bytes = (size_t)gv.hq * gv.kst * v2::z_kt(g.lNz) * g.kpz * 12 * p->esz;     // y and z packed by symmetry
+        p->k_bytes = (size_t)gv.hq * gv.kst * v2::z_kt(g.lNz, p->esz) * g.kpz * 12 * p->esz;     // y and z packed by symmetry
         if (p->cf.film) { p->w2_bytes = 256; p->k_bytes = (size_t)gv.hq * g.kpy * 12 * p->esz; }
     }
     auto alloc_all = [&]() -> demag_status {
@@ -492,8 +492,8 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                 // x kernels do not gain (R2C) or lose (C2R: one request per 32-256 byte piece)
                 // With a tensor map the whole strided tile is ONE request (profiles/r2_01_prefetch.md): the z kernel then gains
                 // 4 % with narrow rows too (C3, C5), the x C2R kernel 5 % where its pieces are 32-64 bytes (long rows, C4)
-                const bool z_wide = (size_t)v2::z_ty(g.lNz) * 4 * p->esz >= 512, z_tmap = g.nz <= 256 && !getenv("DEMAG_NO_TMAP");
-                int mask = 2 | 8 | (g.lNz >= 4 && (z_wide || z_tmap) ? 4 : 0) | (v2::x_rp(g.lLc) <= 2 && !sharded && !getenv("DEMAG_NO_TMAP") ? 16 : 0);
+                const bool z_wide = (size_t)v2::z_ty(g.lNz, p->esz) * 4 * p->esz >= 512, z_tmap = g.nz <= 256 && !getenv("DEMAG_NO_TMAP");
+                int mask = 2 | 8 | (g.lNz >= 4 && (z_wide || z_tmap) ? 4 : 0) | (v2::x_rp(g.lLc, p->esz) <= 2 && !sharded && !getenv("DEMAG_NO_TMAP") ? 16 : 0);
                 if (const char* e = getenv("DEMAG_PF_MASK")) mask = atoi(e);
                 auto apply_mask = [&](auto& c) {
                     if (!(mask & 1)) c.pf_xf = 0;
@@ -539,7 +539,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
             // tensor maps for the one-request tile prefetch (kernels_v2.cuh pf_l2_tensor); a failure only disables it
             const v2::GeoV& gv = p->cf.g;
             const unsigned long long q = 4 * p->esz;                                   // bytes per quad
-            const int ty = v2::z_ty(g.lNz);
+            const int ty = v2::z_ty(g.lNz, p->esz);
             if (g.lNz >= 4 && g.nz <= 256 && ty * 4 <= 256) {                          // z kernel: box {TY quads, nz, 1, 3}
                 const unsigned long long dim[4] = {(unsigned long long)g.Ny * 4, (unsigned long long)g.nz, (unsigned long long)p->nq_auto, 3};
                 const unsigned long long sb[3] = {g.Ny * q, (unsigned long long)g.nz * g.Ny * q, (unsigned long long)p->nq_auto * g.nz * g.Ny * q};
@@ -549,7 +549,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
                 else if (ty * 4 * p->esz < 512) p->cf.pf_z = p->cd.pf_z = 0;          // no map: narrow rows do not prefetch
             }
             if (!sharded) {                                                             // x C2R: box {2 RP quads, 1, 256 pairs, 1}
-                const int rp = v2::x_rp(g.lLc);
+                const int rp = v2::x_rp(g.lLc, p->esz);
                 const unsigned long long dim[4] = {(unsigned long long)g.ny * 4, (unsigned long long)g.nz, (unsigned long long)gv.hq, 3};
                 const unsigned long long sb[3] = {g.ny * q, (unsigned long long)g.nz * g.ny * q, (unsigned long long)gv.hq * g.nz * g.ny * q};
                 const unsigned box[4] = {(unsigned)(2 * rp * 4), 1, (unsigned)std::min(gv.hq, 256), 1};
@@ -763,9 +763,9 @@ extern "C" demag_status demag_set_kernel(demag_plan_t p, const double* N6_host)
                 const size_t n = (size_t)gv.hq * g.kpz * g.Ny;
                 const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, 1u << 20);
                 if (p->prec == DEMAG_FP32)
-                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->kpitch_v, p->ypos2freq, p->yslot, 0.5 * scale, p->q0);
+                    v2::k_pack_kernel_v<float><<<grid, 256>>>(B3, (float*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz, p->esz), p->kpitch_v, p->ypos2freq, p->yslot, 0.5 * scale, p->q0);
                 else
-                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz), p->kpitch_v, p->ypos2freq, p->yslot, 0.5 * scale, p->q0);
+                    v2::k_pack_kernel_v<double><<<grid, 256>>>(B3, (double*)p->K, c, gv.Lc, gv.hq, g.kpy, g.kpz, g.Ny, v2::z_kt(g.lNz, p->esz), p->kpitch_v, p->ypos2freq, p->yslot, 0.5 * scale, p->q0);
             }
             else if (p->prec == DEMAG_FP32) launch_pack<float>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
             else launch_pack<double>(B3, (char*)p->K + c * p->kcomp_stride * p->esz, g, par[c][1], scale);
@@ -1005,7 +1005,7 @@ void install_peers(demag_plan_s* p, v2::Ctx<T>& c, void* const* in, void* const*
     demag_shard_range(hq, p->world, 0, 1, &b0, &cnt);
     c.m_in.G = p->world; c.m_in.per = cnt; c.m_in.total = hq; c.m_in.off = p->y0; c.m_in.pitch = p->g.ny;
     // y inverse -> W1out of the row's owner: rows per rank, this rank's first pair, pairs = whole hq
-    demag_shard_range(p->g.ny, p->world, 0, 2 * v2::x_rp(p->g.lLc), &b0, &cnt);
+    demag_shard_range(p->g.ny, p->world, 0, 2 * v2::x_rp(p->g.lLc, p->esz), &b0, &cnt);
     c.m_out.G = p->world; c.m_out.per = cnt; c.m_out.total = p->g.ny; c.m_out.off = p->q0; c.m_out.pitch = hq;
     for (int r = 0; r < v2::kMaxRanks; ++r) {
         c.m_in.base[r] = r < p->world ? (v2::CQ<T>*)in[r] : nullptr;

@@ -42,6 +42,14 @@ template <> struct ZCfg<8>  { static constexpr int POL = 1, TY = 4,  NT = 64,  M
 template <> struct ZCfg<9>  { static constexpr int POL = 1, TY = 4,  NT = 128, MINB = 1; };   // 8 . 8 . 8
 template <> struct ZCfg<10> { static constexpr int POL = 1, TY = 2,  NT = 128, MINB = 1; };   // 16 . 8 . 8
 template <> struct ZCfg<11> { static constexpr int POL = 1, TY = 1,  NT = 64,  MINB = 1; };   // 4 . 8 . 8 . 8
+// fp64 (opt-in, DEMAG_PATH=fast): a quad is 32 bytes, so the same tile shapes would take twice the shared memory and halve
+// the resident blocks; tiles of half the width keep the occupancy of the fp32 shapes (C3 fp64: 1.24 -> 1.02 ms; quarter
+// width measured slower for every stage; the generic family, 1.06 ms, stays the default for fp64 plans)
+template <int LLC> struct XCfgD { static constexpr int POL = XCfg<LLC>::POL, RP = (LLC >= 8 && XCfg<LLC>::RP >= 2) ? XCfg<LLC>::RP / 2 : XCfg<LLC>::RP, NT = XCfg<LLC>::NT; };
+template <int LNY> struct YCfgD { static constexpr int POL = YCfg<LNY>::POL, BP = (LNY >= 9 && YCfg<LNY>::BP >= 2) ? YCfg<LNY>::BP / 2 : YCfg<LNY>::BP, NT = YCfg<LNY>::NT; };
+template <int LNZ> struct ZCfgD { static constexpr int POL = ZCfg<LNZ>::POL, TY = (LNZ >= 6 && ZCfg<LNZ>::TY >= 2) ? ZCfg<LNZ>::TY / 2 : ZCfg<LNZ>::TY, NT = ZCfg<LNZ>::NT, MINB = ZCfg<LNZ>::MINB; };
+template <typename F, typename D, typename T> struct CfgSel { using type = F; };
+template <typename F, typename D> struct CfgSel<F, D, double> { using type = D; };
 
 // quads of the y tile (skewed when the schedule has >= 2 passes, kernels_v2.cuh "tile addressing")
 constexpr int y_tile_quads(int LNY, int POL, int BP)
@@ -61,7 +69,7 @@ inline int y_w2_pos_to_tile_pos(int LNY, int POL, int pw)
 }
 constexpr int kXMin = 4, kXMax = 13, kYMin = 4, kYMax = 13, kZMin = 2, kZMax = 11;
 
-inline int x_rp(int lLc)
+inline int x_rp_f(int lLc)
 {
     switch (lLc) { case 10: return XCfg<10>::RP; case 11: return XCfg<11>::RP; case 12: return XCfg<12>::RP; case 13: return XCfg<13>::RP; default: return 8; }
 }
@@ -69,7 +77,8 @@ inline int x_pol(int lLc) { return lLc == 8 ? XCfg<8>::POL : lLc == 12 ? XCfg<12
 inline bool y_has32(int lNy) { return lNy == 9 || lNy == 13; }
 inline int y_pol(int lNy, bool y32 = false) { return y32 && y_has32(lNy) ? 6 : 1; }
 inline int z_pol(int lNz) { return lNz == 4 ? ZCfg<4>::POL : 1; }
-inline int z_ty(int lNz)
+inline int x_rp(int lLc, size_t esz = 4) { const int r = x_rp_f(lLc); return (esz == 8 && lLc >= 8 && r >= 2) ? r / 2 : r; }
+inline int z_ty_f(int lNz)
 {
     switch (lNz) {
     case 0: case 2: case 3: return 1;
@@ -78,6 +87,7 @@ inline int z_ty(int lNz)
     default: return 1 << 30;
     }
 }
+inline int z_ty(int lNz, size_t esz = 4) { const int t = z_ty_f(lNz); return (esz == 8 && lNz >= 6 && t >= 2 && t < (1 << 30)) ? t / 2 : t; }
 
 // Can the fast path run this geometry?  (all axes zero padded, sizes inside the instantiated range, tiles divide)
 inline bool supported(int nx, int ny, int nz, int Nx, int Ny, int Nz, int lLc, int lNy, int lNz, size_t esz, int max_smem)
@@ -85,14 +95,15 @@ inline bool supported(int nx, int ny, int nz, int Nx, int Ny, int Nz, int lLc, i
     const bool film = nz == 1 && Nz == 1;          // a one-cell-thick mesh has no z transform (R6): multiply only
     if (Nx != 2 * nx || Ny != 2 * ny || (Nz != 2 * nz && !film)) return false;
     if (lLc < kXMin || lLc > kXMax || lNy < kYMin || lNy > kYMax || ((lNz < kZMin || lNz > kZMax) && !film)) return false;
-    if (ny % (2 * x_rp(lLc)) != 0) return false;
-    if (lNz >= 4 && Ny % z_ty(lNz) != 0) return false;
+    if (ny % (2 * x_rp(lLc, esz)) != 0) return false;
+    if (lNz >= 4 && Ny % z_ty(lNz, esz) != 0) return false;
     if (lNz < 4 && Ny < 32) return false;
     // shared memory of the y tile (the largest): Ny * (BP|1) quads
-    const int bp = lNy <= 9 ? 8 : lNy == 10 ? 4 : lNy == 11 ? 2 : 1;
+    int bp = lNy <= 9 ? 8 : lNy == 10 ? 4 : lNy == 11 ? 2 : 1;
+    if (esz == 8 && lNy >= 9 && bp >= 2) bp /= 2;
     if ((size_t)y_tile_quads(lNy, y_pol(lNy), bp) * 4 * esz > (size_t)max_smem) return false;
-    if ((size_t)x_tile_quads(lLc, x_pol(lLc), x_rp(lLc)) * 4 * esz > (size_t)max_smem) return false;
-    if (lNz >= 4 && (size_t)z_tile_quads(lNz, z_pol(lNz), z_ty(lNz)) * 4 * esz > (size_t)max_smem) return false;
+    if ((size_t)x_tile_quads(lLc, x_pol(lLc), x_rp(lLc, esz)) * 4 * esz > (size_t)max_smem) return false;
+    if (lNz >= 4 && (size_t)z_tile_quads(lNz, z_pol(lNz), z_ty(lNz, esz)) * 4 * esz > (size_t)max_smem) return false;
     return true;
 }
 
@@ -144,7 +155,7 @@ cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>*
     return cudaSuccess;
 }
 
-inline int z_kt(int lNz) { return lNz >= 4 ? z_ty(lNz) : 32; }     // slot tile = the z kernel's column tile (32: register kernels)
+inline int z_kt(int lNz, size_t esz = 4) { return lNz >= 4 ? z_ty(lNz, esz) : 32; }     // slot tile = the z kernel's column tile (32: register kernels)
 // ---- plan-time pack of the transformed tensor into the pair layout -----------------------------------------
 // A = real 3D transform of one component, [kz'][ky'][kx] (kx = 0..Lc).  Kv[q][slot / KT][kz'][chunk][slot % KT], lines (q, Lc-q)
 // (kernels_v2.cuh "Kv").  ypos2freq[py] = y frequency stored at W2v position py (the y schedule's digit reversal);
@@ -280,7 +291,7 @@ template <typename G> inline G with_pft(G g, bool on) { g.pft = on ? 1 : 0; retu
 
 #define V2_CASE_X(L, KERN, ...)                                                                                     \
     case L: {                                                                                                        \
-        using C = XCfg<L>;                                                                                           \
+        using C = typename CfgSel<XCfg<L>, XCfgD<L>, T>::type;                                                                                           \
         constexpr int smem = x_tile_quads(L, C::POL, C::RP) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) { *err = cudaFuncSetAttribute(KERN<T, L, C::POL, C::RP, C::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
                          *pfd = pf_distance(c.pf_waves, c.sm_count, KERN<T, L, C::POL, C::RP, C::NT>, C::NT, smem); }  \
@@ -368,7 +379,7 @@ bool x_inv_e(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, 
 }
 
 #define V2_CASE_Y(L, KERN, A, B) case L: V2_BODY_Y(L, KERN, A, B)
-#define V2_BODY_Y(L, KERN, A, B) V2_BODY_Y_C(YCfg<L>, L, KERN, A, B)
+#define V2_BODY_Y(L, KERN, A, B) V2_BODY_Y_C(typename CfgSel<YCfg<L> COMMA YCfgD<L> COMMA T>::type, L, KERN, A, B)
 #define V2_BODY_Y_C(CFG, L, KERN, A, B)                                                                             \
     {                                                                                                                \
         using C = CFG;                                                                                               \
@@ -378,7 +389,8 @@ bool x_inv_e(int mode, const Ctx<T>& c, cudaStream_t st, const CQ<T>* W1, T* H, 
         else launch_pdl(c.pdl, KERN<T, L, C::POL, C::BP, C::NT>, (unsigned)((3LL * nq * c.g.nz + C::BP - 1) / C::BP), C::NT, smem, st, with_pf(c.g, *pfd), q0, nq, A, B, c.twy); \
         return true;                                                                                                 \
     }
-#define V2_BODY_YLONG(L) V2_BODY_YLONG_C(YCfg<L>, L)
+#define COMMA ,
+#define V2_BODY_YLONG(L) V2_BODY_YLONG_C(typename CfgSel<YCfg<L> COMMA YCfgD<L> COMMA T>::type, L)
 #define V2_BODY_YLONG_C(CFG, L)                                                                                     \
     {                                                                                                                \
         using C = CFG;                                                                                               \
@@ -425,7 +437,7 @@ bool y_inv(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const CQ<
 }
 
 // several GPUs: the cropped rows stored at the ranks that own them (k_y_inv_sh_v)
-#define V2_CASE_YSH(L) case L: V2_BODY_YSH_C(YCfg<L>, L)
+#define V2_CASE_YSH(L) case L: V2_BODY_YSH_C(typename CfgSel<YCfg<L> COMMA YCfgD<L> COMMA T>::type, L)
 #define V2_BODY_YSH_C(CFG, L)                                                                                       \
     {                                                                                                                \
         using C = CFG;                                                                                               \
@@ -451,7 +463,7 @@ bool y_inv_sh(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, const 
 
 #define V2_CASE_Z(L)                                                                                                \
     case L: {                                                                                                        \
-        using C = ZCfg<L>;                                                                                           \
+        using C = typename CfgSel<ZCfg<L>, ZCfgD<L>, T>::type;                                                                                           \
         constexpr int smem = z_tile_quads(L, C::POL, C::TY) * (int)sizeof(CQ<T>);                                    \
         if (mode == 0) { *err = cudaFuncSetAttribute(k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
                          c.pf_z = pf_distance(c.pf_waves, c.sm_count, k_z_v<T, L, C::POL, C::TY, C::NT, C::MINB>, C::NT, smem); } \
