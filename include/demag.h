@@ -128,6 +128,23 @@ demag_status demag_apply_atomistic(demag_plan_t plan, const void* S_dev, void* H
  * demag_workspace_bytes from then on).  Idempotent; synchronous (cudaMalloc); DEMAG_ERR_ALLOC if out of memory. */
 demag_status demag_atomistic_reserve(demag_plan_t plan);
 
+/* demag_apply_atomistic for callers that cannot call cudaMalloc at all (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it): the same three steps (Eq. (9) average, the plan's convolution, scatter), with
+ * the two macrocell arrays taken from one file-scope device array of DEMAG_STATIC_SCRATCH_BYTES inside the library instead of
+ * from demag_atomistic_reserve.  Same arguments, same result bit for bit.  It calls no cudaMalloc / cudaFree / allocating
+ * routine; its first call on a device resolves the array's device address (cudaGetSymbolAddress, no allocation).
+ *   - Limit: 2 * 3 * nx*ny*nz reals (each half rounded up to 256 bytes) must fit: at most 699,050 cells in fp32, 349,525 in
+ *     fp64; larger meshes return DEMAG_ERR_UNSUPPORTED (use demag_atomistic_reserve + demag_apply_atomistic).
+ *   - Every GPU that loads the library holds the array until the process exits.
+ *   - All calls of all plans share the array, which keeps the last call's contents (nothing in it needs clearing: both halves
+ *     are fully overwritten before they are read).  Calls that OVERLAP on the GPU (different streams or threads) race on it:
+ *     serialise them on one stream. */
+#define DEMAG_STATIC_SCRATCH_BYTES (16u << 20)
+demag_status demag_apply_atomistic_static(demag_plan_t plan, const void* S_dev, void* Hs_dev,
+                                          int cx, int cy, int cz, double mu_s_in_muB, double a,
+                                          int accumulate, void* cuda_stream);
+size_t demag_static_scratch_bytes(void);      /* = DEMAG_STATIC_SCRATCH_BYTES of the loaded library */
+
 /* Copy back the REAL-SPACE tensor the plan was given or built: double[6][nz][ny][nx] (host).
  * For builder-vs-oracle parity tests.  Synchronous. */
 demag_status demag_get_kernel_real(demag_plan_t plan, double* N6_host);

@@ -25,6 +25,7 @@ EXPORTS = ["demag_plan_create", "demag_set_kernel", "demag_apply", "demag_energy
            "demag_shard_range", "demag_plan_create_sharded", "demag_shard_info", "demag_shard_buffers",
            "demag_shard_ipc_export", "demag_shard_ipc_connect", "demag_shard_set_peers", "demag_apply_sharded",
            "demag_set_pbc_images", "demag_extrapolate", "demag_atomistic_reserve",
+           "demag_apply_atomistic_static", "demag_static_scratch_bytes",
            "demag_plan_dims", "demag_llg_create", "demag_llg_set_field", "demag_llg_step", "demag_llg_mean",
            "demag_llg_counts", "demag_llg_reset", "demag_llg_destroy"]
 
@@ -61,6 +62,9 @@ def lib():
         L.demag_apply_profiled.argtypes = [vp, vp, vp, vp, vp, vp]
         L.demag_apply_atomistic.argtypes = [vp, vp, vp, i, i, i, d, d, i, vp]
         L.demag_atomistic_reserve.argtypes = [vp]
+        L.demag_apply_atomistic_static.argtypes = [vp, vp, vp, i, i, i, d, d, i, vp]
+        L.demag_static_scratch_bytes.argtypes = []
+        L.demag_static_scratch_bytes.restype = ctypes.c_size_t
         L.demag_plan_dims.argtypes = [vp, vp, vp, vp, vp]
         L.demag_llg_create.argtypes = [ctypes.POINTER(vp), vp, d, d, d]
         L.demag_llg_set_field.argtypes = [vp, d, d, d]
@@ -90,7 +94,7 @@ def lib():
         L.demag_shard_set_peers.argtypes = [vp, vp, vp]
         L.demag_apply_sharded.argtypes = [vp, i, vp, vp, vp]
         for name in EXPORTS:
-            if name not in ("demag_workspace_bytes", "demag_launches_per_apply", "demag_last_error"):
+            if name not in ("demag_workspace_bytes", "demag_launches_per_apply", "demag_last_error", "demag_static_scratch_bytes"):
                 getattr(L, name).restype = i
         _lib = L
     return _lib
@@ -155,6 +159,16 @@ def demag_energy(plan, M, H, E, stream=None):
 def demag_apply_atomistic(plan, S, Hs, c, mu_s, a, accumulate=False, stream=None):
     _check(lib().demag_apply_atomistic(plan, S.data_ptr(), Hs.data_ptr(), int(c[0]), int(c[1]), int(c[2]),
                                        float(mu_s), float(a), int(bool(accumulate)), _stream(stream)))
+
+
+def demag_apply_atomistic_static(plan, S, Hs, c, mu_s, a, accumulate=False, stream=None):
+    """demag_apply_atomistic with the macrocell arrays in the library's fixed static device array: allocates nothing."""
+    _check(lib().demag_apply_atomistic_static(plan, S.data_ptr(), Hs.data_ptr(), int(c[0]), int(c[1]), int(c[2]),
+                                              float(mu_s), float(a), int(bool(accumulate)), _stream(stream)))
+
+
+def demag_static_scratch_bytes() -> int:
+    return int(lib().demag_static_scratch_bytes())
 
 
 def demag_atomistic_reserve(plan):
@@ -366,6 +380,9 @@ class Plan:
 
     def apply_atomistic(self, S, Hs, c, mu_s, a, accumulate=False, stream=None):
         demag_apply_atomistic(self.handle, S, Hs, c, mu_s, a, accumulate, stream)
+
+    def apply_atomistic_static(self, S, Hs, c, mu_s, a, accumulate=False, stream=None):
+        demag_apply_atomistic_static(self.handle, S, Hs, c, mu_s, a, accumulate, stream)
 
     def get_kernel_real(self):
         return demag_get_kernel_real(self.handle, self.n)

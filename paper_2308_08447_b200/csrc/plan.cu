@@ -1249,3 +1249,87 @@ extern "C" demag_status demag_apply_atomistic(demag_plan_t p, const void* S_dev,
     CUDA_TRY(cudaGetLastError());
     return DEMAG_OK;
 }
+
+// ================================================================================ no-allocation atomistic entry point
+// For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it):
+// demag_apply_atomistic with its two macrocell arrays (M and H on the plan's mesh, the scratch that
+// demag_atomistic_reserve would allocate) taken from ONE file-scope device array of fixed size instead.
+//   * Every GPU that loads this library holds the DEMAG_STATIC_SCRATCH_BYTES (16 MiB) of the array until the process exits.
+//   * In host code `g_static_scratch` is only a stand-in for the symbol, NOT a device address: its device address is
+//     resolved with cudaGetSymbolAddress once per device (with that device current) and cached; kernels get that pointer.
+//   * All calls share the array and it keeps the last call's contents.  Nothing in it has to start at zero: the
+//     average kernel writes every cell of M and the convolution writes every cell of H before the scatter reads it.
+//   * Calls that overlap on the GPU (two streams, two plans, two threads) race on the array: serialise them.
+namespace {
+constexpr size_t kStaticScratchBytes = DEMAG_STATIC_SCRATCH_BYTES;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+constexpr int kMaxDevices = 64;
+void* g_static_scratch_addr[kMaxDevices] = {};     // device address of g_static_scratch on each device (NULL: not resolved yet)
+
+demag_status static_scratch_ptr(int device, void** out)
+{
+    if (device < 0 || device >= kMaxDevices) return fail(DEMAG_ERR_UNSUPPORTED, "device %d: the static scratch serves devices 0..%d", device, kMaxDevices - 1);
+    void* q = __atomic_load_n(&g_static_scratch_addr[device], __ATOMIC_ACQUIRE);
+    if (!q) {      // set-up, once per device, with that device current (the caller checked): no allocation involved
+        cudaError_t e = cudaGetSymbolAddress(&q, g_static_scratch);
+        if (e != cudaSuccess || !q) return fail(DEMAG_ERR_CUDA, "cudaGetSymbolAddress(static scratch): %s", cudaGetErrorString(e));
+        __atomic_store_n(&g_static_scratch_addr[device], q, __ATOMIC_RELEASE);
+    }
+    *out = q;
+    return DEMAG_OK;
+}
+}  // namespace
+
+extern "C" size_t demag_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+extern "C" demag_status demag_apply_atomistic_static(demag_plan_t p, const void* S_dev, void* Hs_dev, int cx, int cy, int cz,
+                                                     double mu_s_in_muB, double a, int accumulate, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!p) return fail(DEMAG_ERR_INVALID_ARG, "plan is NULL");
+    if (cx < 1 || cy < 1 || cz < 1 || !(a > 0) || !isfinite(mu_s_in_muB))
+        return fail(DEMAG_ERR_INVALID_ARG, "bad macrocell / lattice arguments");
+    struct { int nx, ny, nz; } g = {p->on[0], p->on[1], p->on[2]};     // the caller's macrocell mesh
+    const double want[3] = {cx * a, cy * a, cz * a};
+    for (int i = 0; i < 3; ++i)
+        if (fabs(want[i] - p->h[i]) > 1e-9 * p->h[i])
+            return fail(DEMAG_ERR_INVALID_ARG, "plan cell size must equal macrocell size c*a (axis %d)", i);
+    const size_t nc = (size_t)g.nx * g.ny * g.nz;
+    const size_t half = (3 * nc * p->esz + 255) / 256 * 256;          // M at offset 0, H at offset `half`
+    if (2 * half > kStaticScratchBytes)
+        return fail(DEMAG_ERR_UNSUPPORTED, "mesh %d x %d x %d needs %zu bytes of macrocell scratch, the static array holds %zu "
+                    "(at most %zu cells in this precision): use demag_atomistic_reserve + demag_apply_atomistic",
+                    g.nx, g.ny, g.nz, 2 * half, kStaticScratchBytes, kStaticScratchBytes / (6 * p->esz));
+    const size_t nspin3 = (size_t)3 * g.nx * cx * g.ny * cy * g.nz * cz;
+    demag_status s = check_apply_args(p, S_dev, Hs_dev, nspin3 * p->esz);      // incl. "the plan's device is the current device"
+    if (s) return s;
+    if (!p->has_kernel) return fail(DEMAG_ERR_NO_KERNEL, "demag_set_kernel has not been called");
+    void* base = nullptr;
+    if ((s = static_scratch_ptr(p->device, &base))) return s;
+    void* Mc = base;
+    void* Hc = (unsigned char*)base + half;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const double muB = 9.2740100783e-24;
+    const double f = muB * mu_s_in_muB / ((double)cx * cy * cz * a * a * a);
+    const unsigned ga = (unsigned)std::min<size_t>((3 * nc + 255) / 256, (size_t)1 << 22);
+    const unsigned gs = (unsigned)std::min<size_t>((nspin3 / 4 + 255) / 256 + 1, (size_t)p->sm_count * 32);
+    if (p->prec == DEMAG_FP32 && cx == 4 && g.ny <= 65535 && 3 * g.nz <= 65535) {
+        const dim3 g3((unsigned)((g.nx + 127) / 128), (unsigned)g.ny, (unsigned)(3 * g.nz));
+        k_macro_avg_x4<<<g3, 128, 0, st>>>(g.nx, cy, cz, (const float*)S_dev, (float*)Mc, f);
+        s = apply_outer<float>(p, (const float*)Mc, (float*)Hc, st);
+        if (s) return s;
+        k_macro_scatter_x4<<<g3, 128, 0, st>>>(g.nx, cy, cz, (const float*)Hc, (float*)Hs_dev, accumulate);
+    } else if (p->prec == DEMAG_FP32) {
+        k_macro_avg<float><<<ga, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const float*)S_dev, (float*)Mc, f);
+        s = apply_outer<float>(p, (const float*)Mc, (float*)Hc, st);
+        if (s) return s;
+        k_macro_scatter<float><<<gs, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const float*)Hc, (float*)Hs_dev, accumulate);
+    } else {
+        k_macro_avg<double><<<ga, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const double*)S_dev, (double*)Mc, f);
+        s = apply_outer<double>(p, (const double*)Mc, (double*)Hc, st);
+        if (s) return s;
+        k_macro_scatter<double><<<gs, 256, 0, st>>>(g.nx, g.ny, g.nz, cx, cy, cz, (const double*)Hc, (double*)Hs_dev, accumulate);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return DEMAG_OK;
+}
