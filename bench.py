@@ -50,6 +50,9 @@ def parse():
     ap.add_argument("--virtual-ranks", type=int, default=0,
                     help="with --sharded on ONE GPU: emulate G ranks as G plans on this device, phase by phase, and "
                          "report the per-rank device time of each phase (a compute-share model, no NVLink involved)")
+    ap.add_argument("--llg", action="store_true",
+                    help="time the minimal LLG RK4 integrator (demag_llg_*, PAPER.md:91-96) on --config (default C3): ms per "
+                         "step with the demagnetizing field convolved at every stage vs extrapolated at the sub-steps")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     return ap.parse_args()
 
@@ -734,6 +737,52 @@ def run_sharded(args, cfg, fp64):
         dist.destroy_process_group()
 
 
+def run_llg(args, cfg, fp64):
+    """The consumer of the convolution: K RK4 steps of the LLG equation with H_eff = H_d + H_Zee,
+    once with H_d convolved at all four stages, once with the sub-step fields extrapolated from the five last full-step
+    fields.  Device time by CUDA events around the K steps; reports the convolution counts."""
+    import torch
+    from paper_2308_08447_b200 import binding as B
+    B.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    if cfg.kind == "atomistic":
+        raise SystemExit("--llg: mesh workloads only (C1-C4)")
+    dt = torch.float64 if fp64 else torch.float32
+    n = cfg.n
+    nc = int(np.prod(n))
+    M0 = torch.from_numpy(W.make_magnetisation(cfg)).to("cuda", dt)
+    out = {}
+    with B.Plan(n, cfg.h, 0, B.DEMAG_FP64 if fp64 else B.DEMAG_FP32) as plan:
+        plan.set_kernel(None)
+        for name, extrap in (("every_stage", False), ("extrapolated", True)):
+            with B.LLG(plan, cfg.Ms, 0.02) as L:
+                L.set_field((-2.0e4, 1.0e3, 0.0))                      # the switching field of PAPER.md:47
+                M = M0.clone()
+                for _ in range(max(5, args.warmup)):                   # >= 5 steps: the history of the quartic is full
+                    L.step(M, 1.0e-13, extrap)
+                c0 = L.counts()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                a.record()
+                for _ in range(args.steps):
+                    L.step(M, 1.0e-13, extrap)
+                b.record(); torch.cuda.synchronize()
+                c1 = L.counts()
+                assert bool(torch.isfinite(M).all())
+                out[name] = {"ms_per_rk4_step": a.elapsed_time(b) / args.steps,
+                             "convolutions_per_step": (c1["convolutions"] - c0["convolutions"]) / args.steps,
+                             "extrapolation_passes_per_step": (c1["extrapolations"] - c0["extrapolations"]) / args.steps}
+    line = {"metric": "llg_rk4_step_ms", "unit": "ms", "n_gpus": 1, "steps": args.steps, "warmup": max(5, args.warmup),
+            "dtype": "f64" if fp64 else "f32", "data": "synthetic", "config": config_of(cfg, fp64),
+            "every_stage": out["every_stage"], "extrapolated": out["extrapolated"],
+            "speedup": out["every_stage"]["ms_per_rk4_step"] / out["extrapolated"]["ms_per_rk4_step"],
+            "Mcell_steps_per_s_extrapolated": nc / out["extrapolated"]["ms_per_rk4_step"] / 1e3,
+            "note": "H_eff = H_d + uniform field only; L2 not flushed (back-to-back steps of one integrator); PAPER.md:96 quotes a "
+                    "decrease of the demagnetizing time 'by a factor between 2 to 2.5' for this scheme"}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
     name = args.config or HEADLINE
@@ -741,6 +790,8 @@ def main():
     cfg = W.CONFIGS[name[:2]]
     if args.impl == "reference":
         run_reference(args, cfg, fp64)
+    elif args.llg:
+        run_llg(args, W.CONFIGS[(args.config or "C3")[:2]], (args.config or "C3").endswith("d"))
     elif args.sharded and args.virtual_ranks > 0:
         run_virtual_ranks(args, cfg, fp64)
     elif args.sharded:
