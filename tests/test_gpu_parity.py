@@ -151,7 +151,8 @@ def test_linearity(torch, B, oracle):
 
 
 # --------------------------------------------------------------------------------- general mesh sizes
-GENERAL = [(12, 10, 3), (7, 1, 1), (1, 9, 5), (48, 48, 1), (33, 17, 9), (100, 36, 5), (65, 16, 2)]
+GENERAL = [(12, 10, 3), (7, 1, 1), (1, 9, 5), (48, 48, 1), (33, 17, 9), (100, 36, 5), (65, 16, 2),
+           (130, 70, 3), (18, 130, 6), (1030, 18, 2), (480, 30, 2)]     # even nx on the fast path: zeros / crop inside the x kernels
 
 
 @pytest.mark.parametrize("n", GENERAL)
@@ -526,7 +527,8 @@ def _margins_intact(torch, buf, nel):
     return bool((buf[:GUARD] == s).all()) and bool((buf[GUARD + nel:] == s).all())
 
 
-@pytest.mark.parametrize("n", [(64, 64, 8), (16, 32, 16), (32, 16, 1), (256, 32, 1), (4, 128, 8), (24, 10, 6), (1, 1, 64)])
+@pytest.mark.parametrize("n", [(64, 64, 8), (16, 32, 16), (32, 16, 1), (256, 32, 1), (4, 128, 8), (24, 10, 6), (1, 1, 64),
+                               (130, 70, 3), (1030, 18, 2)])
 @pytest.mark.parametrize("prec", [0, 1])
 def test_apply_writes_exactly_H_and_leaves_M_untouched(torch, B, oracle, n, prec):
     """demag_apply / demag_apply_add / demag_energy on caller arrays surrounded by sentinel margins: every element of
