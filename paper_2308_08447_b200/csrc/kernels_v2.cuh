@@ -946,6 +946,157 @@ __global__ void __launch_bounds__(128, MINB) k_z16_v(GeoV g, int q0, int nq, CQ<
     pdl_leave(g);
 }
 
+// Nz = 256 / 512 (fp32): the zero-padded z transform as TWO independent half-length transforms of the same nz inputs
+// (decimation in frequency with a zero upper half, as in k_z16_v):
+//     M^[2k]   = DFT_{Nz/2}(m[z])[k]                 "E" tile,   M^[2k+1] = DFT_{Nz/2}(m[z] w_Nz^z)[k]      "O" tile,
+// and the cropped inverse  h[z] = IDFT_{Nz/2}(H^_even)[z] + conj(w_Nz^z) IDFT_{Nz/2}(H^_odd)[z],  z < nz.
+// A half-length transform is TWO passes, radix Nz/16 (16 or 32, straight from / to global memory, in registers) and
+// radix 8 (the fused pass: last forward . multiply . first inverse), where the padded length needs three (4.8.8 / 8.8.8):
+// every point of the tile is written and read twice instead of four times.  The shared-memory traffic is what bounds the
+// z stage of long columns (C5: 68 % of the L1 data pipe with the three-pass kernel).
+// Lanes 0-15 / 16-31 of a warp are the E / O halves of the same 16 (butterfly, line) items: they load the same addresses
+// and exchange their halves of the inverse by one shuffle per value.  The fused pass is the paired one of k_z_v:
+// butterfly f = 2 d + parity of tile (E / O) position 8 d holds kz = f + m Nz/8.
+template <typename T, int LNZ, int TY, int NT>
+__global__ void __launch_bounds__(NT, 1) k_z_eo_v(GeoV g, int q0, int nq, CQ<T>* W2, const typename kchunks<T>::V* __restrict__ K,
+                                                 const int* __restrict__ yslot, TwSet<T> tw, const CQ<T>* __restrict__ two,
+                                                 const __grid_constant__ CUtensorMap tmap)
+{
+    pdl_enter(g);
+    constexpr int NZ = 1 << LNZ, LNH = LNZ - 1, NH = 1 << LNH, B = 3 * TY;
+    constexpr int LR1 = LNH - 3, R1 = 1 << LR1, S1 = 8, RF = 8;          // make_sched(LNH, 7): R1 . 8
+    constexpr int PE = tile_pe(B, 0);
+    constexpr int OPAD = TY;         // quads of padding in front of the O tile: in the fused pass a quarter-warp holds one E and one
+                                     // O butterfly (TY quads each); without it both fall into the same banks (NH * B * 16 B = 0 mod 128)
+    constexpr int NPAIR = S1 * B, PER_ROUND = NT / 2;
+    static_assert(NPAIR % 16 == 0 && NT % 32 == 0 && NT % TY == 0 && TY >= 4, "k_z_eo_v: tile shape");
+    CQ<T>* s = reinterpret_cast<CQ<T>*>(smem_v2);                        // E tile: points [0, NH), O tile: [NH, 2 NH)
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const bool odd = lane >= 16;
+    const int tilesY = g.Ny / TY;
+    const int pyt = blockIdx.x % tilesY, ql = blockIdx.x / tilesY;
+    const int py0 = pyt * TY;
+    const size_t cstride = (size_t)nq * g.nz * g.Ny;
+    CQ<T>* base = W2 + (size_t)ql * g.nz * g.Ny + py0;
+    const int Ny = g.Ny;
+    if (g.pf && blockIdx.x + g.pf < gridDim.x) {                         // next tile's field rows and spectrum rows into L2
+        const int bn = blockIdx.x + g.pf, pytn = bn % tilesY, qln = bn / tilesY;
+        const CQ<T>* bnx = W2 + (size_t)qln * g.nz * g.Ny + pytn * TY;
+        if (g.pft) { if (tid == 0) pf_l2_tensor(&tmap, pytn * TY * 4, 0, qln, 0); }
+        else for (int r = tid; r < 3 * g.nz; r += NT) { const int c = r / g.nz, z = r - c * g.nz; pf_l2_span(bnx + c * cstride + (size_t)z * Ny, (uint32_t)(TY * sizeof(CQ<T>))); }
+        if (tid >= NT - 2) {
+            const int sl = __ldg(yslot + pytn * TY + (tid == NT - 1 ? TY - 1 : 0)) & 0x7fffffff;
+            const uint32_t kb = (uint32_t)(g.kpz * kchunks<T>::N * TY * sizeof(typename kchunks<T>::V));
+            pf_l2_bulk(K + ((size_t)(q0 + qln) * g.kst + sl / TY) * g.kpz * (kchunks<T>::N * TY), kb);
+        }
+    }
+    float sy;
+    const size_t slot = kslot<TY, kchunks<T>::N>(yslot, py0 + tid % TY, g.kpz, sy);
+    const CQ<T>* tab = tw.p[0];                                          // w_NH^(i m), [(m - 1) * 8 + i]
+    // ---- first pass of both half transforms, inputs straight from global (all nz = NH of them: nothing is padded here)
+    for (int qb = wid * 16; qb < NPAIR; qb += PER_ROUND) {
+        const int q = qb + (lane & 15), b = q % B, i = q / B;
+        const int c = b / TY, ty = b - c * TY;
+        const CQ<T>* col = base + c * cstride + ty;
+        CQ<T> a[R1];
+#pragma unroll
+        for (int r = 0; r < R1; ++r) a[r] = ldsq(col + (size_t)(i + S1 * r) * Ny);
+        if (odd) {
+#pragma unroll
+            for (int r = 0; r < R1; ++r) a[r] = cmul(a[r], ldgq(two + i + S1 * r));
+        }
+        dftR<LR1, false, false>(a);
+        CQ<T>* d = s + tile_addr<PE>((odd ? NH : 0) + i, b) + (odd ? OPAD : 0);
+        stq(d, a[0]);
+#pragma unroll
+        for (int m = 1; m < R1; ++m) stq(d + tile_leg<PE, S1>(m), cmul(a[m], ldgq(tab + ((m - 1) << 3) + i)));
+    }
+    __syncthreads();
+    {   // ---- fused pass (k_z_v's paired form): unit u = butterflies (u, W - u), unit 0 = (0, W/2)
+        constexpr int W = NZ >> 3, UNITS = (W / 2) * TY, ROW = kchunks<T>::N * TY;
+        const typename kchunks<T>::V* Kcol = K + (size_t)(q0 + ql) * g.kst * g.kpz * (kchunks<T>::N * TY) + slot;
+        auto pos_of = [](int f) { return (f & 1) * NH + (f >> 1) * 8; };
+        auto pad_of = [](int p0) { return p0 >= NH ? OPAD : 0; };
+        auto load_fwd = [&](CQ<T> (*a)[RF], int p0, int ty) {
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+#pragma unroll
+                for (int m = 0; m < RF; ++m) a[cc][m] = ldq(s + tile_addr<PE>(p0, cc * TY + ty) + pad_of(p0) + tile_leg<PE, 1>(m));
+                dftR<3, false, false>(a[cc]);
+            }
+        };
+        auto inv_store = [&](CQ<T> (*a)[RF], int p0, int ty) {
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+                dftR<3, true, false>(a[cc]);
+#pragma unroll
+                for (int m = 0; m < RF; ++m) stq(s + tile_addr<PE>(p0, cc * TY + ty) + pad_of(p0) + tile_leg<PE, 1>(m), a[cc][m]);
+            }
+        };
+        auto ksel = [](bool c, const KQ<T>& x, const KQ<T>& y) {
+            KQ<T> r;
+            r.xx = c ? x.xx : y.xx; r.yy = c ? x.yy : y.yy; r.zz = c ? x.zz : y.zz; r.xy = c ? x.xy : y.xy; r.xz = c ? x.xz : y.xz; r.yz = c ? x.yz : y.yz;
+            return r;
+        };
+#pragma unroll 1
+        for (int t = tid; t < UNITS; t += NT) {
+            const int ty = t % TY, u = t / TY;
+            const bool self = u == 0;
+            const int fA = u, fB = self ? W / 2 : W - u;
+            KQ<T> KA[4], KB[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { KA[j] = ldk<TY>(Kcol + (fA + j * W) * ROW); KB[j] = ldk<TY>(Kcol + (fB + j * W) * ROW); }
+            const KQ<T> KN = ldk<TY>(Kcol + (self ? 4 * W : fB + 3 * W) * ROW);
+            CQ<T> a[3][RF];
+            {
+                const int p0 = pos_of(fA);
+                load_fwd(a, p0, ty);
+#pragma unroll
+                for (int m = 0; m < 4; ++m) apply_kernel<1>(KA[m], a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+                apply_kernel<0>(ksel(self, KN, KB[3]), a[0][4], a[1][4], a[2][4], self ? (T)1 : (T)-1, (T)sy);
+#pragma unroll
+                for (int m = 5; m < 8; ++m) apply_kernel<-1>(ksel(self, KA[8 - m], KB[7 - m]), a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+                inv_store(a, p0, ty);
+            }
+            {
+                const int p0 = pos_of(fB);
+                load_fwd(a, p0, ty);
+#pragma unroll
+                for (int m = 0; m < 4; ++m) apply_kernel<1>(KB[m], a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+#pragma unroll
+                for (int m = 4; m < 8; ++m) apply_kernel<-1>(ksel(self, KB[7 - m], KA[7 - m]), a[0][m], a[1][m], a[2][m], (T)1, (T)sy);
+                inv_store(a, p0, ty);
+            }
+        }
+    }
+    __syncthreads();
+    // ---- last pass of both half inverses; the E lane finishes z = i + 8 r for r < R1/2, the O lane for r >= R1/2
+    for (int qb = wid * 16; qb < NPAIR; qb += PER_ROUND) {
+        const int q = qb + (lane & 15), b = q % B, i = q / B;
+        const int c = b / TY, ty = b - c * TY;
+        CQ<T>* col = base + c * cstride + ty;
+        const CQ<T>* d = s + tile_addr<PE>((odd ? NH : 0) + i, b) + (odd ? OPAD : 0);
+        CQ<T> a[R1];
+        a[0] = ldq(d);
+#pragma unroll
+        for (int m = 1; m < R1; ++m) a[m] = cmulc(ldq(d + tile_leg<PE, S1>(m)), ldgq(tab + ((m - 1) << 3) + i));
+        dftR<LR1, true, false>(a);
+        if (odd) {
+#pragma unroll
+            for (int r = 0; r < R1; ++r) a[r] = cmulc(a[r], ldgq(two + i + S1 * r));
+        }
+#pragma unroll
+        for (int j = 0; j < R1 / 2; ++j) {
+            const CQ<T> give = odd ? a[j] : a[j + R1 / 2], keep = odd ? a[j + R1 / 2] : a[j];
+            CQ<T> got;
+            got.re.x = __shfl_xor_sync(0xffffffffu, give.re.x, 16); got.re.y = __shfl_xor_sync(0xffffffffu, give.re.y, 16);
+            got.im.x = __shfl_xor_sync(0xffffffffu, give.im.x, 16); got.im.y = __shfl_xor_sync(0xffffffffu, give.im.y, 16);
+            stq(col + (size_t)(i + S1 * (j + (odd ? R1 / 2 : 0))) * Ny, cadd(keep, got));
+        }
+    }
+    pdl_leave(g);
+}
+
 // =========================================================================================== K1v / K5v: x stage
 // A tile = RP pairs of consecutive y rows of one (component, z); the two rows of a pair are the two lines of a quad.
 // The real rows are transformed as packed complex sequences z[m] = x[2m] + i x[2m+1] of length Lc (upper half

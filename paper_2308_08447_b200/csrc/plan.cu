@@ -396,6 +396,7 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
         p->cf.sm_count = p->cd.sm_count = p->sm_count;
         p->cf.ylong = p->cd.ylong = getenv("DEMAG_NO_YLONG") == nullptr;
         p->cf.z16 = precision == DEMAG_FP32 && getenv("DEMAG_NO_Z16") == nullptr ? (getenv("DEMAG_Z16_MINB3") ? 1 : 2) : 0;   // 2 blocks x 255 registers measured 3 % faster than 3 x 168
+        p->cf.zeo = precision == DEMAG_FP32 && (g.lNz == 8 || g.lNz == 9) && g.Nz == 2 * nz && getenv("DEMAG_NO_ZEO") == nullptr;   // Nz = 128: measured slower (211 vs 150 us at C3: no pass saved there)
         p->cf.y32 = precision == DEMAG_FP32 && getenv("DEMAG_NO_Y32") == nullptr;
         {   // L2 prefetch of the tile that starts when the current one ends (kernels_v2.cuh pf_l2_*), in waves of
             // co-resident blocks; 0 = off
@@ -447,6 +448,9 @@ static demag_status plan_create_impl(demag_plan_t* out, int nx, int ny, int nz, 
             cudaError_t verr = cudaSuccess;
             if (precision == DEMAG_FP32) {
                 for (int a = 0; a < 3; ++a) {
+                    if (a == 2 && p->cf.zeo)      // k_z_eo_v: tables of the HALF-length schedule (radix Nz/16, then 8) + w_Nz^z
+                        CUDA_TRY(v2::build_axis_tables<float>(g.lNz - 1, 7, 0, &p->tf[a], nullptr, g.Nz, &p->cf.two));
+                    else
                     CUDA_TRY(v2::build_axis_tables<float>(LL[a], POL[a], a == 0 ? nx : 0, &p->tf[a], a == 0 ? &p->cf.twpost : nullptr));
                     p->tw_bytes += p->tf[a].bytes;
                 }

@@ -261,6 +261,7 @@ template <int LR, bool INV, bool HALF_IN, typename T> DM_HD void dftR(CQ<T>* a)
 //   POL 2: as many radix-16 as the remainder allows: LL%3==1 -> 16,8,..; LL%3==2 -> 16,16,8,.. (LL >= 8)
 //   POL 3: radix 8 passes, remainder, radix 4 LAST (LL >= 4)
 //   POL 5: radix 16 passes, remainder LAST
+//   POL 7: two passes, radix 2^(LL-3) then radix 8 (LL = 7, 8)
 //   POL 6: radix 16 passes, remainder, and a radix-32 LAST pass (LL >= 8; the y stage: the last forward / first
 //          inverse pass runs straight against global memory, so 512 = 16 . 32 sweeps the tile once each way)
 struct Sched {
@@ -278,6 +279,8 @@ DM_HDC Sched make_sched(int LL, int POL)
     } else if (POL == 5) {          // radix 16 passes, remainder LAST (long x rows: fewest sweeps)
         while (rem >= 4) { s.lr[s.n++] = 4; rem -= 4; }
         if (rem) s.lr[s.n++] = rem;
+    } else if (POL == 7) {          // two passes: radix 2^(LL-3), then radix 8 (the even / odd half transforms of k_z_eo_v)
+        s.lr[s.n++] = LL - 3; s.lr[s.n++] = 3;
     } else if (POL == 6) {          // radix 16 passes, remainder, and a radix-32 LAST pass
         rem -= 5;
         while (rem >= 4) { s.lr[s.n++] = 4; rem -= 4; }

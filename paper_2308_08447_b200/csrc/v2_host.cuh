@@ -117,7 +117,8 @@ struct AxisTables {
     TwSet<T> set;
 };
 template <typename T>
-cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>* out, const CQ<T>** post)
+cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>* out, const CQ<T>** post,
+                              int eo_N = 0, const CQ<T>** eo = nullptr)
 {
     const Sched sc = make_sched(LL, POL);
     std::vector<T> h;
@@ -144,6 +145,15 @@ cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>*
             h.push_back(wr); h.push_back(wr); h.push_back(wi); h.push_back(wi);
         }
     }
+    size_t eo_off = h.size();
+    if (eo_N > 0) {              // w_N^z = exp(-2 pi i z / N), z = 0..N/2-1 (the odd half transform of k_z_eo_v)
+        for (int z = 0; z < eo_N / 2; ++z) {
+            const long double a = tp * (long double)z / (long double)eo_N;
+            T wr = (T)cosl(a), wi = (T)(-sinl(a));
+            if (4 * z == eo_N) { wr = 0; wi = -1; }
+            h.push_back(wr); h.push_back(wr); h.push_back(wi); h.push_back(wi);
+        }
+    }
     if (h.empty()) h.resize(4, (T)0);
     out->bytes = h.size() * sizeof(T);
     cudaError_t e = cudaMalloc(&out->dev, out->bytes);
@@ -152,6 +162,7 @@ cudaError_t build_axis_tables(int LL, int POL, int extra_post_Lc, AxisTables<T>*
     if (e != cudaSuccess) return e;
     for (int j = 0; j < 6; ++j) out->set.p[j] = has[j] ? reinterpret_cast<const CQ<T>*>((const T*)out->dev + off[j]) : nullptr;
     if (post) *post = extra_post_Lc > 0 ? reinterpret_cast<const CQ<T>*>((const T*)out->dev + post_off) : nullptr;
+    if (eo) *eo = eo_N > 0 ? reinterpret_cast<const CQ<T>*>((const T*)out->dev + eo_off) : nullptr;
     return cudaSuccess;
 }
 
@@ -245,6 +256,8 @@ template <typename T> struct Ctx {
     GeoV gfilm;                 // one-cell-thick meshes: geometry of the fused y stage (k_z_v FILM)
     bool film;
     bool pdl = false;           // programmatic dependent launch of the five kernels (plan.cu; DEMAG_PDL; GeoV::trig = where the next grid is let in)
+    bool zeo = false;           // fp32, Nz = 256 / 512: the z stage as two half-length two-pass transforms (k_z_eo_v; DEMAG_NO_ZEO)
+    const CQ<T>* two = nullptr; // w_Nz^z, z < Nz/2 (k_z_eo_v)
     int z16 = 0;                // fp32, Nz = 16: the z stage in registers, two lanes per column (k_z16_v; DEMAG_NO_Z16)
     bool y32 = false;           // fp32: y schedule with a radix-32 last pass where one is instantiated (YCfg32; DEMAG_NO_Y32)
     bool ylong = true;          // long y lines (Ny >= 4096) through the staged persistent kernel (DEMAG_NO_YLONG, read at plan creation)
@@ -480,6 +493,19 @@ bool z_mul(int mode, const Ctx<T>& c, cudaStream_t st, int q0, int nq, CQ<T>* W2
             else c.pf_z = c.pf_waves > 0.f ? 1 : 0;
             return true;
         }
+    }
+    if constexpr (sizeof(T) == 4) {
+#define V2_ZEO(L, TY_, NT_)                                                                                           \
+        {                                                                                                            \
+            constexpr int smem = ((1 << L) * 3 * TY_ + TY_) * (int)sizeof(CQ<T>);                                    \
+            if (mode == 0) { *err = cudaFuncSetAttribute(k_z_eo_v<T, L, TY_, NT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+                             c.pf_z = pf_distance(c.pf_waves, c.sm_count, k_z_eo_v<T, L, TY_, NT_>, NT_, smem); }    \
+            else launch_pdl(c.pdl, k_z_eo_v<T, L, TY_, NT_>, (unsigned)(nq * (c.g.Ny / TY_)), NT_, smem, st,          \
+                            with_pft(with_pf(c.g, c.pf_z), nq == c.tm_z_nq), q0, nq, W2, K, c.yslot, c.twz, c.two, c.tm_z.m); \
+            return true;                                                                                             \
+        }
+        if (c.zeo && c.lNz == 9) V2_ZEO(9, 4, 128)
+        if (c.zeo && c.lNz == 8) V2_ZEO(8, 4, 64)
     }
     switch (c.lNz) {
     case 0: if (mode) launch_pdl(c.pdl, k_z1_v<T, 0>, (unsigned)(nq * (c.g.Ny / (c.g.Ny < 128 ? c.g.Ny : 128))), c.g.Ny < 128 ? c.g.Ny : 128, 0, st, c.g, q0, nq, W2, K, c.yslot); return true;

@@ -105,6 +105,27 @@ def test_fast_and_generic_families_agree(torch, B, oracle, n, monkeypatch):
     assert np.abs(Hf - Hg).max() / Ms <= 1e-12
 
 
+@pytest.mark.parametrize("n", [(16, 32, 128), (32, 16, 256), (64, 64, 128)])
+def test_long_z_columns_both_z_kernels(torch, B, oracle, n, monkeypatch):
+    """Nz = 256 / 512 (fp32): the even / odd two-pass z kernel (k_z_eo_v, default) and the three-pass kernel it replaces
+    (DEMAG_NO_ZEO) against the oracle, and against each other at rounding level."""
+    from paper_2308_08447_b200 import workloads as W
+    h, Ms = (2e-9, 3e-9, 1e-9), 8e5
+    M = W.random_unit_vectors(n, Ms, 23)
+    T = oracle.tensor_table(n, h)
+    ref = oracle.fft_conv(T, M.astype(np.float64))
+    cells = W.sample_cells(n, 24, 5)
+    Hs = oracle.direct_sum_sampled(T, M.astype(np.float64), cells)
+    assert np.abs(ref.reshape(3, -1)[:, cells].T - Hs).max() / Ms < 1e-12       # the cross-check is Eq. (1) where sampled
+    He = _run(torch, B, n, h, T, M, 0, expect_path=1)
+    monkeypatch.setenv("DEMAG_NO_ZEO", "1")
+    H3 = _run(torch, B, n, h, T, M, 0, expect_path=1)
+    monkeypatch.delenv("DEMAG_NO_ZEO")
+    assert np.abs(He - ref).max() / Ms <= TOL32 and np.abs(H3 - ref).max() / Ms <= TOL32
+    assert np.abs(He - H3).max() / Ms <= 2e-6
+    assert not np.array_equal(He, H3)                                           # two different kernels did run
+
+
 @pytest.mark.parametrize("slab", [1, 2, 5])
 def test_fast_family_slab_size_does_not_change_result(torch, B, oracle, slab):
     from paper_2308_08447_b200 import workloads as W
