@@ -489,6 +489,8 @@ def measure(name, steps, warmup, cpu_seconds, with_cufft, with_cpu, env):
             actual[2] = "k_z1_v"
         elif Nz == 16 and not fp64 and Ny % 64 == 0:
             actual[2] = "k_z16_v"
+        elif Nz in (256, 512) and not fp64:
+            actual[2] = "k_z_eo_v"
         if Ny >= 4096 and n[2] > 1:
             actual[1] = "k_y_fwd_long_v"
     achieved = sb[dom] / (st_ms[dom] * 1e-3) / 1e9
